@@ -1,0 +1,139 @@
+/* hydro.h -- C ABI of the B200 (sm_100a) unsplit patch-group fluid solver.
+ *
+ * Hot path of Schive, Zhang & Chiueh, "Directionally Unsplit Hydrodynamic Schemes with Hybrid
+ * MPI/OpenMP/GPU Parallelization in AMR" (arXiv:1103.3373): the Riemann-solver-based,
+ * directionally unsplit update of a batch of AMR patch groups.
+ *
+ *   - unit of work: a patch group = 2x2x2 patches of 8^3 cells = 16^3 interior cells, sent to the
+ *     GPU together with its ghost zones (section 3.1; section 4.2);
+ *   - the update: steps (1)-(5) of PAPER.md:39-44 (section 2): reconstruct + half-step face values,
+ *     Riemann solve, transverse-flux correction + second Riemann solve (CTU), conservative update,
+ *     store of the fluxes across patch boundaries;
+ *   - options: schemes MHM / VL / CTU, PLM / PPM with four limiters on primitive
+ *     or characteristic variables, exact / HLLE / HLLC / Roe solvers with the Roe
+ *     failure fallback;
+ *   - the evolution time-step (a CPU task in the paper) as a device reduction.
+ *
+ * The paper gives no formulas; the exact arithmetic is fixed by DESIGN.md ("Readings").
+ *
+ * Conventions
+ *   variables   v = 0..4 : rho, rho*vx, rho*vy, rho*vz, E ; ideal gas E = P/(gamma-1) + rho|v|^2/2.
+ *   layout      x fastest, structure of arrays per group, S = 16 + 2*nghost:
+ *                 in       [Ng][5][S][S][S]            (z, y, x)
+ *                 out      [Ng][5][16][16][16]
+ *                 face_flux[Ng][9][5][16][16]          plane p = 3*d + s, d = 0,1,2 (x,y,z normal),
+ *                                                       s = 0,1,2 <-> face index f = 0, 8, 16 (the
+ *                                                       boundaries of the 8^3 patches); in-plane
+ *                                                       order d=x:[k][j], d=y:[k][i], d=z:[j][i];
+ *                                                       raw time-centred flux density (not x dt, area).
+ *   ownership   every pointer is caller-owned; the library allocates nothing, frees nothing and
+ *               keeps no state between calls (hydro_pipeline_* below owns only its own staging).
+ *               Device pointers must be 16-byte aligned; in / out / face_flux must not overlap.
+ *   async       device entry points only enqueue work on `stream` and return; no host sync.
+ *   errors      0 = success; < 0 = argument error detected on the host before any launch
+ *               (HYDRO_E_*); > 0 = cudaError_t of a failed launch.  Ng == 0 is a no-op returning 0.
+ *               Numerical trouble (non-positive rho/P, Roe failure, Newton failure) is never an
+ *               error code: it is counted in hydro_opts::status.
+ *   no fallback there is no CPU path and no other backend.
+ */
+#ifndef HYDRO_H_
+#define HYDRO_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define HYDRO_API __attribute__((visibility("default")))
+#else
+#define HYDRO_API
+#endif
+
+typedef struct CUstream_st* hydro_stream_t; /* == cudaStream_t; 0 = the legacy default stream */
+
+enum { HYDRO_MHM = 0, HYDRO_VL = 1, HYDRO_CTU = 2 };                       /* scheme */
+enum { HYDRO_EXACT = 0, HYDRO_HLLE = 1, HYDRO_HLLC = 2, HYDRO_ROE = 3 };   /* riemann */
+enum { HYDRO_GMINMOD = 0, HYDRO_VANLEER = 1, HYDRO_VANALBADA = 2, HYDRO_HYBRID = 3 }; /* limiter PAPER.md:48 */
+enum { HYDRO_PLM = 0, HYDRO_PPM = 1 };                                     /* recon */
+enum { HYDRO_IMPL_AUTO = 0, HYDRO_IMPL_STAGED = 1, HYDRO_IMPL_FUSED = 2 };
+
+enum {
+  HYDRO_OK = 0,
+  HYDRO_E_ENUM = -1,      /* scheme / riemann / limiter / recon / roe_fallback / norm / impl out of range */
+  HYDRO_E_COUNT = -2,     /* Ng < 0 */
+  HYDRO_E_NULL = -3,      /* a required pointer is NULL */
+  HYDRO_E_ALIGN = -4,     /* a device pointer is not 16-byte aligned */
+  HYDRO_E_GHOST = -5,     /* nghost < hydro_min_ghost(scheme, recon), or > 8 */
+  HYDRO_E_WORKSPACE = -6, /* staged path selected and workspace missing / smaller than one slot */
+  HYDRO_E_VALUE = -7,     /* gamma <= 1, dh <= 0, dt < 0, minmod_coeff outside [1,2], negative floor, cfl <= 0 */
+  HYDRO_E_NOFUSED = -8    /* impl == HYDRO_IMPL_FUSED and no fused kernel exists for this variant */
+};
+
+typedef struct hydro_opts {      /* NULL => all defaults */
+  int recon;            /* HYDRO_PLM (default) / HYDRO_PPM */
+  int nghost;           /* ghost width of `in`; 0 => hydro_min_ghost(scheme, recon)                  */
+  int char_limit;       /* 0 limit primitive variables (default), 1 characteristic */
+  float minmod_coeff;   /* theta in [1,2] of the generalized minmod limiter; 0 => 1.5                */
+  int roe_fallback;     /* solver used at a face where Roe fails: 0/1 HLLE, 2 HLLC, 3 exact PAPER.md:50 */
+  double min_dens;      /* density floor, 0 => none (default)                                        */
+  double min_pres;      /* pressure floor, 0 => none (default)                                       */
+  long long* status;    /* device long long[3] or NULL; accumulated atomically:
+                           [0] Roe failures, [1] non-positive rho or P seen by a conversion,
+                           [2] exact-solver vacuum / non-convergence                                 */
+  void* workspace;      /* device scratch for the staged path (hydro_workspace_bytes); else NULL     */
+  size_t workspace_bytes;
+  int impl;             /* HYDRO_IMPL_AUTO: fused z-marching kernel when one exists, else staged     */
+  const void* max_speed;/* device scalar (float / double as the call) or NULL.  If set, the `dt` argument is
+                           ignored and dt/dh = cfl / *max_speed is formed on the device, so that
+                           hydro_dt -> hydro_solve stays asynchronous (no host read of the reduction)   */
+  double cfl;           /* CFL number used with max_speed (> 0)                                       */
+} hydro_opts;
+
+/* One unsplit update of Ng patch groups.  in/out/face_flux: device pointers,
+ * layouts above; face_flux may be NULL (step (5) skipped).  dt, dh, gamma: one value per call (a batch
+ * belongs to one AMR level). */
+HYDRO_API int hydro_solve_f32(const float* in, float* out, float* face_flux, int Ng, float dt, float dh, float gamma,
+                    int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream);
+HYDRO_API int hydro_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma,
+                    int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream);
+
+/* Evolution time-step reduction: maximum over the INTERIOR cells of all groups of
+ *   norm 0: max_d |v_d| + c        norm 1: sum_d |v_d| + 3 c ,   c = sqrt(gamma P / rho).
+ * u has the layout of `in` with ghost width nghost (>= 0).  *max_speed (device scalar) is overwritten;
+ * it is NaN if any interior cell has non-positive rho or P.  The caller forms dt = CFL*dh / *max_speed. */
+HYDRO_API int hydro_dt_f32(const float* u, int Ng, int nghost, float gamma, int norm, float* max_speed, hydro_stream_t stream);
+HYDRO_API int hydro_dt_f64(const double* u, int Ng, int nghost, double gamma, int norm, double* max_speed, hydro_stream_t stream);
+
+/* Host-buffer entry points (the paper's asynchronous-copy pipeline: `nstreams`
+ * CUDA streams, each cycling chunks of `groups_per_chunk` patch groups through H2D copy -> kernel ->
+ * D2H copy so that transfers overlap the solver).  The pipeline object owns its device staging
+ * buffers and streams; in/out/face_flux are HOST pointers (pinned memory gives real overlap) and the
+ * call returns after all results are in `out` / `face_flux`.  opts->workspace/status/max_speed are
+ * ignored; status counters, if wanted, are returned in status_host[3] (host, may be NULL).
+ * max_speed_host (host scalar, may be NULL) receives the hydro_dt reduction (norm 0) of the UPDATED
+ * state, computed chunk by chunk while the data is still on the device: the next step's dt. */
+typedef struct hydro_pipeline hydro_pipeline;
+HYDRO_API int hydro_pipeline_create(hydro_pipeline** p, int precision_bytes, int nghost, int groups_per_chunk, int nstreams);
+HYDRO_API void hydro_pipeline_destroy(hydro_pipeline* p);
+HYDRO_API int hydro_pipeline_solve_f32(hydro_pipeline* p, const float* in, float* out, float* face_flux, int Ng, float dt,
+                             float dh, float gamma, int scheme, int riemann, int limiter, const hydro_opts* opts,
+                             long long* status_host, float* max_speed_host);
+HYDRO_API int hydro_pipeline_solve_f64(hydro_pipeline* p, const double* in, double* out, double* face_flux, int Ng, double dt,
+                             double dh, double gamma, int scheme, int riemann, int limiter, const hydro_opts* opts,
+                             long long* status_host, double* max_speed_host);
+
+/* Sizes and capabilities. */
+HYDRO_API int hydro_min_ghost(int scheme, int recon);                 /* 2/3 (MHM, CTU with PLM/PPM), 3/4 (VL)   */
+HYDRO_API int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann); /* 1 if a fused kernel exists */
+/* bytes of opts->workspace needed by hydro_solve_* in HYDRO_IMPL_AUTO mode (0 when the fused kernel runs) */
+HYDRO_API size_t hydro_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon);
+/* bytes needed when HYDRO_IMPL_STAGED is forced */
+HYDRO_API size_t hydro_staged_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon);
+HYDRO_API const char* hydro_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HYDRO_H_ */

@@ -1,0 +1,228 @@
+"""Thin ctypes binding of include/hydro.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of libhydro.so; PyTorch supplies device memory
+and streams.  There is no CPU fallback: if the library cannot be built or loaded, importing the
+entry points raises.  Names follow the C ABI: hydro_solve, hydro_dt, hydro_min_ghost,
+hydro_has_fused, hydro_workspace_bytes, hydro_strerror, HydroPipeline (hydro_pipeline_*).
+"""
+import ctypes as C
+import os
+
+import torch  # loads libcudart before libhydro.so is opened
+
+from . import build as _build
+
+MHM, VL, CTU = 0, 1, 2
+EXACT, HLLE, HLLC, ROE = 0, 1, 2, 3
+GMINMOD, VANLEER, VANALBADA, HYBRID = 0, 1, 2, 3
+PLM, PPM = 0, 1
+IMPL_AUTO, IMPL_STAGED, IMPL_FUSED = 0, 1, 2
+PS = 16
+
+EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64", "hydro_pipeline_create",
+           "hydro_pipeline_destroy", "hydro_pipeline_solve_f32", "hydro_pipeline_solve_f64", "hydro_min_ghost",
+           "hydro_has_fused", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror")
+
+
+class HydroOpts(C.Structure):
+    _fields_ = [("recon", C.c_int), ("nghost", C.c_int), ("char_limit", C.c_int), ("minmod_coeff", C.c_float),
+                ("roe_fallback", C.c_int), ("min_dens", C.c_double), ("min_pres", C.c_double),
+                ("status", C.c_void_p), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+                ("impl", C.c_int), ("max_speed", C.c_void_p), ("cfl", C.c_double)]
+
+
+class HydroError(RuntimeError):
+    def __init__(self, code, what):
+        super().__init__(f"{what}: {hydro_strerror(code)} (code {code})")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load (building if stale) libhydro.so.  Raises if nvcc / the library is unavailable."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if os.environ.get("HYDRO_NO_BUILD") != "1" or not os.path.exists(path):
+            path = _build.build()
+        L = C.CDLL(path)
+        vp, i, sz = C.c_void_p, C.c_int, C.c_size_t
+        for name, ft in (("f32", C.c_float), ("f64", C.c_double)):
+            getattr(L, "hydro_solve_" + name).argtypes = [vp, vp, vp, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
+            getattr(L, "hydro_dt_" + name).argtypes = [vp, i, i, ft, i, vp, vp]
+            getattr(L, "hydro_pipeline_solve_" + name).argtypes = [vp, vp, vp, vp, i, ft, ft, ft, i, i, i,
+                                                                   C.POINTER(HydroOpts), vp, vp]
+        L.hydro_pipeline_create.argtypes = [C.POINTER(vp), i, i, i, i]
+        L.hydro_pipeline_destroy.argtypes = [vp]
+        L.hydro_pipeline_destroy.restype = None
+        L.hydro_min_ghost.argtypes = [i, i]
+        L.hydro_has_fused.argtypes = [i, i, i, i]
+        L.hydro_workspace_bytes.argtypes = [i, i, i, i]
+        L.hydro_workspace_bytes.restype = sz
+        L.hydro_staged_workspace_bytes.argtypes = [i, i, i, i]
+        L.hydro_staged_workspace_bytes.restype = sz
+        L.hydro_strerror.argtypes = [i]
+        L.hydro_strerror.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def hydro_strerror(code):
+    return lib().hydro_strerror(int(code)).decode()
+
+
+def hydro_min_ghost(scheme, recon=PLM):
+    return lib().hydro_min_ghost(scheme, recon)
+
+
+def hydro_has_fused(dtype, scheme, recon=PLM, riemann=ROE):
+    return bool(lib().hydro_has_fused(torch.empty((), dtype=dtype).element_size(), scheme, recon, riemann))
+
+
+def hydro_workspace_bytes(Ng, dtype, scheme, recon=PLM, impl=IMPL_AUTO):
+    es = torch.empty((), dtype=dtype).element_size()
+    if impl == IMPL_STAGED:
+        return lib().hydro_staged_workspace_bytes(Ng, es, scheme, recon)
+    return lib().hydro_workspace_bytes(Ng, es, scheme, recon)
+
+
+_ws_cache = {}
+
+
+def _workspace(nbytes, device):
+    """Caller-owned scratch for the staged path, cached per device and grown on demand."""
+    if nbytes == 0:
+        return None
+    w = _ws_cache.get(device)
+    if w is None or w.numel() < nbytes:
+        w = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        _ws_cache[device] = w
+    return w
+
+
+def _suffix(t):
+    if t.dtype == torch.float32:
+        return "f32", C.c_float
+    if t.dtype == torch.float64:
+        return "f64", C.c_double
+    raise TypeError("hydro: dtype must be float32 or float64")
+
+
+def make_opts(*, recon=PLM, nghost=0, char_limit=0, minmod_coeff=0.0, roe_fallback=0, min_dens=0.0, min_pres=0.0,
+              status=None, workspace=None, impl=IMPL_AUTO, max_speed=None, cfl=0.0):
+    o = HydroOpts()
+    o.recon, o.nghost, o.char_limit, o.minmod_coeff, o.roe_fallback = recon, nghost, char_limit, minmod_coeff, roe_fallback
+    o.min_dens, o.min_pres, o.impl = min_dens, min_pres, impl
+    o.max_speed = max_speed.data_ptr() if max_speed is not None else None
+    o.cfl = cfl
+    o.status = status.data_ptr() if status is not None else None
+    o.workspace = workspace.data_ptr() if workspace is not None else None
+    o.workspace_bytes = workspace.numel() * workspace.element_size() if workspace is not None else 0
+    return o
+
+
+def hydro_solve(in_, dt, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, out=None, face_flux=True,
+                status=None, stream=None, **optkw):
+    """hydro_solve_f32/f64 on CUDA tensors.  in_[Ng,5,S,S,S]; returns (out[Ng,5,16,16,16], face_flux or None).
+
+    face_flux: True -> allocate, False/None -> skip step (5), or a tensor [Ng,9,5,16,16] to fill.
+    status: optional int64 CUDA tensor [3], accumulated.  Asynchronous on `stream` (default: current).
+    max_speed=<device scalar from hydro_dt>, cfl=<number>: dt is formed on the device and `dt` is ignored.
+    """
+    if not in_.is_cuda:
+        raise ValueError("hydro_solve: `in_` must be a CUDA tensor (host buffers go through HydroPipeline)")
+    if not in_.is_contiguous() or in_.dim() != 5 or in_.shape[1] != 5:
+        raise ValueError("hydro_solve: in_ must be contiguous [Ng,5,S,S,S]")
+    sfx, ft = _suffix(in_)
+    Ng, S = in_.shape[0], in_.shape[2]
+    g = (S - PS) // 2
+    if tuple(in_.shape[2:]) != (S, S, S) or S != PS + 2 * g:
+        raise ValueError("hydro_solve: bad padded shape")
+    if out is None:
+        out = torch.empty((Ng, 5, PS, PS, PS), dtype=in_.dtype, device=in_.device)
+    if face_flux is True:
+        face_flux = torch.empty((Ng, 9, 5, PS, PS), dtype=in_.dtype, device=in_.device)
+    elif face_flux is False:
+        face_flux = None
+    for t in (out, face_flux):
+        if t is not None and (t.dtype != in_.dtype or t.device != in_.device or not t.is_contiguous()):
+            raise ValueError("hydro_solve: out / face_flux must match in_ (dtype, device) and be contiguous")
+    recon = optkw.get("recon", PLM)
+    impl = optkw.get("impl", IMPL_AUTO)
+    ws = optkw.pop("workspace", None)
+    if ws is None:
+        ws = _workspace(hydro_workspace_bytes(Ng, in_.dtype, scheme, recon, impl), in_.device)
+    o = make_opts(nghost=g, status=status, workspace=ws, **optkw)
+    st = (stream or torch.cuda.current_stream(in_.device)).cuda_stream
+    with torch.cuda.device(in_.device):
+        rc = getattr(lib(), "hydro_solve_" + sfx)(in_.data_ptr(), out.data_ptr(),
+                                                  face_flux.data_ptr() if face_flux is not None else None, Ng,
+                                                  ft(dt), ft(dh), ft(gamma), scheme, riemann, limiter, C.byref(o), st)
+    if rc != 0:
+        raise HydroError(rc, "hydro_solve_" + sfx)
+    return out, face_flux
+
+
+def hydro_dt(u, gamma, norm=0, *, max_speed=None, stream=None):
+    """hydro_dt_f32/f64: device scalar tensor holding the maximum wave speed over interior cells."""
+    if not u.is_cuda or not u.is_contiguous() or u.dim() != 5 or u.shape[1] != 5:
+        raise ValueError("hydro_dt: u must be a contiguous CUDA tensor [Ng,5,S,S,S]")
+    sfx, ft = _suffix(u)
+    Ng, S = u.shape[0], u.shape[2]
+    g = (S - PS) // 2
+    if max_speed is None:
+        max_speed = torch.empty((), dtype=u.dtype, device=u.device)
+    st = (stream or torch.cuda.current_stream(u.device)).cuda_stream
+    with torch.cuda.device(u.device):
+        rc = getattr(lib(), "hydro_dt_" + sfx)(u.data_ptr(), Ng, g, ft(gamma), norm, max_speed.data_ptr(), st)
+    if rc != 0:
+        raise HydroError(rc, "hydro_dt_" + sfx)
+    return max_speed
+
+
+class HydroPipeline:
+    """hydro_pipeline_*: host buffers in, host buffers out, chunks streamed over `nstreams` CUDA streams
+    (PAPER.md:107, 123).  Tensors passed to solve() are CPU tensors (pinned for real overlap)."""
+
+    def __init__(self, dtype, nghost, groups_per_chunk=256, nstreams=4, device=None):
+        self.dtype = dtype
+        self.g = nghost
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self._h = C.c_void_p()
+        es = torch.empty((), dtype=dtype).element_size()
+        with torch.cuda.device(self.device):
+            rc = lib().hydro_pipeline_create(C.byref(self._h), es, nghost, groups_per_chunk, nstreams)
+        if rc != 0:
+            raise HydroError(rc, "hydro_pipeline_create")
+
+    def solve(self, in_, out, face_flux, dt, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, status=None,
+              max_speed=None, **optkw):
+        """status: CPU int64 tensor [3] or None; max_speed: CPU scalar tensor of in_.dtype or None (receives the
+        wave-speed maximum of the updated state)."""
+        if in_.is_cuda or out.is_cuda or (face_flux is not None and face_flux.is_cuda):
+            raise ValueError("HydroPipeline.solve takes host tensors")
+        sfx, ft = _suffix(in_)
+        Ng = in_.shape[0]
+        o = make_opts(nghost=self.g, **optkw)
+        with torch.cuda.device(self.device):
+            rc = getattr(lib(), "hydro_pipeline_solve_" + sfx)(
+                self._h, in_.data_ptr(), out.data_ptr(), face_flux.data_ptr() if face_flux is not None else None, Ng,
+                ft(dt), ft(dh), ft(gamma), scheme, riemann, limiter, C.byref(o),
+                status.data_ptr() if status is not None else None,
+                max_speed.data_ptr() if max_speed is not None else None)
+        if rc != 0:
+            raise HydroError(rc, "hydro_pipeline_solve_" + sfx)
+        return out, face_flux
+
+    def close(self):
+        if self._h:
+            lib().hydro_pipeline_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,431 @@
+// hydro_api.cu -- the C ABI of include/hydro.h: argument validation, variant dispatch, the
+// hydro_dt reduction kernel and the host-buffer streaming pipeline.
+#include <cuda_runtime.h>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/hydro.h"
+#include "hydro_launch.cuh"
+
+namespace hydro {
+
+// ---- dispatch tables ---------------------------------------------------------------------------
+#define DECL_STAGED(R, S, RC, RS) extern template cudaError_t launch_staged<R, S, RC, RS>(const SolveArgs<R>&);
+#define DECL_FUSED(R, S, RC, RS) extern template cudaError_t launch_fused<R, S, RC, RS>(const SolveArgs<R>&);
+#define FOR_RS(M, R, S, RC) M(R, S, RC, RS_EXACT) M(R, S, RC, RS_HLLE) M(R, S, RC, RS_HLLC) M(R, S, RC, RS_ROE)
+#define FOR_RC(M, R, S) FOR_RS(M, R, S, RECON_PLM) FOR_RS(M, R, S, RECON_PPM)
+#define FOR_S(M, R) FOR_RC(M, R, SCHEME_MHM) FOR_RC(M, R, SCHEME_VL) FOR_RC(M, R, SCHEME_CTU)
+FOR_S(DECL_STAGED, float)
+FOR_S(DECL_STAGED, double)
+FOR_S(DECL_FUSED, float)
+FOR_S(DECL_FUSED, double)
+
+template <class R> static LaunchFn<R> staged_fn(int scheme, int recon, int rs) {
+#define ROW(R_, S, RC) {&launch_staged<R_, S, RC, RS_EXACT>, &launch_staged<R_, S, RC, RS_HLLE>, \
+                        &launch_staged<R_, S, RC, RS_HLLC>, &launch_staged<R_, S, RC, RS_ROE>}
+  static const LaunchFn<R> t[3][2][4] = {
+      {ROW(R, SCHEME_MHM, RECON_PLM), ROW(R, SCHEME_MHM, RECON_PPM)},
+      {ROW(R, SCHEME_VL, RECON_PLM), ROW(R, SCHEME_VL, RECON_PPM)},
+      {ROW(R, SCHEME_CTU, RECON_PLM), ROW(R, SCHEME_CTU, RECON_PPM)}};
+#undef ROW
+  return t[scheme][recon][rs];
+}
+template <class R> static LaunchFn<R> fused_fn(int scheme, int recon, int rs) {
+#define ROW(R_, S, RC) {&launch_fused<R_, S, RC, RS_EXACT>, &launch_fused<R_, S, RC, RS_HLLE>, \
+                        &launch_fused<R_, S, RC, RS_HLLC>, &launch_fused<R_, S, RC, RS_ROE>}
+  static const LaunchFn<R> t[3][2][4] = {
+      {ROW(R, SCHEME_MHM, RECON_PLM), ROW(R, SCHEME_MHM, RECON_PPM)},
+      {ROW(R, SCHEME_VL, RECON_PLM), ROW(R, SCHEME_VL, RECON_PPM)},
+      {ROW(R, SCHEME_CTU, RECON_PLM), ROW(R, SCHEME_CTU, RECON_PPM)}};
+#undef ROW
+  return t[scheme][recon][rs];
+}
+
+// ---- hydro_dt (DESIGN.md c6) -------------------------------------------------------
+// Non-negative IEEE values order like their bit patterns, and the canonical NaN pattern is larger
+// than +inf, so one integer atomicMax per CTA yields "max, or NaN if any cell was bad".
+template <class R> struct Bits;
+template <> struct Bits<float> {
+  using U = unsigned int;
+  static __device__ __forceinline__ U of(float x) { return __float_as_uint(x); }
+  static __device__ __forceinline__ U nan() { return 0x7fc00000u; }
+};
+template <> struct Bits<double> {
+  using U = unsigned long long;
+  static __device__ __forceinline__ U of(double x) { return (U)__double_as_longlong(x); }
+  static __device__ __forceinline__ U nan() { return 0x7ff8000000000000ull; }
+};
+
+constexpr int DT_NT = 256;
+constexpr int DT_ROWS_PER_THREAD = 4;  // independent 16-cell rows in flight per half-warp
+
+template <class R>
+__global__ void __launch_bounds__(DT_NT) dt_kernel(const R* __restrict__ u, long long nrows, int g, R gamma, int norm,
+                                                   typename Bits<R>::U* __restrict__ result) {
+  using U = typename Bits<R>::U;
+  const int S = PS + 2 * g;
+  const size_t nS = (size_t)S * S * S;
+  const int lane16 = threadIdx.x & 15;
+  const long long hw = ((long long)blockIdx.x * DT_NT + threadIdx.x) >> 4;  // global half-warp id
+  const long long nhw = ((long long)gridDim.x * DT_NT) >> 4;
+  U best = 0;
+  // a "row" = the 16 interior cells (fixed j,k) of one group: 16 consecutive elements per variable
+  for (long long r0 = hw * DT_ROWS_PER_THREAD; r0 < nrows; r0 += nhw * DT_ROWS_PER_THREAD) {
+    R v[DT_ROWS_PER_THREAD][5];
+#pragma unroll
+    for (int t = 0; t < DT_ROWS_PER_THREAD; ++t) {
+      const long long r = r0 + t;
+      if (r < nrows) {
+        const long long grp = r >> 8;
+        const int j = (int)(r & 15), k = (int)((r >> 4) & 15);
+        const R* b = u + (size_t)grp * 5 * nS + ((size_t)(k + g) * S + (j + g)) * S + g + lane16;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) v[t][q] = __ldg(b + q * nS);
+      } else {
+        v[t][0] = R(1); v[t][1] = v[t][2] = v[t][3] = R(0); v[t][4] = R(1);
+      }
+    }
+#pragma unroll
+    for (int t = 0; t < DT_ROWS_PER_THREAD; ++t) {
+      const R rho = v[t][0], ir = R(1) / rho;
+      const R vx = v[t][1] * ir, vy = v[t][2] * ir, vz = v[t][3] * ir;
+      const R P = (gamma - R(1)) * (v[t][4] - R(0.5) * rho * ((vx * vx + vy * vy) + vz * vz));
+      const R c = m_sqrt(gamma * P * ir);
+      const R ax = m_abs(vx), ay = m_abs(vy), az = m_abs(vz);
+      const R s = norm == 0 ? m_max(m_max(ax, ay), az) + c : ((ax + ay) + az) + R(3) * c;
+      const bool bad = !(rho > R(0)) || !(P > R(0)) || !(s == s);
+      const U bits = bad ? Bits<R>::nan() : Bits<R>::of(s);
+      best = bits > best ? bits : best;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const U other = __shfl_xor_sync(0xffffffffu, best, o);
+    best = other > best ? other : best;
+  }
+  __shared__ U wmax[DT_NT / 32];
+  if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    U m = wmax[0];
+#pragma unroll
+    for (int w = 1; w < DT_NT / 32; ++w) m = wmax[w] > m ? wmax[w] : m;
+    atomicMax(result, m);
+  }
+}
+
+static int g_sm_count = 0;
+static int sm_count() {
+  if (!g_sm_count) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+      g_sm_count = n;
+    else
+      g_sm_count = 148;
+  }
+  return g_sm_count;
+}
+
+template <class R>
+static int dt_impl(const R* u, int Ng, int nghost, R gamma, int norm, R* max_speed, cudaStream_t st, bool accumulate = false) {
+  if (Ng < 0) return HYDRO_E_COUNT;
+  if (!max_speed || (Ng > 0 && !u)) return HYDRO_E_NULL;
+  if (norm < 0 || norm > 1) return HYDRO_E_ENUM;
+  if (nghost < 0 || nghost > 8) return HYDRO_E_GHOST;
+  if (!(gamma > R(1))) return HYDRO_E_VALUE;
+  if (((uintptr_t)u & 15) || ((uintptr_t)max_speed & (sizeof(R) - 1))) return HYDRO_E_ALIGN;
+  if (!accumulate) {
+    cudaError_t e = cudaMemsetAsync(max_speed, 0, sizeof(R), st);
+    if (e != cudaSuccess) return (int)e;
+  }
+  if (Ng == 0) return HYDRO_OK;
+  const long long nrows = (long long)Ng * PS * PS;
+  long long blocks = (nrows * 16 / DT_ROWS_PER_THREAD + DT_NT - 1) / DT_NT;
+  const long long cap = (long long)sm_count() * 8;
+  if (blocks > cap) blocks = cap;
+  dt_kernel<R><<<(unsigned)blocks, DT_NT, 0, st>>>(u, nrows, nghost, gamma, norm,
+                                                  reinterpret_cast<typename Bits<R>::U*>(max_speed));
+  return (int)cudaGetLastError();
+}
+
+// ---- hydro_solve ---------------------------------------------------------------------------------
+struct Plan {
+  int recon, g, impl;  // impl resolved to STAGED or FUSED
+};
+
+template <class R>
+static int make_plan(const void* in, const void* out, const void* ff, int Ng, R dt, R dh, R gamma, int scheme, int riemann,
+                     int limiter, const hydro_opts* o, bool device_ptrs, Par<R>& par, Plan& pl) {
+  if (scheme < 0 || scheme > 2 || riemann < 0 || riemann > 3 || limiter < 0 || limiter > 3) return HYDRO_E_ENUM;
+  const int recon = o ? o->recon : 0;
+  const int fb = (o && o->roe_fallback) ? o->roe_fallback : 1;
+  const int impl = o ? o->impl : 0;
+  if (recon < 0 || recon > 1 || fb < 1 || fb > 3 || impl < 0 || impl > 2) return HYDRO_E_ENUM;
+  if (o && (o->char_limit < 0 || o->char_limit > 1)) return HYDRO_E_ENUM;
+  if (Ng < 0) return HYDRO_E_COUNT;
+  if (Ng > 0 && (!in || !out)) return HYDRO_E_NULL;
+  if (device_ptrs && (((uintptr_t)in & 15) || ((uintptr_t)out & 15) || ((uintptr_t)ff & 15))) return HYDRO_E_ALIGN;
+  if (device_ptrs && o && o->status && ((uintptr_t)o->status & 7)) return HYDRO_E_ALIGN;
+  const int gmin = min_ghost(scheme, recon);
+  const int g = (o && o->nghost) ? o->nghost : gmin;
+  if (g < gmin || g > 8) return HYDRO_E_GHOST;
+  const double theta = (o && o->minmod_coeff != 0.0f) ? (double)o->minmod_coeff : 1.5;
+  if (!(gamma > R(1)) || !(dh > R(0)) || !(dt >= R(0)) || !(theta >= 1.0 && theta <= 2.0)) return HYDRO_E_VALUE;
+  if (o && (!(o->min_dens >= 0.0) || !(o->min_pres >= 0.0))) return HYDRO_E_VALUE;
+  if (o && o->max_speed && (!(o->cfl > 0.0) || ((uintptr_t)o->max_speed & (sizeof(R) - 1)))) return HYDRO_E_VALUE;
+  par.gamma = gamma;
+  par.gm1 = gamma - R(1);
+  par.nu = dt / dh;
+  par.hnu = R(0.5) * par.nu;
+  par.theta = (R)theta;
+  par.min_dens = o ? (R)o->min_dens : R(0);
+  par.min_pres = o ? (R)o->min_pres : R(0);
+  par.limiter = limiter;
+  par.char_limit = o ? o->char_limit : 0;
+  par.roe_fallback = fb;
+  const bool has = hydro_has_fused((int)sizeof(R), scheme, recon, riemann) != 0;
+  if (impl == HYDRO_IMPL_FUSED && !has) return HYDRO_E_NOFUSED;
+  pl.recon = recon;
+  pl.g = g;
+  pl.impl = (impl == HYDRO_IMPL_STAGED || !has) ? HYDRO_IMPL_STAGED : HYDRO_IMPL_FUSED;
+  return HYDRO_OK;
+}
+
+template <class R>
+static int solve_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, int scheme, int riemann, int limiter,
+                      const hydro_opts* o, cudaStream_t st) {
+  SolveArgs<R> a;
+  Plan pl;
+  const int rc = make_plan<R>(in, out, ff, Ng, dt, dh, gamma, scheme, riemann, limiter, o, true, a.par, pl);
+  if (rc != HYDRO_OK) return rc;
+  if (Ng == 0) return HYDRO_OK;
+  a.in = in;
+  a.out = out;
+  a.face_flux = ff;
+  a.Ng = Ng;
+  a.g = pl.g;
+  a.max_speed = o ? static_cast<const R*>(o->max_speed) : nullptr;
+  a.cfl = o ? (R)o->cfl : R(0);
+  a.status = o ? o->status : nullptr;
+  a.workspace = o ? o->workspace : nullptr;
+  a.workspace_bytes = o ? o->workspace_bytes : 0;
+  a.stream = st;
+  if (pl.impl == HYDRO_IMPL_STAGED) {
+    if (!a.workspace || ((uintptr_t)a.workspace & 15) || a.workspace_bytes < staged_slot_bytes(scheme, pl.recon, sizeof(R)))
+      return HYDRO_E_WORKSPACE;
+    return (int)staged_fn<R>(scheme, pl.recon, riemann)(a);
+  }
+  return (int)fused_fn<R>(scheme, pl.recon, riemann)(a);
+}
+
+}  // namespace hydro
+
+// ---- the host-buffer streaming pipeline ---------------------------------------
+struct hydro_pipeline {
+  int prec, g, chunk, ns;
+  size_t in_elems, out_elems, ff_elems;  // per group
+  std::vector<cudaStream_t> streams;
+  std::vector<void*> d_in, d_out, d_ff, d_ws;
+  size_t ws_bytes;
+  long long* d_status;
+  void* d_speed;  // [ns] per-stream running maxima of the updated state's wave speed
+};
+
+namespace hydro {
+template <class R>
+static int pipeline_solve(hydro_pipeline* p, const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, int scheme, int riemann,
+                          int limiter, const hydro_opts* o, long long* status_host, R* max_speed_host) {
+  if (!p) return HYDRO_E_NULL;
+  if (p->prec != (int)sizeof(R)) return HYDRO_E_VALUE;
+  hydro_opts oo;
+  if (o) oo = *o; else std::memset(&oo, 0, sizeof(oo));
+  oo.nghost = p->g;
+  oo.status = status_host ? p->d_status : nullptr;
+  oo.max_speed = nullptr;
+  Par<R> par;
+  Plan pl;
+  int rc = make_plan<R>(in, out, ff, Ng, dt, dh, gamma, scheme, riemann, limiter, &oo, false, par, pl);
+  if (rc != HYDRO_OK) return rc;
+  if (Ng == 0) return HYDRO_OK;
+  if (pl.impl == HYDRO_IMPL_STAGED) {
+    const size_t need = hydro_staged_workspace_bytes(p->chunk, p->prec, scheme, pl.recon);
+    if (p->ws_bytes < need) {  // (re)allocate per-stream scratch once for this variant
+      for (auto& w : p->d_ws) { if (w) cudaFree(w); w = nullptr; }
+      for (auto& w : p->d_ws) if (cudaMalloc(&w, need) != cudaSuccess) return (int)cudaErrorMemoryAllocation;
+      p->ws_bytes = need;
+    }
+  }
+  if (status_host) cudaMemsetAsync(p->d_status, 0, 3 * sizeof(long long), p->streams[0]);
+  if (max_speed_host) cudaMemsetAsync(p->d_speed, 0, p->ns * sizeof(double), p->streams[0]);
+  if (status_host || max_speed_host) cudaStreamSynchronize(p->streams[0]);
+  int s = 0;
+  for (int n0 = 0; n0 < Ng; n0 += p->chunk, s = (s + 1) % p->ns) {
+    const int n = (Ng - n0 < p->chunk) ? Ng - n0 : p->chunk;
+    cudaStream_t st = p->streams[s];
+    cudaError_t e = cudaMemcpyAsync(p->d_in[s], in + (size_t)n0 * p->in_elems, (size_t)n * p->in_elems * sizeof(R),
+                                    cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return (int)e;
+    oo.workspace = p->d_ws[s];
+    oo.workspace_bytes = p->ws_bytes;
+    rc = solve_impl<R>((const R*)p->d_in[s], (R*)p->d_out[s], ff ? (R*)p->d_ff[s] : nullptr, n, dt, dh, gamma, scheme,
+                       riemann, limiter, &oo, st);
+    if (rc != HYDRO_OK) return rc;
+    if (max_speed_host) {  // next step's CFL reduction while the chunk is still on the device
+      rc = dt_impl<R>((const R*)p->d_out[s], n, 0, gamma, 0, reinterpret_cast<R*>(static_cast<double*>(p->d_speed) + s), st, true);
+      if (rc != HYDRO_OK) return rc;
+    }
+    e = cudaMemcpyAsync(out + (size_t)n0 * p->out_elems, p->d_out[s], (size_t)n * p->out_elems * sizeof(R),
+                        cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return (int)e;
+    if (ff) {
+      e = cudaMemcpyAsync(ff + (size_t)n0 * p->ff_elems, p->d_ff[s], (size_t)n * p->ff_elems * sizeof(R),
+                          cudaMemcpyDeviceToHost, st);
+      if (e != cudaSuccess) return (int)e;
+    }
+  }
+  for (auto st : p->streams) {
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return (int)e;
+  }
+  if (status_host) {
+    cudaError_t e = cudaMemcpy(status_host, p->d_status, 3 * sizeof(long long), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return (int)e;
+  }
+  if (max_speed_host) {
+    double h[16];
+    cudaError_t e = cudaMemcpy(h, p->d_speed, p->ns * sizeof(double), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return (int)e;
+    R m = R(0);
+    for (int i = 0; i < p->ns; ++i) {
+      R v;
+      std::memcpy(&v, &h[i], sizeof(R));
+      m = (v != v || m != m) ? (R)NAN : (v > m ? v : m);
+    }
+    *max_speed_host = m;
+  }
+  return HYDRO_OK;
+}
+}  // namespace hydro
+
+extern "C" {
+
+int hydro_min_ghost(int scheme, int recon) {
+  if (scheme < 0 || scheme > 2 || recon < 0 || recon > 1) return HYDRO_E_ENUM;
+  return hydro::min_ghost(scheme, recon);
+}
+
+int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann) {
+  if (scheme < 0 || scheme > 2 || recon < 0 || recon > 1 || riemann < 0 || riemann > 3) return 0;
+  if (precision_bytes != 4 && precision_bytes != 8) return 0;
+  return hydro::fused_available(precision_bytes, scheme, recon) ? 1 : 0;
+}
+
+size_t hydro_staged_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon) {
+  if (scheme < 0 || scheme > 2 || recon < 0 || recon > 1 || Ng <= 0) return 0;
+  if (precision_bytes != 4 && precision_bytes != 8) return 0;
+  const size_t slots = Ng < hydro::STAGED_MAX_SLOTS ? (size_t)Ng : (size_t)hydro::STAGED_MAX_SLOTS;
+  return slots * hydro::staged_slot_bytes(scheme, recon, (size_t)precision_bytes);
+}
+
+size_t hydro_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon) {
+  if (hydro_has_fused(precision_bytes, scheme, recon, 0)) return 0;
+  return hydro_staged_workspace_bytes(Ng, precision_bytes, scheme, recon);
+}
+
+const char* hydro_strerror(int code) {
+  switch (code) {
+    case HYDRO_OK: return "success";
+    case HYDRO_E_ENUM: return "enum argument out of range";
+    case HYDRO_E_COUNT: return "negative group count";
+    case HYDRO_E_NULL: return "required pointer is NULL";
+    case HYDRO_E_ALIGN: return "device pointer not 16-byte aligned";
+    case HYDRO_E_GHOST: return "ghost width smaller than the scheme needs (or > 8)";
+    case HYDRO_E_WORKSPACE: return "staged path needs opts->workspace of hydro_workspace_bytes()";
+    case HYDRO_E_VALUE: return "scalar argument out of range";
+    case HYDRO_E_NOFUSED: return "no fused kernel for this variant";
+    default: return code > 0 ? cudaGetErrorString((cudaError_t)code) : "unknown hydro error";
+  }
+}
+
+int hydro_solve_f32(const float* in, float* out, float* face_flux, int Ng, float dt, float dh, float gamma, int scheme,
+                    int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream) {
+  return hydro::solve_impl<float>(in, out, face_flux, Ng, dt, dh, gamma, scheme, riemann, limiter, opts, (cudaStream_t)stream);
+}
+int hydro_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int scheme,
+                    int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream) {
+  return hydro::solve_impl<double>(in, out, face_flux, Ng, dt, dh, gamma, scheme, riemann, limiter, opts, (cudaStream_t)stream);
+}
+int hydro_dt_f32(const float* u, int Ng, int nghost, float gamma, int norm, float* max_speed, hydro_stream_t stream) {
+  return hydro::dt_impl<float>(u, Ng, nghost, gamma, norm, max_speed, (cudaStream_t)stream);
+}
+int hydro_dt_f64(const double* u, int Ng, int nghost, double gamma, int norm, double* max_speed, hydro_stream_t stream) {
+  return hydro::dt_impl<double>(u, Ng, nghost, gamma, norm, max_speed, (cudaStream_t)stream);
+}
+
+int hydro_pipeline_create(hydro_pipeline** pp, int precision_bytes, int nghost, int groups_per_chunk, int nstreams) {
+  if (!pp) return HYDRO_E_NULL;
+  *pp = nullptr;
+  if (precision_bytes != 4 && precision_bytes != 8) return HYDRO_E_VALUE;
+  if (nghost < 2 || nghost > 8) return HYDRO_E_GHOST;
+  if (groups_per_chunk < 1 || nstreams < 1 || nstreams > 16) return HYDRO_E_VALUE;
+  hydro_pipeline* p = new (std::nothrow) hydro_pipeline();
+  if (!p) return (int)cudaErrorMemoryAllocation;
+  p->prec = precision_bytes;
+  p->g = nghost;
+  p->chunk = groups_per_chunk;
+  p->ns = nstreams;
+  const size_t S = hydro::PS + 2 * nghost;
+  p->in_elems = 5 * S * S * S;
+  p->out_elems = 5 * (size_t)hydro::PS * hydro::PS * hydro::PS;
+  p->ff_elems = 9 * 5 * (size_t)hydro::PS * hydro::PS;
+  p->ws_bytes = 0;
+  p->d_status = nullptr;
+  p->d_speed = nullptr;
+  p->streams.assign(nstreams, nullptr);
+  p->d_in.assign(nstreams, nullptr);
+  p->d_out.assign(nstreams, nullptr);
+  p->d_ff.assign(nstreams, nullptr);
+  p->d_ws.assign(nstreams, nullptr);
+  bool ok = cudaMalloc(&p->d_status, 3 * sizeof(long long)) == cudaSuccess;
+  ok = ok && cudaMalloc(&p->d_speed, 16 * sizeof(double)) == cudaSuccess;
+  for (int s = 0; ok && s < nstreams; ++s) {
+    ok = ok && cudaStreamCreateWithFlags(&p->streams[s], cudaStreamNonBlocking) == cudaSuccess;
+    ok = ok && cudaMalloc(&p->d_in[s], p->in_elems * groups_per_chunk * precision_bytes) == cudaSuccess;
+    ok = ok && cudaMalloc(&p->d_out[s], p->out_elems * groups_per_chunk * precision_bytes) == cudaSuccess;
+    ok = ok && cudaMalloc(&p->d_ff[s], p->ff_elems * groups_per_chunk * precision_bytes) == cudaSuccess;
+  }
+  if (!ok) {
+    hydro_pipeline_destroy(p);
+    return (int)cudaErrorMemoryAllocation;
+  }
+  *pp = p;
+  return HYDRO_OK;
+}
+
+void hydro_pipeline_destroy(hydro_pipeline* p) {
+  if (!p) return;
+  for (auto s : p->streams) if (s) { cudaStreamSynchronize(s); cudaStreamDestroy(s); }
+  for (auto v : {&p->d_in, &p->d_out, &p->d_ff, &p->d_ws})
+    for (auto b : *v) if (b) cudaFree(b);
+  if (p->d_status) cudaFree(p->d_status);
+  if (p->d_speed) cudaFree(p->d_speed);
+  delete p;
+}
+
+int hydro_pipeline_solve_f32(hydro_pipeline* p, const float* in, float* out, float* face_flux, int Ng, float dt, float dh,
+                             float gamma, int scheme, int riemann, int limiter, const hydro_opts* opts, long long* status_host,
+                             float* max_speed_host) {
+  return hydro::pipeline_solve<float>(p, in, out, face_flux, Ng, dt, dh, gamma, scheme, riemann, limiter, opts, status_host,
+                                      max_speed_host);
+}
+int hydro_pipeline_solve_f64(hydro_pipeline* p, const double* in, double* out, double* face_flux, int Ng, double dt,
+                             double dh, double gamma, int scheme, int riemann, int limiter, const hydro_opts* opts,
+                             long long* status_host, double* max_speed_host) {
+  return hydro::pipeline_solve<double>(p, in, out, face_flux, Ng, dt, dh, gamma, scheme, riemann, limiter, opts, status_host,
+                                       max_speed_host);
+}
+
+}  // extern "C"

@@ -41,3 +41,27 @@ def run_grid(backend, U, steps, dh, gamma, scheme, riemann, limiter, *, recon=0,
         if on_step:
             on_step(s, U, ff, G, dt)
     return U, t, total, dts
+
+
+class CudaBackend:
+    """The CUDA library behind the same two calls (numpy in / numpy out; device work in libhydro)."""
+
+    def __init__(self, impl=0, device="cuda:0"):
+        import torch
+        from paper_1103_3373_b200 import binding as B
+        self.B, self.torch, self.impl, self.device = B, torch, impl, device
+
+    def dt(self, G, gamma, norm):
+        t = self.torch.from_numpy(np.ascontiguousarray(G)).to(self.device)
+        return float(self.B.hydro_dt(t, gamma, norm).item())
+
+    def solve(self, G, dt, dh, gamma, scheme, riemann, limiter, **kw):
+        torch = self.torch
+        t = torch.from_numpy(np.ascontiguousarray(G)).to(self.device)
+        status = torch.zeros(3, dtype=torch.int64, device=self.device)
+        kw.pop("nthreads", None)
+        want_flux = kw.pop("want_flux", True)
+        out, ff = self.B.hydro_solve(t, dt, dh, gamma, scheme, riemann, limiter, face_flux=want_flux, status=status,
+                                     impl=self.impl, **kw)
+        torch.cuda.synchronize()
+        return out.cpu().numpy(), (ff.cpu().numpy() if ff is not None else None), status.cpu().numpy()

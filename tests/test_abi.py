@@ -1,0 +1,81 @@
+"""Host-side checks of the C ABI (no GPU): the library builds for sm_100a, loads, and exports every
+symbol include/hydro.h declares; argument validation happens on the host before any launch."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1103_3373_b200 import binding
+    binding.lib()
+    return binding
+
+
+def test_exports_match_header(B):
+    hdr = open(os.path.join(ROOT, "include", "hydro.h")).read()
+    declared = set(re.findall(r"HYDRO_API\s+[\w\s\*]+?\b(hydro_\w+)\s*\(", hdr))
+    assert declared == set(B.EXPORTS)
+    L = B.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_min_ghost_table(B):
+    # S1: CTU/MHM need 2 (PLM) / 3 (PPM); VL one more
+    assert [B.hydro_min_ghost(s, r) for s in (B.MHM, B.VL, B.CTU) for r in (B.PLM, B.PPM)] == [2, 3, 3, 4, 2, 3]
+    assert B.hydro_min_ghost(7, 0) == -1
+
+
+def test_strerror(B):
+    assert B.hydro_strerror(0) == "success"
+    for code in range(-8, 0):
+        assert "unknown" not in B.hydro_strerror(code)
+
+
+def test_argument_validation_on_host(B):
+    """Errors are detected before any launch, so these calls need no GPU (pointers are never dereferenced)."""
+    L = B.lib()
+    o = B.make_opts()
+    a = 4096  # fake, 16-byte aligned "device" address
+    call = lambda **k: L.hydro_solve_f32(k.get("in_", a), k.get("out", a * 2), k.get("ff", None), k.get("Ng", 1),
+                                         C.c_float(k.get("dt", 0.1)), C.c_float(k.get("dh", 1.0)),
+                                         C.c_float(k.get("gamma", 1.4)), k.get("scheme", 2), k.get("riemann", 3),
+                                         k.get("limiter", 1), C.byref(k.get("o", o)), None)
+    assert call(scheme=3) == -1 and call(riemann=4) == -1 and call(limiter=-1) == -1
+    assert call(Ng=-1) == -2
+    assert call(in_=None) == -3
+    assert call(in_=a + 4) == -4
+    assert call(o=B.make_opts(nghost=1)) == -5
+    assert call(o=B.make_opts(recon=B.PPM, nghost=2)) == -5
+    assert call(gamma=1.0) == -7 and call(dh=0.0) == -7 and call(dt=-1.0) == -7
+    assert call(o=B.make_opts(minmod_coeff=2.5)) == -7
+    assert call(Ng=0) == 0  # no-op
+    # staged path without workspace
+    if not B.hydro_has_fused(__import__("torch").float32, B.CTU, B.PLM, B.ROE):
+        assert call() == -6
+    assert call(o=B.make_opts(impl=B.IMPL_STAGED)) == -6
+    assert L.hydro_dt_f32(a, 1, 2, C.c_float(1.4), 5, a, None) == -1
+    assert L.hydro_dt_f32(a, 1, 2, C.c_float(1.4), 0, None, None) == -3
+
+
+def test_workspace_sizes(B):
+    import torch
+    n = B.hydro_workspace_bytes(8, torch.float64, B.VL, B.PPM, impl=B.IMPL_STAGED)
+    assert n == 8 * 50 * 24 ** 3 * 8
+    assert B.hydro_workspace_bytes(10 ** 6, torch.float32, B.CTU, B.PLM, impl=B.IMPL_STAGED) == 148 * 4 * 50 * 20 ** 3 * 4
+
+
+def test_product_does_not_import_oracle():
+    """The product path must not route through the oracle (or any CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_1103_3373_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", src, re.M), f
+                assert "liboracle" not in src and "hydro_oracle" not in src, f
