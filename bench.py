@@ -1,0 +1,341 @@
+#!/usr/bin/env python
+"""bench.py -- cell updates/s of the unsplit patch-group update on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--dtype f32|f64]
+
+A "step" is one pass of the whole hot path over one batch of synthetic patch groups:
+hydro_dt (CFL reduction) -> hydro_solve (steps (1)-(5)), the time-step
+formed on the device from the reduction (no host sync inside the timed region).  The workload is
+BASELINE.json configs[2] (the AMR-shaped batch the metric's CTU+PLM+Roe fp32 number is quoted on):
+8192 patch groups of 16^3 cells with 3 ghost cells (22^3 input), 5 fp32 variables SoA, one
+CTU + PLM (van Leer) + Roe step with the patch-boundary fluxes returned.  Inputs (1.7 GB) exceed L2.
+
+Prints ONE JSON line (rank 0).  Keys beyond the base contract: roofline, cpu_baseline, e2e, clocks,
+gpu_launches, and f64 (the same step in double precision, same kernels templated on double).
+--impl reference times the CPU oracle (oracle/, plain C++ on the host cores) on the same config.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell updates/sec (CTU+PLM+Roe, fp32/fp64) and % of HBM/FLOP roofline"
+UNIT = "cell updates/s"
+NG, GHOST, GAMMA, DH, CFL = 8192, 3, 5.0 / 3.0, 1.0, 0.5
+CELLS = 16 ** 3
+SCHEME, RIEMANN, LIMITER = 2, 3, 1  # CTU, Roe, van Leer (PLM on primitive variables: opts defaults)
+
+
+def load_json(path, default=None):
+    try:
+        with open(path) as f:
+            return json.load(f)
+    except Exception:
+        return default
+
+
+def workload_name(dtype):
+    return f"configs[2]: AMR batch, {NG} patch groups x 16^3 cells, g={GHOST} (22^3 in), {dtype}, CTU+PLM(vanLeer)+Roe, face fluxes on"
+
+
+def algorithmic_flops_per_cell(dtype):
+    """Counted on the oracle with a counting scalar (oracle/count_flops.py -> oracle/flops_per_cell.json);
+    falls back to the hand estimate of SURVEY.md 8(d) until that file exists."""
+    d = load_json(os.path.join(ROOT, "oracle", "flops_per_cell.json"), {})
+    e = d.get("ctu_plm_roe_vanleer_g3", {})
+    if "flops_per_cell" in e:
+        return float(e["flops_per_cell"]), "counted (oracle/count_flops.py)"
+    return 2300.0, "hand estimate (SURVEY.md 8(d))"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples, self.mask, self.max_mhz, self.ok = index, False, [], 0, None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self.stop_flag:
+            try:
+                self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "samples": len(s),
+                "reasons": [n for b, n in self.REASONS.items() if self.mask & b]}
+
+
+def physical_gpu_index(local):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local])
+        except Exception:
+            return local
+    return local
+
+
+def time_oracle(G, dt, nthreads, target_s=12.0):
+    """The oracle as it stands on a bounded sample: calibrate on 2*nthreads groups, then ~target_s of work."""
+    from oracle import oracle as O
+    n0 = min(len(G), 2 * nthreads)
+    t0 = time.perf_counter()
+    O.hydro_dt(G[:n0], GAMMA, 0)
+    O.hydro_solve(G[:n0], dt, DH, GAMMA, SCHEME, RIEMANN, LIMITER, nthreads=nthreads)
+    per_group = (time.perf_counter() - t0) / n0
+    n = int(max(n0, min(len(G), target_s / max(per_group, 1e-9))))
+    t0 = time.perf_counter()
+    O.hydro_dt(G[:n], GAMMA, 0)
+    O.hydro_solve(G[:n], dt, DH, GAMMA, SCHEME, RIEMANN, LIMITER, nthreads=nthreads)
+    el = time.perf_counter() - t0
+    return n * CELLS / el, n, el
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, same config/metric; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import numpy as np
+    from oracle import oracle as O
+    from paper_1103_3373_b200 import workloads as wl
+    dtype = "float32" if args.dtype == "f32" else "float64"
+    nthreads = min(O.max_threads(), len(os.sched_getaffinity(0)))
+    nsample = int(os.environ.get("HYDRO_REF_GROUPS", 32 * nthreads))
+    G = wl.amr_batch(nsample, g=GHOST, gamma=GAMMA, seed=0, dtype=dtype).numpy()
+    smax = O.hydro_dt(G, GAMMA, 0)
+    dt = float(G.dtype.type(CFL * DH / smax))
+    for _ in range(max(0, min(args.warmup, 1))):
+        O.hydro_solve(G[:nthreads], dt, DH, GAMMA, SCHEME, RIEMANN, LIMITER, nthreads=nthreads)
+    steps = max(1, args.steps)
+    budget = float(os.environ.get("HYDRO_REF_BUDGET_S", "120"))
+    t0 = time.perf_counter()
+    done = 0
+    for _ in range(steps):
+        O.hydro_dt(G, GAMMA, 0)
+        O.hydro_solve(G, dt, DH, GAMMA, SCHEME, RIEMANN, LIMITER, nthreads=nthreads)
+        done += 1
+        if time.perf_counter() - t0 > budget:
+            break
+    el = time.perf_counter() - t0
+    value = done * nsample * CELLS / el
+    sample = f"{nsample} of {NG} patch groups per step, {done} steps, {nthreads} OpenMP threads over groups (PAPER.md:137)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
+        "warmup": args.warmup, "ms_per_step": 1e3 * el / done, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": workload_name(args.dtype), "note": "CPU oracle (oracle/hydro_oracle.cpp, g++ -O2 -ffp-contract=off) on a bounded sample"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": nthreads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--dtype", default="f32", choices=("f32", "f64"))
+    ap.add_argument("--ng", type=int, default=NG, help="patch groups per GPU (default: the config's 8192)")
+    ap.add_argument("--kernel", default="auto", choices=("auto", "staged", "fused"))
+    ap.add_argument("--no-extras", action="store_true", help="skip the e2e / cpu_baseline / f64 legs (profiling runs)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1103_3373_b200 import binding as B, workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    B.lib()
+    warmup = max(3, args.warmup)
+    steps = max(1, args.steps)
+    impl = {"auto": B.IMPL_AUTO, "staged": B.IMPL_STAGED, "fused": B.IMPL_FUSED}[args.kernel]
+    Ng = args.ng
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def device_leg(tdtype, nsteps, nwarm, sample_clocks):
+        """K steps of hydro_dt -> [max all-reduce over ranks] -> hydro_solve, inputs resident in HBM."""
+        name = str(tdtype).replace("torch.", "")
+        u = wl.amr_batch(Ng, g=GHOST, gamma=GAMMA, seed=1000 * rank, dtype=name, device=dev)
+        out = torch.empty((Ng, 5, 16, 16, 16), dtype=tdtype, device=dev)
+        ff = torch.empty((Ng, 9, 5, 16, 16), dtype=tdtype, device=dev)
+        smax = torch.empty((), dtype=tdtype, device=dev)
+        status = torch.zeros(3, dtype=torch.int64, device=dev)
+
+        def step():
+            B.hydro_dt(u, GAMMA, 0, max_speed=smax)
+            if world > 1:  # the path's only exchange: one scalar max
+                dist.all_reduce(smax, op=dist.ReduceOp.MAX)
+            B.hydro_solve(u, 0.0, DH, GAMMA, SCHEME, RIEMANN, LIMITER, out=out, face_flux=ff, status=status,
+                          max_speed=smax, cfl=CFL, impl=impl)
+
+        for _ in range(nwarm):
+            step()
+        ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(nsteps)]
+        t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        sampler = ClockSampler(physical_gpu_index(local)) if sample_clocks else None
+        barrier()
+        if sampler:
+            sampler.start()
+        t_begin.record()
+        for k in range(nsteps):
+            ev[k][0].record()
+            B.hydro_dt(u, GAMMA, 0, max_speed=smax)
+            if world > 1:
+                dist.all_reduce(smax, op=dist.ReduceOp.MAX)
+            ev[k][1].record()
+            B.hydro_solve(u, 0.0, DH, GAMMA, SCHEME, RIEMANN, LIMITER, out=out, face_flux=ff, status=status,
+                          max_speed=smax, cfl=CFL, impl=impl)
+            ev[k][2].record()
+        t_end.record()
+        barrier()
+        if sampler:
+            sampler.stop_flag = True
+            sampler.join()
+        total_ms = t_begin.elapsed_time(t_end)
+        if world > 1:
+            t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            total_ms = float(t.item())
+        dt_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / nsteps
+        solve_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / nsteps
+        st = status.cpu().tolist()
+        return {"total_ms": total_ms, "dt_ms": dt_ms, "solve_ms": solve_ms, "status": st, "u": u,
+                "clocks": sampler.summary() if sampler else None, "smax": float(smax.item())}
+
+    main_dtype = torch.float32 if args.dtype == "f32" else torch.float64
+    leg = device_leg(main_dtype, steps, warmup, True)
+    value = world * Ng * CELLS * steps / (leg["total_ms"] * 1e-3)
+    es = 4 if args.dtype == "f32" else 8
+    S = 16 + 2 * GHOST
+
+    # ---- roofline of the dominant kernel (hydro_solve): plain-ALU bound ----
+    peaks = load_json(os.path.join(ROOT, "MEASURED_PEAKS.json"), {}) or {}
+    clocks = leg["clocks"] or {}
+    sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    lanes = 128 if args.dtype == "f32" else 64  # FP32 / FP64 FMA lanes per SM
+    peak_tflops = 148 * lanes * 2 * sm_max * 1e6 / 1e12
+    flops_cell, flops_src = algorithmic_flops_per_cell(args.dtype)
+    achieved_tflops = flops_cell * Ng * CELLS / (leg["solve_ms"] * 1e-3) / 1e12
+    bytes_cell = es * (5 * S ** 3 + 5 * CELLS + 45 * 256) / CELLS
+    hbm = float(peaks.get("hbm_gbs") or 6650.0)
+    hbm_src = "measured (MEASURED_PEAKS.json)" if peaks.get("hbm_gbs") else "fallback (B200_PROFILING.md)"
+    traffic = (load_json(os.path.join(ROOT, "profiles", "traffic.json"), {}) or {}).get(f"solve_{args.dtype}_{args.kernel}")
+    roofline = {
+        "bound": "alu", "kernel": "hydro_solve (ctu fused)" if B.hydro_has_fused(main_dtype, SCHEME) and impl != B.IMPL_STAGED else "hydro_solve (staged)",
+        "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved_tflops / peak_tflops,
+        "traffic": traffic,
+        "flops_per_cell": flops_cell, "flops_source": flops_src,
+        "peak_source": f"148 SM x {lanes} lanes x 2 x {sm_max:.0f} MHz (nominal unit counts at clocks.max.sm)",
+        "kernel_ms": leg["solve_ms"], "share_of_step": leg["solve_ms"] / (leg["solve_ms"] + leg["dt_ms"]),
+        "hbm": {"bytes_per_cell": bytes_cell, "achieved_gbs": bytes_cell * Ng * CELLS / (leg["solve_ms"] * 1e-3) / 1e9,
+                "peak_gbs": hbm, "peak_source": hbm_src,
+                "hydro_dt_gbs": 5 * es * Ng * CELLS / (leg["dt_ms"] * 1e-3) / 1e9},
+        "cells_per_s_at_alu_roof": peak_tflops * 1e12 / flops_cell,
+        "cells_per_s_at_hbm_roof": hbm * 1e9 / bytes_cell,
+    }
+
+    result = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": leg["total_ms"] / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": workload_name(args.dtype), "groups_per_gpu": Ng, "l2": "inputs (1.7 GB fp32) larger than L2; no flush",
+                   "step": "hydro_dt + hydro_solve, dt formed on device", "kernel": args.kernel,
+                   "parallelism": f"{world} x independent patch-group shards (max all-reduce of one scalar)"},
+        "roofline": roofline, "clocks": clocks, "gpu_launches": 2 * steps, "status": leg["status"],
+    }
+
+    if rank == 0 and world == 1 and not args.no_extras:
+        # ---- e2e: HOST buffers through the C ABI pipeline, copies inside the timed region
+        u = leg["u"]
+        hin = torch.empty(u.shape, dtype=u.dtype, pin_memory=True)
+        hin.copy_(u)
+        del leg["u"], u
+        hout = torch.empty((Ng, 5, 16, 16, 16), dtype=main_dtype, pin_memory=True)
+        hff = torch.empty((Ng, 9, 5, 16, 16), dtype=main_dtype, pin_memory=True)
+        hs = torch.zeros((), dtype=main_dtype)
+        pipe = B.HydroPipeline(main_dtype, GHOST, groups_per_chunk=512, nstreams=4, device=dev)
+        dt0 = CFL * DH / leg["smax"]
+        pipe.solve(hin, hout, hff, dt0, DH, GAMMA, SCHEME, RIEMANN, LIMITER, max_speed=hs, impl=impl)
+        ne = max(2, min(5, steps))
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(ne):
+            pipe.solve(hin, hout, hff, dt0, DH, GAMMA, SCHEME, RIEMANN, LIMITER, max_speed=hs, impl=impl)
+        torch.cuda.synchronize()
+        e2e_s = (time.perf_counter() - t0) / ne
+        pipe.close()
+        result["e2e"] = {"value": Ng * CELLS / e2e_s, "unit": UNIT, "h2d_bytes_per_step": hin.numel() * es,
+                         "d2h_bytes_per_step": (hout.numel() + hff.numel()) * es + es, "ms_per_step": 1e3 * e2e_s,
+                         "api": "hydro_pipeline_solve (pinned host in/out, 4 streams x 512-group chunks; hydro_dt of the updated state fused per chunk)"}
+        # ---- cpu_baseline: the oracle as it stands, bounded sample, all host cores
+        from oracle import oracle as O
+        nthreads = min(O.max_threads(), len(os.sched_getaffinity(0)))
+        G = hin[: min(Ng, 4096)].numpy()
+        cpu_v, cpu_n, cpu_s = time_oracle(G, float(G.dtype.type(dt0)), nthreads)
+        result["cpu_baseline"] = {"value": cpu_v, "unit": UNIT, "cores": nthreads, "kind": "oracle",
+                                  "sample": f"first {cpu_n} of {Ng} patch groups of the same batch, hydro_dt + one {args.dtype} CTU+PLM+Roe step, {cpu_s:.1f} s, OpenMP over groups"}
+        del hin, hout, hff
+        torch.cuda.empty_cache()
+        # ---- the other precision, device-resident leg only
+        other = torch.float64 if args.dtype == "f32" else torch.float32
+        oname = "f64" if args.dtype == "f32" else "f32"
+        leg2 = device_leg(other, max(3, steps // 2), 3, False)
+        v2 = Ng * CELLS * max(3, steps // 2) / (leg2["total_ms"] * 1e-3)
+        lanes2 = 64 if oname == "f64" else 128
+        peak2 = 148 * lanes2 * 2 * sm_max * 1e6 / 1e12
+        ach2 = flops_cell * Ng * CELLS / (leg2["solve_ms"] * 1e-3) / 1e12
+        result[oname] = {"value": v2, "unit": UNIT, "ms_per_step": leg2["total_ms"] / max(3, steps // 2),
+                         "roofline": {"bound": "alu", "achieved": ach2, "peak": peak2, "unit": "TFLOP/s", "frac": ach2 / peak2}}
+    elif "u" in leg:
+        del leg["u"]
+    if "e2e" not in result:
+        result["e2e"] = None
+    if rank == 0:
+        print(json.dumps(result))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -127,7 +127,10 @@ HYDRO_API int hydro_pipeline_solve_f64(hydro_pipeline* p, const double* in, doub
 /* Sizes and capabilities. */
 HYDRO_API int hydro_min_ghost(int scheme, int recon);                 /* 2/3 (MHM, CTU with PLM/PPM), 3/4 (VL)   */
 HYDRO_API int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann); /* 1 if a fused kernel exists */
-/* bytes of opts->workspace needed by hydro_solve_* in HYDRO_IMPL_AUTO mode (0 when the fused kernel runs) */
+/* 1 if that fused kernel's tiles fit in shared memory for ghost width nghost (else AUTO uses the staged path) */
+HYDRO_API int hydro_fused_fits(int precision_bytes, int scheme, int recon, int nghost);
+/* bytes of opts->workspace that hydro_solve_* may need in HYDRO_IMPL_AUTO mode for any ghost width
+ * (0 only when the fused kernel runs for every nghost <= 8) */
 HYDRO_API size_t hydro_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon);
 /* bytes needed when HYDRO_IMPL_STAGED is forced */
 HYDRO_API size_t hydro_staged_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon);

@@ -21,7 +21,7 @@ PS = 16
 
 EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64", "hydro_pipeline_create",
            "hydro_pipeline_destroy", "hydro_pipeline_solve_f32", "hydro_pipeline_solve_f64", "hydro_min_ghost",
-           "hydro_has_fused", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror")
+           "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror")
 
 
 class HydroOpts(C.Structure):
@@ -59,6 +59,7 @@ def lib():
         L.hydro_pipeline_destroy.restype = None
         L.hydro_min_ghost.argtypes = [i, i]
         L.hydro_has_fused.argtypes = [i, i, i, i]
+        L.hydro_fused_fits.argtypes = [i, i, i, i]
         L.hydro_workspace_bytes.argtypes = [i, i, i, i]
         L.hydro_workspace_bytes.restype = sz
         L.hydro_staged_workspace_bytes.argtypes = [i, i, i, i]
@@ -81,11 +82,16 @@ def hydro_has_fused(dtype, scheme, recon=PLM, riemann=ROE):
     return bool(lib().hydro_has_fused(torch.empty((), dtype=dtype).element_size(), scheme, recon, riemann))
 
 
-def hydro_workspace_bytes(Ng, dtype, scheme, recon=PLM, impl=IMPL_AUTO):
+def hydro_fused_fits(dtype, scheme, recon=PLM, nghost=0):
+    return bool(lib().hydro_fused_fits(torch.empty((), dtype=dtype).element_size(), scheme, recon, nghost))
+
+
+def hydro_workspace_bytes(Ng, dtype, scheme, recon=PLM, impl=IMPL_AUTO, nghost=0):
+    """Scratch bytes hydro_solve needs: 0 when the fused kernel runs for this ghost width."""
     es = torch.empty((), dtype=dtype).element_size()
-    if impl == IMPL_STAGED:
+    if impl == IMPL_STAGED or (impl == IMPL_AUTO and not lib().hydro_fused_fits(es, scheme, recon, nghost)):
         return lib().hydro_staged_workspace_bytes(Ng, es, scheme, recon)
-    return lib().hydro_workspace_bytes(Ng, es, scheme, recon)
+    return 0
 
 
 _ws_cache = {}
@@ -153,7 +159,7 @@ def hydro_solve(in_, dt, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *,
     impl = optkw.get("impl", IMPL_AUTO)
     ws = optkw.pop("workspace", None)
     if ws is None:
-        ws = _workspace(hydro_workspace_bytes(Ng, in_.dtype, scheme, recon, impl), in_.device)
+        ws = _workspace(hydro_workspace_bytes(Ng, in_.dtype, scheme, recon, impl, g), in_.device)
     o = make_opts(nghost=g, status=status, workspace=ws, **optkw)
     st = (stream or torch.cuda.current_stream(in_.device)).cuda_stream
     with torch.cuda.device(in_.device):

@@ -186,8 +186,8 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   par.limiter = limiter;
   par.char_limit = o ? o->char_limit : 0;
   par.roe_fallback = fb;
-  const bool has = hydro_has_fused((int)sizeof(R), scheme, recon, riemann) != 0;
-  if (impl == HYDRO_IMPL_FUSED && !has) return HYDRO_E_NOFUSED;
+  const bool has = fused_fits((int)sizeof(R), scheme, recon, g);  // kernel exists and its tiles fit in shared memory
+  if (impl == HYDRO_IMPL_FUSED && !has) return HYDRO_E_NOFUSED;  // no kernel, or its tiles do not fit for this g
   pl.recon = recon;
   pl.g = g;
   pl.impl = (impl == HYDRO_IMPL_STAGED || !has) ? HYDRO_IMPL_STAGED : HYDRO_IMPL_FUSED;
@@ -323,6 +323,13 @@ int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann) {
   return hydro::fused_available(precision_bytes, scheme, recon) ? 1 : 0;
 }
 
+int hydro_fused_fits(int precision_bytes, int scheme, int recon, int nghost) {
+  if (!hydro_has_fused(precision_bytes, scheme, recon, 0)) return 0;
+  if (nghost == 0) nghost = hydro::min_ghost(scheme, recon);
+  if (nghost < hydro::min_ghost(scheme, recon) || nghost > 8) return 0;
+  return hydro::fused_fits(precision_bytes, scheme, recon, nghost) ? 1 : 0;
+}
+
 size_t hydro_staged_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon) {
   if (scheme < 0 || scheme > 2 || recon < 0 || recon > 1 || Ng <= 0) return 0;
   if (precision_bytes != 4 && precision_bytes != 8) return 0;
@@ -331,7 +338,7 @@ size_t hydro_staged_workspace_bytes(int Ng, int precision_bytes, int scheme, int
 }
 
 size_t hydro_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon) {
-  if (hydro_has_fused(precision_bytes, scheme, recon, 0)) return 0;
+  if (hydro_fused_fits(precision_bytes, scheme, recon, 8)) return 0;
   return hydro_staged_workspace_bytes(Ng, precision_bytes, scheme, recon);
 }
 

@@ -538,4 +538,18 @@ __device__ __forceinline__ V5<R> riemann_d(const V5<R>& WL, const V5<R>& WR, con
   return from_normal<D>(riemann_n<RS>(to_normal<D>(WL), to_normal<D>(WR), p, c));
 }
 
+// add the per-thread event counters of a CTA to hydro_opts::status
+__device__ __forceinline__ void flush_counters(const Cnt& c, long long* status) {
+  if (!status) return;
+  // warp-aggregate, then one atomic per warp and counter (rare events; status may be nullptr)
+  int v[3] = {c.roe_fb, c.bad, c.exact};
+#pragma unroll
+  for (int q = 0; q < 3; ++q) {
+    int s = v[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0 && s) atomicAdd(reinterpret_cast<unsigned long long*>(status + q), (unsigned long long)s);
+  }
+}
+
 }  // namespace hydro

@@ -139,19 +139,6 @@ template <class R> __device__ __forceinline__ V5<R> load_in(const R* in, size_t 
   return U;
 }
 
-__device__ __forceinline__ void flush_counters(const Cnt& c, long long* status) {
-  if (!status) return;
-  // warp-aggregate, then one atomic per warp and counter (rare events; status may be nullptr)
-  int v[3] = {c.roe_fb, c.bad, c.exact};
-#pragma unroll
-  for (int q = 0; q < 3; ++q) {
-    int s = v[q];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-    if ((threadIdx.x & 31) == 0 && s) atomicAdd(reinterpret_cast<unsigned long long*>(status + q), (unsigned long long)s);
-  }
-}
-
 template <class R, int SCHEME, int RECON, int RS>
 __global__ void __launch_bounds__(STAGED_NT) staged_kernel(const R* __restrict__ in, R* __restrict__ out,
                                                            R* __restrict__ face_flux, int Ng, int g, Par<R> p,

@@ -1,10 +1,9 @@
-// variants without a fused kernel: the launcher exists only to fill the dispatch table
+// schemes without a fused kernel yet (MHM, VL): launchers that only fill the dispatch table
 #include "hydro_fused.cuh"
 namespace hydro {
 #define INST(R, S, RC, RS) template cudaError_t launch_fused<R, S, RC, RS>(const SolveArgs<R>&);
 #define FOR_RS(M, R, S, RC) M(R, S, RC, RS_EXACT) M(R, S, RC, RS_HLLE) M(R, S, RC, RS_HLLC) M(R, S, RC, RS_ROE)
 #define FOR_RC(M, R, S) FOR_RS(M, R, S, RECON_PLM) FOR_RS(M, R, S, RECON_PPM)
-#define FOR_S(M, R) FOR_RC(M, R, SCHEME_MHM) FOR_RC(M, R, SCHEME_VL) FOR_RC(M, R, SCHEME_CTU)
-FOR_S(INST, float)
-FOR_S(INST, double)
+FOR_RC(INST, float, SCHEME_MHM) FOR_RC(INST, float, SCHEME_VL)
+FOR_RC(INST, double, SCHEME_MHM) FOR_RC(INST, double, SCHEME_VL)
 }  // namespace hydro

@@ -56,8 +56,9 @@ def test_argument_validation_on_host(B):
     assert call(o=B.make_opts(minmod_coeff=2.5)) == -7
     assert call(Ng=0) == 0  # no-op
     # staged path without workspace
-    if not B.hydro_has_fused(__import__("torch").float32, B.CTU, B.PLM, B.ROE):
+    if not B.hydro_fused_fits(__import__("torch").float32, B.CTU, B.PLM, 2):
         assert call() == -6
+    assert call(scheme=B.MHM) == -6 or B.hydro_fused_fits(__import__("torch").float32, B.MHM, B.PLM, 2)
     assert call(o=B.make_opts(impl=B.IMPL_STAGED)) == -6
     assert L.hydro_dt_f32(a, 1, 2, C.c_float(1.4), 5, a, None) == -1
     assert L.hydro_dt_f32(a, 1, 2, C.c_float(1.4), 0, None, None) == -3

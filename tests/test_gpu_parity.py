@@ -66,10 +66,10 @@ def check(out, ff, ref_out, ref_ff, dtype, what):
         assert e <= TOL32, (what, "face_flux", e)
 
 
-def impls(B, dtype, scheme, recon):
+def impls(B, dtype, scheme, recon, g=0):
     import torch
     t = {np.float32: torch.float32, np.float64: torch.float64}[dtype]
-    return (STAGED, FUSED) if B.hydro_has_fused(t, scheme, recon) else (STAGED,)
+    return (STAGED, FUSED) if B.hydro_fused_fits(t, scheme, recon, g) else (STAGED,)
 
 
 def gpu_solve(B, G, dt, dh, gamma, scheme, riemann, limiter, impl, **kw):
@@ -110,7 +110,7 @@ def test_extra_ghosts_and_options(B, oracle, dtype):
         dt = 0.3 * dh / oracle.hydro_dt(G, gamma, 0)
         for kw in (dict(minmod_coeff=1.0), dict(minmod_coeff=2.0), dict(roe_fallback=2), dict(roe_fallback=3)):
             ref = oracle.hydro_solve(G, dt, dh, gamma, scheme, ROE, GMINMOD, recon=recon, **kw)
-            for impl in impls(B, dtype, scheme, recon):
+            for impl in impls(B, dtype, scheme, recon, g):
                 out, ff, st = gpu_solve(B, G, dt, dh, gamma, scheme, ROE, GMINMOD, impl, recon=recon, **kw)
                 check(out, ff, ref[0], ref[1], dtype, (scheme, recon, g, kw, impl))
 
