@@ -90,7 +90,7 @@ __global__ void __launch_bounds__(DT_NT) dt_kernel(const R* __restrict__ u, long
     }
 #pragma unroll
     for (int t = 0; t < DT_ROWS_PER_THREAD; ++t) {
-      const R rho = v[t][0], ir = R(1) / rho;
+      const R rho = v[t][0], ir = m_rcp(rho);
       const R vx = v[t][1] * ir, vy = v[t][2] * ir, vz = v[t][3] * ir;
       const R P = (gamma - R(1)) * (v[t][4] - R(0.5) * rho * ((vx * vx + vy * vy) + vz * vz));
       const R c = m_sqrt(gamma * P * ir);
@@ -178,6 +178,7 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   if (o && o->max_speed && (!(o->cfl > 0.0) || ((uintptr_t)o->max_speed & (sizeof(R) - 1)))) return HYDRO_E_VALUE;
   par.gamma = gamma;
   par.gm1 = gamma - R(1);
+  par.igm1 = R(1) / par.gm1;
   par.nu = dt / dh;
   par.hnu = R(0.5) * par.nu;
   par.theta = (R)theta;

@@ -21,8 +21,6 @@ enum : int { RECON_PLM = 0, RECON_PPM = 1 };
 constexpr int PS = 16;  // interior cells per side of a patch group
 
 // ---- scalar helpers (one overload per precision) -------------------------------------------
-__device__ __forceinline__ float  m_sqrt(float x) { return sqrtf(x); }
-__device__ __forceinline__ double m_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ float  m_abs(float x) { return fabsf(x); }
 __device__ __forceinline__ double m_abs(double x) { return fabs(x); }
 __device__ __forceinline__ float  m_min(float a, float b) { return fminf(a, b); }
@@ -31,8 +29,28 @@ __device__ __forceinline__ float  m_max(float a, float b) { return fmaxf(a, b); 
 __device__ __forceinline__ double m_max(double a, double b) { return fmax(a, b); }
 __device__ __forceinline__ float  m_pow(float a, float b) { return powf(a, b); }
 __device__ __forceinline__ double m_pow(double a, double b) { return pow(a, b); }
+
+// Division / reciprocal / square-root policy.  fp64: IEEE-rounded.  fp32: the SFU approximations
+// (div.approx / rcp.approx / sqrt.approx, <= 2 ulp, subnormals flushed), as the paper's own kernel did
+// with -prec-div=false -ftz=true.  An IEEE fp32 division costs MUFU.RCP + FCHK + 4 FFMA +
+// a branch to a slow-path subroutine, ~200 times per cell update; the error of the approximations is
+// far inside the fp32 parity budget (L1 <= 1e-5 per step).  -DHYDRO_F32_IEEE=1
+// restores IEEE fp32 arithmetic for A/B measurements.
+#ifndef HYDRO_F32_IEEE
+#define HYDRO_F32_IEEE 0
+#endif
+#if HYDRO_F32_IEEE
+__device__ __forceinline__ float  m_sqrt(float x) { return sqrtf(x); }
 __device__ __forceinline__ float  m_rcp(float x) { return 1.0f / x; }
+__device__ __forceinline__ float  m_div(float a, float b) { return a / b; }
+#else
+__device__ __forceinline__ float  m_sqrt(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float  m_rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float  m_div(float a, float b) { float r; asm("div.approx.ftz.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b)); return r; }
+#endif
+__device__ __forceinline__ double m_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ double m_rcp(double x) { return 1.0 / x; }
+__device__ __forceinline__ double m_div(double a, double b) { return a / b; }
 
 template <class R> struct ExactTol;
 template <> struct ExactTol<float> { static __device__ __forceinline__ float v() { return 1e-6f; } };
@@ -47,6 +65,7 @@ template <class R> struct V5 {
 // run-time parameters of one hydro_solve call (uniform over the grid)
 template <class R> struct Par {
   R gamma, gm1;   // gamma, gamma-1
+  R igm1;         // 1/(gamma-1), formed once on the host
   R nu, hnu;      // dt/dh and half of it
   R theta;        // generalized-minmod coefficient (S7)
   R min_dens, min_pres;
@@ -56,7 +75,7 @@ template <class R> struct Par {
 // dt/dh from the device-resident hydro_dt result (hydro_opts::max_speed), uniform over the grid
 template <class R> __device__ __forceinline__ void apply_device_dt(Par<R>& p, const R* max_speed, R cfl) {
   if (max_speed) {
-    p.nu = cfl / __ldg(max_speed);
+    p.nu = m_div(cfl, __ldg(max_speed));
     p.hnu = R(0.5) * p.nu;
   }
 }
@@ -91,7 +110,7 @@ template <class R> __device__ __forceinline__ V5<R> prim2cons(const V5<R>& W, co
   U[1] = W[0] * W[1];
   U[2] = W[0] * W[2];
   U[3] = W[0] * W[3];
-  U[4] = W[4] / p.gm1 + R(0.5) * W[0] * ((W[1] * W[1] + W[2] * W[2]) + W[3] * W[3]);
+  U[4] = W[4] * p.igm1 + R(0.5) * W[0] * ((W[1] * W[1] + W[2] * W[2]) + W[3] * W[3]);
   return U;
 }
 
@@ -118,7 +137,7 @@ template <int D, class R> __device__ __forceinline__ V5<R> from_normal(const V5<
 // physical flux and conserved vector of a normal-frame primitive state
 template <class R> __device__ __forceinline__ void flux_and_cons(const V5<R>& W, const Par<R>& p, V5<R>& F, V5<R>& U) {
   const R rho = W[0], vn = W[1];
-  const R E = W[4] / p.gm1 + R(0.5) * rho * ((vn * vn + W[2] * W[2]) + W[3] * W[3]);
+  const R E = W[4] * p.igm1 + R(0.5) * rho * ((vn * vn + W[2] * W[2]) + W[3] * W[3]);
   U[0] = rho;
   U[1] = rho * vn;
   U[2] = rho * W[2];
@@ -142,14 +161,14 @@ template <class R> __device__ __forceinline__ R limited_slope(R dL, R dR, const 
   if (!(prod > R(0))) return R(0);  // S19: zero product -> zero slope
   const R dC = R(0.5) * (dL + dR);
   switch (p.limiter) {
-    case LIM_VANLEER: return R(2) * prod / (dL + dR);
-    case LIM_VANALBADA: return prod * (dL + dR) / (dL * dL + dR * dR);
+    case LIM_VANLEER: return m_div(R(2) * prod, dL + dR);
+    case LIM_VANALBADA: return m_div(prod * (dL + dR), dL * dL + dR * dR);
     case LIM_GMINMOD: {
       const R m = m_min(m_min(p.theta * m_abs(dL), p.theta * m_abs(dR)), m_abs(dC));
       return dC > R(0) ? m : -m;
     }
     default: {  // hybrid: generalized minmod (theta = 2) combined with van Leer
-      const R vl = m_abs(R(2) * prod / (dL + dR));
+      const R vl = m_abs(m_div(R(2) * prod, dL + dR));
       const R m = m_min(m_min(R(2) * m_abs(dL), R(2) * m_abs(dR)), m_min(m_abs(dC), vl));
       return dC > R(0) ? m : -m;
     }
@@ -229,8 +248,8 @@ __device__ __forceinline__ void reconstruct(const V5<R>& Wm2, const V5<R>& Wm1, 
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       const R w0 = W0[q];
-      R wl = R(0.5) * (Wm1[q] + w0) - (dW[q] - dWm[q]) / R(6);
-      R wr = R(0.5) * (w0 + Wp1[q]) - (dWp[q] - dW[q]) / R(6);
+      R wl = R(0.5) * (Wm1[q] + w0) - (dW[q] - dWm[q]) * R(1.0 / 6.0);
+      R wr = R(0.5) * (w0 + Wp1[q]) - (dWp[q] - dW[q]) * R(1.0 / 6.0);
       if ((wr - w0) * (w0 - wl) <= R(0)) {
         wl = w0;
         wr = w0;
@@ -288,7 +307,7 @@ __device__ __forceinline__ void reconstruct(const V5<R>& Wm2, const V5<R>& Wm1, 
       DpW6[q] = D[q] + W6[q];
     }
     const V5<R> aDm = e.project(DmW6), aDp = e.project(DpW6), a6 = e.project(W6);
-    const R n23 = nu * nu / R(3);
+    const R n23 = nu * nu * R(1.0 / 3.0);
     // upper face (lambda > 0): A = (nu/2)(lamM - lambda), B = (nu^2/3)(lamM^2 - lambda^2)
     const bool p0 = lam0 > R(0), p1 = vn > R(0), m1 = vn < R(0), m4 = lamM < R(0);
     const R A0 = p0 ? R(0.5) * nu * (lamM - lam0) : R(0), B0 = p0 ? n23 * (lamM * lamM - lam0 * lam0) : R(0);
@@ -308,7 +327,7 @@ __device__ __forceinline__ void reconstruct(const V5<R>& Wm2, const V5<R>& Wm1, 
     am[3] = C1 * aDp[3] + D1 * a6[3];
     am[4] = C4 * aDp[4] + D4 * a6[4];
     const V5<R> tp = e.expand(ap), tm = e.expand(am);
-    const R kp = R(1) - R(2) / R(3) * sgp, km = R(1) + R(2) / R(3) * sgm;
+    const R kp = R(1) - R(2.0 / 3.0) * sgp, km = R(1) + R(2.0 / 3.0) * sgm;
 #pragma unroll
     for (int q = 0; q < 5; ++q) {
       Wup[q] = (WR[q] - R(0.5) * sgp * (D[q] - kp * W6[q])) + tp[q];
@@ -323,7 +342,7 @@ template <class R> struct RoeAvg { R vn, v1, v2, H, a; };
 template <class R>
 __device__ __forceinline__ RoeAvg<R> roe_average(const V5<R>& WL, const V5<R>& WR, const V5<R>& UL, const V5<R>& UR,
                                                  const Par<R>& p) {
-  const R HL = (UL[4] + WL[4]) / WL[0], HR = (UR[4] + WR[4]) / WR[0];
+  const R HL = m_div(UL[4] + WL[4], WL[0]), HR = m_div(UR[4] + WR[4], WR[0]);
   const R sL = m_sqrt(WL[0]), sR = m_sqrt(WR[0]), id = m_rcp(sL + sR);
   RoeAvg<R> r;
   r.vn = (sL * WL[1] + sR * WR[1]) * id;
@@ -339,7 +358,7 @@ __device__ __forceinline__ RoeAvg<R> roe_average(const V5<R>& WL, const V5<R>& W
 template <class R>
 __device__ __forceinline__ V5<R> hlle_from(const V5<R>& WL, const V5<R>& WR, const V5<R>& UL, const V5<R>& UR,
                                            const V5<R>& FL, const V5<R>& FR, const RoeAvg<R>& r, const Par<R>& p) {
-  const R cL = m_sqrt(p.gamma * WL[4] / WL[0]), cR = m_sqrt(p.gamma * WR[4] / WR[0]);
+  const R cL = m_sqrt(m_div(p.gamma * WL[4], WL[0])), cR = m_sqrt(m_div(p.gamma * WR[4], WR[0]));
   const R SL = m_min(r.vn - r.a, WL[1] - cL), SR = m_max(r.vn + r.a, WR[1] + cR);
   const R bm = m_min(SL, R(0)), bp = m_max(SR, R(0));
   const R iw = m_rcp(bp - bm), bb = bp * bm;
@@ -359,13 +378,13 @@ template <class R> __device__ __forceinline__ V5<R> hlle(const V5<R>& WL, const 
 // HLLC with Toro's pressure-based wave-speed estimates (S9)
 template <class R> __device__ __forceinline__ V5<R> hllc(const V5<R>& WL, const V5<R>& WR, const Par<R>& p) {
   const R g = p.gamma;
-  const R cL = m_sqrt(g * WL[4] / WL[0]), cR = m_sqrt(g * WR[4] / WR[0]);
+  const R cL = m_sqrt(m_div(g * WL[4], WL[0])), cR = m_sqrt(m_div(g * WR[4], WR[0]));
   const R rb = R(0.5) * (WL[0] + WR[0]), cb = R(0.5) * (cL + cR);
   const R ppv = R(0.5) * (WL[4] + WR[4]) - R(0.5) * (WR[1] - WL[1]) * rb * cb;
   const R ps = m_max(R(0), ppv);
-  const R gf = (g + R(1)) / (R(2) * g);
-  const R qL = (ps <= WL[4]) ? R(1) : m_sqrt(R(1) + gf * (ps / WL[4] - R(1)));
-  const R qR = (ps <= WR[4]) ? R(1) : m_sqrt(R(1) + gf * (ps / WR[4] - R(1)));
+  const R gf = m_div(g + R(1), R(2) * g);
+  const R qL = (ps <= WL[4]) ? R(1) : m_sqrt(R(1) + gf * (m_div(ps, WL[4]) - R(1)));
+  const R qR = (ps <= WR[4]) ? R(1) : m_sqrt(R(1) + gf * (m_div(ps, WR[4]) - R(1)));
   const R SL = WL[1] - cL * qL, SR = WR[1] + cR * qR;
   V5<R> UL, UR, FL, FR;
   flux_and_cons(WL, p, FL, UL);
@@ -373,20 +392,20 @@ template <class R> __device__ __forceinline__ V5<R> hllc(const V5<R>& WL, const 
   if (SL >= R(0)) return FL;
   if (SR <= R(0)) return FR;
   const R mL = WL[0] * (SL - WL[1]), mR = WR[0] * (SR - WR[1]);
-  const R Ss = ((WR[4] - WL[4]) + WL[1] * mL - WR[1] * mR) / (mL - mR);
+  const R Ss = m_div((WR[4] - WL[4]) + WL[1] * mL - WR[1] * mR, mL - mR);
   // pick the star region containing x/t = 0 (S19: S* = 0 -> left star)
   const bool left = Ss >= R(0);
   const V5<R>& WK = left ? WL : WR;
   const V5<R>& UK = left ? UL : UR;
   const V5<R>& FK = left ? FL : FR;
   const R SK = left ? SL : SR, mK = left ? mL : mR;
-  const R f = mK / (SK - Ss);
+  const R f = m_div(mK, SK - Ss);
   V5<R> Us;
   Us[0] = f;
   Us[1] = f * Ss;
   Us[2] = f * WK[2];
   Us[3] = f * WK[3];
-  Us[4] = f * (UK[4] / WK[0] + (Ss - WK[1]) * (Ss + WK[4] / mK));
+  Us[4] = f * (m_div(UK[4], WK[0]) + (Ss - WK[1]) * (Ss + m_div(WK[4], mK)));
   V5<R> F;
 #pragma unroll
   for (int q = 0; q < 5; ++q) F[q] = FK[q] + SK * (Us[q] - UK[q]);
@@ -398,22 +417,22 @@ template <class R>
 __device__ __forceinline__ void pressure_fn(R ps, R rhoK, R PK, R cK, const Par<R>& p, R& f, R& df) {
   const R g = p.gamma;
   if (ps > PK) {  // shock branch
-    const R A = R(2) / ((g + R(1)) * rhoK), B = p.gm1 / (g + R(1)) * PK;
-    const R s = m_sqrt(A / (ps + B));
+    const R A = m_div(R(2), (g + R(1)) * rhoK), B = m_div(p.gm1, g + R(1)) * PK;
+    const R s = m_sqrt(m_div(A, ps + B));
     f = (ps - PK) * s;
-    df = s * (R(1) - (ps - PK) / (R(2) * (B + ps)));
+    df = s * (R(1) - m_div(ps - PK, R(2) * (B + ps)));
   } else {  // rarefaction branch
-    const R pr = ps / PK;
-    f = R(2) * cK / p.gm1 * (m_pow(pr, p.gm1 / (R(2) * g)) - R(1));
-    df = m_pow(pr, -(g + R(1)) / (R(2) * g)) / (rhoK * cK);
+    const R pr = m_div(ps, PK);
+    f = R(2) * cK * p.igm1 * (m_pow(pr, m_div(p.gm1, R(2) * g)) - R(1));
+    df = m_div(m_pow(pr, m_div(-(g + R(1)), R(2) * g)), rhoK * cK);
   }
 }
 
 template <class R> __device__ __noinline__ V5<R> exact(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
   const R g = p.gamma;
-  const R cL = m_sqrt(g * WL[4] / WL[0]), cR = m_sqrt(g * WR[4] / WR[0]);
+  const R cL = m_sqrt(m_div(g * WL[4], WL[0])), cR = m_sqrt(m_div(g * WR[4], WR[0]));
   const R du = WR[1] - WL[1];
-  if (R(2) * (cL + cR) / p.gm1 <= du) {  // vacuum generation -> HLLE flux
+  if (R(2) * (cL + cR) * p.igm1 <= du) {  // vacuum generation -> HLLE flux
     c.exact++;
     return hlle(WL, WR, p);
   }
@@ -425,9 +444,9 @@ template <class R> __device__ __noinline__ V5<R> exact(const V5<R>& WL, const V5
   for (int it = 0; it < 40; ++it) {
     pressure_fn(ps, WL[0], WL[4], cL, p, fL, dL);
     pressure_fn(ps, WR[0], WR[4], cR, p, fR, dR);
-    R pn = ps - ((fL + fR) + du) / (dL + dR);
+    R pn = ps - m_div((fL + fR) + du, dL + dR);
     if (!(pn > R(0))) pn = epsp;
-    const R chg = R(2) * m_abs(pn - ps) / (pn + ps);
+    const R chg = m_div(R(2) * m_abs(pn - ps), pn + ps);
     ps = pn;
     if (chg < ExactTol<R>::v()) {
       conv = true;
@@ -443,30 +462,30 @@ template <class R> __device__ __noinline__ V5<R> exact(const V5<R>& WL, const V5
   const R sg = left ? R(1) : R(-1);  // mirror the right side onto the left-side formulas
   const R rK = left ? WL[0] : WR[0], PK = left ? WL[4] : WR[4], cK = left ? cL : cR;
   const R vK = left ? WL[1] : WR[1];
-  const R mu = p.gm1 / (g + R(1));
-  const R pr = ps / PK;
+  const R mu = m_div(p.gm1, g + R(1));
+  const R pr = m_div(ps, PK);
   V5<R> W;
   W[2] = left ? WL[2] : WR[2];
   W[3] = left ? WL[3] : WR[3];
   // in the mirrored frame velocities are s*v and the wave runs to the left
   if (ps > PK) {  // shock
-    const R S = vK - sg * cK * m_sqrt((g + R(1)) / (R(2) * g) * pr + p.gm1 / (R(2) * g));
+    const R S = vK - sg * cK * m_sqrt(m_div(g + R(1), R(2) * g) * pr + m_div(p.gm1, R(2) * g));
     const bool undisturbed = left ? (S >= R(0)) : (S <= R(0));
     if (undisturbed) { W[0] = rK; W[1] = vK; W[4] = PK; }
-    else { W[0] = rK * (pr + mu) / (mu * pr + R(1)); W[1] = us; W[4] = ps; }
+    else { W[0] = m_div(rK * (pr + mu), mu * pr + R(1)); W[1] = us; W[4] = ps; }
   } else {  // rarefaction
     const R head = vK - sg * cK;
-    const R cs = cK * m_pow(pr, p.gm1 / (R(2) * g));
+    const R cs = cK * m_pow(pr, m_div(p.gm1, R(2) * g));
     const R tail = us - sg * cs;
     const bool before_head = left ? (head >= R(0)) : (head <= R(0));
     const bool behind_tail = left ? (tail <= R(0)) : (tail >= R(0));
     if (before_head) { W[0] = rK; W[1] = vK; W[4] = PK; }
-    else if (behind_tail) { W[0] = rK * m_pow(pr, R(1) / g); W[1] = us; W[4] = ps; }
+    else if (behind_tail) { W[0] = rK * m_pow(pr, m_rcp(g)); W[1] = us; W[4] = ps; }
     else {
-      const R phi = R(2) / (g + R(1)) + sg * mu * vK / cK;
-      W[0] = rK * m_pow(phi, R(2) / p.gm1);
-      W[1] = R(2) / (g + R(1)) * (sg * cK + R(0.5) * p.gm1 * vK);
-      W[4] = PK * m_pow(phi, R(2) * g / p.gm1);
+      const R phi = m_div(R(2), g + R(1)) + m_div(sg * mu * vK, cK);
+      W[0] = rK * m_pow(phi, R(2) * p.igm1);
+      W[1] = m_div(R(2), g + R(1)) * (sg * cK + R(0.5) * p.gm1 * vK);
+      W[4] = PK * m_pow(phi, R(2) * g * p.igm1);
     }
   }
   return phys_flux(W, p);
@@ -499,8 +518,8 @@ template <class R> __device__ __forceinline__ V5<R> roe(const V5<R>& WL, const V
     A[q] = UL[q] + a1 * K1[q];
     B[q] = UR[q] - a5 * K5[q];
   }
-  const R PA = p.gm1 * (A[4] - R(0.5) * ((A[1] * A[1] + A[2] * A[2]) + A[3] * A[3]) / A[0]);
-  const R PB = p.gm1 * (B[4] - R(0.5) * ((B[1] * B[1] + B[2] * B[2]) + B[3] * B[3]) / B[0]);
+  const R PA = p.gm1 * (A[4] - R(0.5) * m_div((A[1] * A[1] + A[2] * A[2]) + A[3] * A[3], A[0]));
+  const R PB = p.gm1 * (B[4] - R(0.5) * m_div((B[1] * B[1] + B[2] * B[2]) + B[3] * B[3], B[0]));
   if (!(A[0] > R(0)) || !(PA > R(0)) || !(B[0] > R(0)) || !(PB > R(0))) {
     c.roe_fb++;
     if (p.roe_fallback == 2) return hllc(WL, WR, p);
