@@ -59,6 +59,25 @@ constexpr bool fused_fits(int precision_bytes, int scheme, int recon, int g) {
          ctu_smem_bytes((size_t)precision_bytes, recon, g, ctu_sm_mask((size_t)precision_bytes)) <= SMEM_MAX_OPTIN;
 }
 
+// ---- warp-specialised fused CTU kernel (hydro_ws_ctu.cuh): predictor group + corrector group -------
+constexpr int WS_NT1 = 352;                         // group P: one thread per column (+ idle lanes of warp 10)
+constexpr int WS_NT2 = 288;                         // group C: one thread per face, compacted
+constexpr int WS_NT = WS_NT1 + WS_NT2;
+constexpr int WS_COLS = FUSED_COLS;
+constexpr bool ws_available(int precision_bytes, int scheme, int recon) {
+  (void)recon;
+  return precision_bytes == 4 && scheme == SCHEME_CTU;
+}
+// mbarriers | raw planes [2][5][S*S] | W ring | hand-off [2][9][5][324] | F* exchange [2][5][324] | F buffers [2][2][5][324]
+constexpr size_t ws_smem_bytes(size_t elem, int recon, int g) {
+  const size_t S = PS + 2 * g, SWP = PS + 2 * (2 + recon), NW = 2 * (1 + recon) + 1;
+  return 64 + elem * (2 * 5 * S * S + NW * 5 * SWP * SWP + (size_t)(2 * 9 + 2 + 4) * 5 * WS_COLS);
+}
+constexpr bool ws_fits(int precision_bytes, int scheme, int recon, int g) {
+  return ws_available(precision_bytes, scheme, recon) && ws_smem_bytes((size_t)precision_bytes, recon, g) <= SMEM_MAX_OPTIN;
+}
+
+template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_ws(const SolveArgs<R>& a);
 template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_staged(const SolveArgs<R>& a);
 template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_fused(const SolveArgs<R>& a);
 

@@ -18,7 +18,7 @@ MHM, VL, CTU = 0, 1, 2
 EXACT, HLLE, HLLC, ROE = 0, 1, 2, 3
 GMINMOD, VANLEER, VANALBADA, HYBRID = 0, 1, 2, 3
 PLM, PPM = 0, 1
-AUTO, STAGED, FUSED = 0, 1, 2
+AUTO, STAGED, FUSED, WS = 0, 1, 2, 3
 PS = 16
 TOL64, TOL32 = 1e-12, 1e-5
 
@@ -69,7 +69,12 @@ def check(out, ff, ref_out, ref_ff, dtype, what):
 def impls(B, dtype, scheme, recon, g=0):
     import torch
     t = {np.float32: torch.float32, np.float64: torch.float64}[dtype]
-    return (STAGED, FUSED) if B.hydro_fused_fits(t, scheme, recon, g) else (STAGED,)
+    r = (STAGED,)
+    if B.hydro_fused_fits(t, scheme, recon, g):
+        r += (FUSED,)
+    if B.hydro_ws_fits(t, scheme, recon, g):
+        r += (WS,)
+    return r
 
 
 def gpu_solve(B, G, dt, dh, gamma, scheme, riemann, limiter, impl, **kw):
