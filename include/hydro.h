@@ -59,8 +59,9 @@ enum { HYDRO_GMINMOD = 0, HYDRO_VANLEER = 1, HYDRO_VANALBADA = 2, HYDRO_HYBRID =
 enum { HYDRO_PLM = 0, HYDRO_PPM = 1 };                                     /* recon */
 /* kernel organisation (all compute the same update): staged = one phase per stage with global scratch (any
  * variant, any ghost width); fused = z-marching, single-role CTAs; ws = z-marching, warp-specialised
- * predictor / corrector groups.  AUTO picks ws, else fused, else staged, by availability and shared-memory fit. */
-enum { HYDRO_IMPL_AUTO = 0, HYDRO_IMPL_STAGED = 1, HYDRO_IMPL_FUSED = 2, HYDRO_IMPL_WS = 3 };
+ * predictor / corrector groups; lean = z-marching, phase-crossing state in shared memory, two CTAs per SM.
+ * AUTO picks lean, else ws, else fused, else staged, by availability and shared-memory fit. */
+enum { HYDRO_IMPL_AUTO = 0, HYDRO_IMPL_STAGED = 1, HYDRO_IMPL_FUSED = 2, HYDRO_IMPL_WS = 3, HYDRO_IMPL_LEAN = 4 };
 
 enum {
   HYDRO_OK = 0,
@@ -71,7 +72,7 @@ enum {
   HYDRO_E_GHOST = -5,     /* nghost < hydro_min_ghost(scheme, recon), or > 8 */
   HYDRO_E_WORKSPACE = -6, /* staged path selected and workspace missing / smaller than one slot */
   HYDRO_E_VALUE = -7,     /* gamma <= 1, dh <= 0, dt < 0, minmod_coeff outside [1,2], negative floor, cfl <= 0 */
-  HYDRO_E_NOFUSED = -8    /* impl == HYDRO_IMPL_FUSED / HYDRO_IMPL_WS and no such kernel exists (or fits) for this variant */
+  HYDRO_E_NOFUSED = -8    /* impl == HYDRO_IMPL_FUSED / _WS / _LEAN and no such kernel exists (or fits) for this variant */
 };
 
 typedef struct hydro_opts {      /* NULL => all defaults */
@@ -134,6 +135,8 @@ HYDRO_API int hydro_has_fused(int precision_bytes, int scheme, int recon, int ri
 HYDRO_API int hydro_fused_fits(int precision_bytes, int scheme, int recon, int nghost);
 /* 1 if a warp-specialised fused kernel exists for (precision, scheme, recon) and fits for ghost width nghost */
 HYDRO_API int hydro_ws_fits(int precision_bytes, int scheme, int recon, int nghost);
+/* 1 if a lean fused kernel exists for (precision, scheme, recon) and fits for ghost width nghost */
+HYDRO_API int hydro_lean_fits(int precision_bytes, int scheme, int recon, int nghost);
 /* bytes of opts->workspace that hydro_solve_* may need in HYDRO_IMPL_AUTO mode for any ghost width
  * (0 only when the fused kernel runs for every nghost <= 8) */
 HYDRO_API size_t hydro_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon);

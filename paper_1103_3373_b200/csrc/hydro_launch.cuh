@@ -77,6 +77,24 @@ constexpr bool ws_fits(int precision_bytes, int scheme, int recon, int g) {
   return ws_available(precision_bytes, scheme, recon) && ws_smem_bytes((size_t)precision_bytes, recon, g) <= SMEM_MAX_OPTIN;
 }
 
+// ---- lean fused CTU kernel (hydro_lean_ctu.cuh): column-per-thread z-march, phase-crossing state in shared memory,
+// two co-resident CTAs per SM where the tiles allow ------------------------------------------------------------
+constexpr int LEAN_NT = 320;                        // 10 warps: 288 columns of the rows j = 0..15, 32 of the rows j = -1, 16
+constexpr int LEAN_COLS = FUSED_COLS;
+// mbarriers | raw planes [2][5][S*S] | W ring | private z states [2][2][5][NT] | LOX UPX LOY UPY FX FY [6][5][324]
+constexpr size_t lean_smem_bytes(size_t elem, int recon, int g) {
+  const size_t S = PS + 2 * g, SWP = PS + 2 * (2 + recon), NW = 2 * (1 + recon) + 1;
+  return 64 + elem * (2 * 5 * S * S + NW * 5 * SWP * SWP + (size_t)20 * LEAN_NT + (size_t)30 * LEAN_COLS);
+}
+constexpr bool lean_available(int precision_bytes, int scheme, int recon) {
+  (void)precision_bytes; (void)recon;
+  return scheme == SCHEME_CTU;
+}
+constexpr bool lean_fits(int precision_bytes, int scheme, int recon, int g) {
+  return lean_available(precision_bytes, scheme, recon) && lean_smem_bytes((size_t)precision_bytes, recon, g) <= SMEM_MAX_OPTIN;
+}
+
+template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_lean(const SolveArgs<R>& a);
 template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_ws(const SolveArgs<R>& a);
 template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_staged(const SolveArgs<R>& a);
 template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_fused(const SolveArgs<R>& a);

@@ -1,0 +1,24 @@
+// hydro_lean.cuh -- dispatch of the lean fused kernels.  Variants without one return
+// cudaErrorNotSupported; the C ABI never reaches them because lean_available() gates the dispatch.
+#pragma once
+#include "hydro_launch.cuh"
+#include "hydro_lean_ctu.cuh"
+
+namespace hydro {
+
+// co-resident CTAs per SM the register budget is set for: two where the tiles of two groups fit (fp32, PLM)
+template <class R, int RECON> struct LeanTune { static constexpr int MINB = (sizeof(R) == 4 && RECON == RECON_PLM) ? 2 : 1; };
+
+template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_lean(const SolveArgs<R>& a) {
+  if constexpr (SCHEME == SCHEME_CTU) {
+    // compile-time specialisation of the default options: van Leer limiter on primitive variables, no floors
+    const bool fast = a.par.limiter == LIM_VANLEER && !a.par.char_limit && !(a.par.min_dens > R(0)) && !(a.par.min_pres > R(0));
+    if (fast) return launch_ctu_lean<R, RECON, RS, 1, LeanTune<R, RECON>::MINB>(a);
+    return launch_ctu_lean<R, RECON, RS, 0, LeanTune<R, RECON>::MINB>(a);
+  } else {
+    (void)a;
+    return cudaErrorNotSupported;
+  }
+}
+
+}  // namespace hydro

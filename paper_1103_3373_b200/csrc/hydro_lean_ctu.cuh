@@ -1,0 +1,352 @@
+// hydro_lean_ctu.cuh -- "lean" fused z-marching CTU kernel (steps (1)-(5) in one launch).
+//
+// Design point (from the ncu captures of the first two fused kernels, profiles/): the path is bound by
+// instruction issue.  The single-role kernel needed 168 registers (11 warps per SM, issue slots half
+// empty); the warp-specialised one left its corrector group waiting 40 % of the time.  This kernel keeps
+// the column-per-thread z-march but holds only 15 carried values per thread in registers; everything
+// that crosses a phase boundary lives in shared memory, so that a 320-thread CTA fits in 96 registers and
+// about 108 KB of shared memory (fp32, PLM) and TWO CTAs (two patch groups) are resident per SM, each
+// hiding the other's barriers.  The arithmetic is the instruction-lean form of hydro_lean_math.cuh.
+//
+// Thread -> column of the 18 x 18 tile (interior + one-cell ring): warps 0-8 own rows j = 0..15 (18
+// columns each, i = -1..16), warp 9 owns the rows j = -1 and j = 16 (i = 0..15) and, in a second pass of
+// phases C and D, the four corner columns (which only feed F*_x / F*_y of the ring).
+//
+// Step t = -2 .. 16 of a group (plane index; W = primitive planes in a ring, one plane converted per step):
+//   B  z: traced states of plane t+1 (own column of the ring planes) -> private slots;
+//         F*_z(t+1) = RS(up_z(t), lo_z(t+1)); dF*_z(t) kept in registers
+//   C  x,y: traced states of plane t -> LOX, UPX, LOY, UPY                                  | barrier 1
+//   D  F*_x(t), F*_y(t) -> FX, FY;  con->prim of the next raw plane into the ring           | barrier 2
+//   E  transverse correction (half nu, S4) of the x,y states in place and of the z states;
+//      F_z(t) = RS(up_z'(t-1), lo_z'(t)); conservative update + store of plane t-1          | barrier 3
+//   F  F_x(t), F_y(t) -> FX, FY; patch-boundary flux stores                                 | barrier 4
+//   G  carried D_z = (dF_x + dF_y)(t) - F_z(t), so that the update is U - nu (D_z + F_z(t+1))
+// Input planes arrive by 1-D bulk async copies (cp.async.bulk + mbarrier), two planes in flight, running
+// ahead across group boundaries.
+#pragma once
+#include <cstdint>
+#include "hydro_launch.cuh"
+#include "hydro_lean_math.cuh"
+#include "hydro_ptx.cuh"
+
+namespace hydro {
+
+enum : int { LR_Z = 1, LR_FX = 2, LR_FY = 4, LR_INI = 8, LR_INJ = 16, LR_INT = 32, LR_RC = 64 };
+enum : int { LF_LOX = 0, LF_UPX, LF_LOY, LF_UPY, LF_FX, LF_FY };
+
+// variant seams: FAST = van Leer limiter on primitive variables, no floors (compile time)
+template <class R, int RECON, int RS, int FAST> struct LeanOps {
+  static __device__ __forceinline__ V5<R> c2p(const V5<R>& U, const Par<R>& p, Cnt& c) {
+    if (FAST) return lean_cons2prim(U, p, c.bad);
+    return cons2prim(U, p, c);
+  }
+  static __device__ __forceinline__ V5<R> correct(const V5<R>& W, const V5<R>& dq, const Par<R>& p, Cnt& c) {
+    if (FAST) return lean_correct(W, dq, p, c.bad);
+    V5<R> U = prim2cons(W, p);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) U[q] = U[q] - dq[q];
+    return cons2prim(U, p, c);
+  }
+  // traced face states of the middle cell of a normal-frame pencil
+  static __device__ __forceinline__ void recon(const V5<R>& Wm2, const V5<R>& Wm1, const V5<R>& W0, const V5<R>& Wp1,
+                                               const V5<R>& Wp2, const Par<R>& p, V5<R>& lo, V5<R>& up) {
+    if (FAST && RECON == RECON_PLM) lean_plm_trace(Wm1, W0, Wp1, p, p.nu, p.hnu, lo, up);
+    else reconstruct<RECON, true>(Wm2, Wm1, W0, Wp1, Wp2, p, lo, up);
+  }
+  template <int D> static __device__ __forceinline__ V5<R> riemann(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
+    const V5<R> l = to_normal<D>(WL), r = to_normal<D>(WR);
+    if (FAST && RS == RS_ROE) return from_normal<D>(lean_roe(l, r, p, c));
+    if (FAST && RS == RS_HLLC) return from_normal<D>(lean_hllc(l, r, p));
+    return from_normal<D>(riemann_n<RS>(l, r, p, c));
+  }
+};
+
+template <class R, int RECON, int RS, int FAST, int MINB>
+__global__ void __launch_bounds__(LEAN_NT, MINB)
+ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, Par<R> p,
+                const R* __restrict__ max_speed, R cfl, long long* status) {
+  using Op = LeanOps<R, RECON, RS, FAST>;
+  constexpr int GW = 2 + RECON, RW = 1 + RECON, SWP = PS + 2 * GW, WPL = SWP * SWP, NW = 2 * RW + 1, NPL = PS + 2 * GW;
+  constexpr int NC = LEAN_COLS, NT = LEAN_NT, FT = PS + 2;
+  apply_device_dt(p, max_speed, cfl);
+
+  const int S = PS + 2 * g;
+  const int SS = S * S;
+  const size_t nS = (size_t)SS * S;
+  const int off = g - GW;  // unused outer ghost layers
+
+  extern __shared__ __align__(16) unsigned char smem[];
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
+  R* raw = reinterpret_cast<R*>(smem + 64);            // [2][5][SS]      landing zone of the bulk copies
+  R* ring = raw + (size_t)2 * 5 * SS;                  // [NW][5][WPL]    primitive planes
+  R* zs = ring + (size_t)NW * 5 * WPL;                 // [2][2][5][NT]   private traced z states (lo, up) of planes t, t+1
+  R* xy = zs + (size_t)2 * 2 * 5 * NT;                 // [6][5][NC]      LOX UPX LOY UPY FX FY
+
+  const int tid = threadIdx.x;
+  // ---- column and role of this thread (pass 0) and, for warp 9, of its corner column (pass 1)
+  int ii, jj;
+  if (tid < PS * FT) { jj = 1 + tid / FT; ii = tid - (jj - 1) * FT; }
+  else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
+  const int col0 = jj * FT + ii;
+  const bool in_i = ii >= 1 && ii <= PS, in_j = jj >= 1 && jj <= PS;
+  const int role0 = LR_Z | LR_RC | (ii >= 1 ? LR_FX : 0) | (jj >= 1 ? LR_FY : 0) | (in_i ? LR_INI : 0) | (in_j ? LR_INJ : 0) |
+                    ((in_i && in_j) ? LR_INT : 0);
+  const int npass = (tid >= PS * FT) ? 2 : 1;  // warp-uniform
+  const int cl = tid - PS * FT;                // corner id for lanes 0..3 of warp 9
+  const int ci = (cl & 1) ? FT - 1 : 0, cj = (cl & 2) ? FT - 1 : 0;
+  const int col1 = cj * FT + ci;
+  const int role1 = (cl >= 0 && cl < 4) ? (LR_RC | (ci >= 1 ? LR_FX : 0) | (cj >= 1 ? LR_FY : 0)) : 0;
+  const int wb0 = (jj + GW - 1) * SWP + (ii + GW - 1);  // own index in a primitive plane
+
+  // ---- plane pipeline: sequence number n = m * NPL + (plane + GW) over this CTA's groups m
+  const int my_groups = (Ng - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int total_planes = my_groups * NPL;
+  auto issue = [&](int n) {  // thread 0 only
+    if (n >= total_planes) return;
+    const int m = n / NPL, pl = n - m * NPL;
+    const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
+    const R* src = in + grp * 5 * nS + (size_t)(pl + off) * SS;
+    uint64_t* b = bar + (n & 1);
+    R* dst = raw + (size_t)(n & 1) * 5 * SS;
+    mbar_expect_tx(b, (uint32_t)(5 * SS * sizeof(R)));
+#pragma unroll
+    for (int q = 0; q < 5; ++q) bulk_g2s(dst + (size_t)q * SS, src + q * nS, (uint32_t)(SS * sizeof(R)), b);
+  };
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    mbar_init(bar + 1, 1);
+    fence_mbar_init();
+    fence_async_smem();
+  }
+  __syncthreads();
+  if (tid == 0) { issue(0); issue(1); }
+
+  Cnt c = {0, 0, 0};
+  int nseq = 0;  // planes converted so far
+  // con->prim of the next raw plane into ring slot `slot` (all threads)
+  auto convert = [&](int slot) {
+    const int st = nseq & 1;
+    mbar_wait(bar + st, (uint32_t)((nseq >> 1) & 1));
+    const R* rp = raw + (size_t)st * 5 * SS;
+    R* wp = ring + (size_t)slot * 5 * WPL;
+    for (int idx = tid; idx < WPL; idx += NT) {
+      const int b = idx / SWP, a = idx - b * SWP;
+      st5(wp + idx, WPL, Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c));
+    }
+  };
+  // after the barrier that follows a conversion: refill the raw stage it consumed
+  auto refill = [&]() {
+    if (tid == 0) { fence_async_smem(); issue(nseq + 2); }
+    ++nseq;
+  };
+
+  V5<R> f1z, uzc, Dz;  // F*_z at the lower face of plane t+1; corrected up_z of plane t-1; (dF_x + dF_y) - F_z of plane t-1
+#pragma unroll
+  for (int q = 0; q < 5; ++q) { f1z[q] = R(0); uzc[q] = R(0); Dz[q] = R(0); }
+
+  for (int m = 0; m < my_groups; ++m) {
+    const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
+    // ---- prologue: the first NW primitive planes (-GW .. -GW+NW-1)
+    for (int k = 0; k < NW; ++k) {
+      convert(k);
+      __syncthreads();
+      refill();
+    }
+
+#pragma unroll 1
+    for (int t = -2; t <= PS; ++t) {
+      const bool doxy = t >= -1;
+      const bool tin = t >= 0 && t < PS;
+      // ================= B: z states of plane t+1, F*_z(t+1) =================
+      V5<R> dFz;
+#pragma unroll
+      for (int q = 0; q < 5; ++q) dFz[q] = R(0);
+      if (t < PS) {
+        const int kz = t + 1;
+        V5<R> Wz[2 * RW + 1];
+#pragma unroll
+        for (int s = 0; s < 2 * RW + 1; ++s)
+          Wz[s] = to_normal<2>(ld5(ring + (size_t)((kz - RW + s + GW) % NW) * 5 * WPL + wb0, WPL));
+        V5<R> l, u;
+        Op::recon(Wz[0], Wz[RW - 1], Wz[RW], Wz[RW + 1], Wz[2 * RW], p, l, u);
+        const V5<R> lz = from_normal<2>(l), uz = from_normal<2>(u);
+        R* zn = zs + (size_t)(kz & 1) * 10 * NT + tid;
+        st5(zn, NT, lz);
+        st5(zn + 5 * NT, NT, uz);
+        if (kz >= 0) {
+          const V5<R> uzp = ld5(zs + (size_t)(t & 1) * 10 * NT + 5 * NT + tid, NT);
+          const V5<R> f = Op::template riemann<2>(uzp, lz, p, c);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) { dFz[q] = f[q] - f1z[q]; f1z[q] = f[q]; }
+        }
+      }
+      // ================= C: x,y traced states of plane t =================
+      if (doxy) {
+        const R* wpl = ring + (size_t)((t + GW) % NW) * 5 * WPL;
+        for (int ps = 0; ps < npass; ++ps) {
+          const int col = ps ? col1 : col0, role = ps ? role1 : role0;
+          if (role & LR_RC) {
+            const int cjj = col / FT, cii = col - cjj * FT;
+            const R* wt = wpl + (cjj + GW - 1) * SWP + (cii + GW - 1);
+            const V5<R> W0 = ld5(wt, WPL);
+            R* H = xy + col;
+            {
+              const V5<R> Wb = ld5(wt - 1, WPL), Wc = ld5(wt + 1, WPL);
+              V5<R> Wa = Wb, Wd = Wc;
+              if (RECON == RECON_PPM) { Wa = ld5(wt - 2, WPL); Wd = ld5(wt + 2, WPL); }
+              V5<R> l, u;
+              Op::recon(to_normal<0>(Wa), to_normal<0>(Wb), to_normal<0>(W0), to_normal<0>(Wc), to_normal<0>(Wd), p, l, u);
+              st5(H + LF_LOX * 5 * NC, NC, from_normal<0>(l));
+              st5(H + LF_UPX * 5 * NC, NC, from_normal<0>(u));
+            }
+            {
+              const V5<R> Wb = ld5(wt - SWP, WPL), Wc = ld5(wt + SWP, WPL);
+              V5<R> Wa = Wb, Wd = Wc;
+              if (RECON == RECON_PPM) { Wa = ld5(wt - 2 * SWP, WPL); Wd = ld5(wt + 2 * SWP, WPL); }
+              V5<R> l, u;
+              Op::recon(to_normal<1>(Wa), to_normal<1>(Wb), to_normal<1>(W0), to_normal<1>(Wc), to_normal<1>(Wd), p, l, u);
+              st5(H + LF_LOY * 5 * NC, NC, from_normal<1>(l));
+              st5(H + LF_UPY * 5 * NC, NC, from_normal<1>(u));
+            }
+          }
+        }
+      }
+      __syncthreads();  // barrier 1
+
+      // ================= D: F*_x(t), F*_y(t); con->prim of the next plane =================
+      if (doxy) {
+        for (int ps = 0; ps < npass; ++ps) {
+          const int col = ps ? col1 : col0, role = ps ? role1 : role0;
+          R* H = xy + col;
+          if (role & LR_FX)
+            st5(H + LF_FX * 5 * NC, NC,
+                Op::template riemann<0>(ld5(H + LF_UPX * 5 * NC - 1, NC), ld5(H + LF_LOX * 5 * NC, NC), p, c));
+          if (role & LR_FY)
+            st5(H + LF_FY * 5 * NC, NC,
+                Op::template riemann<1>(ld5(H + LF_UPY * 5 * NC - FT, NC), ld5(H + LF_LOY * 5 * NC, NC), p, c));
+        }
+      }
+      const bool conv = t + 2 + RW <= PS - 1 + GW;  // plane t+2+RW replaces plane t+1-RW (read for the last time in B)
+      if (conv) convert((t + 2 + RW + GW) % NW);
+      __syncthreads();  // barrier 2
+      if (conv) refill();
+
+      // ================= E: transverse correction, F_z(t), update of plane t-1 =========
+      if (doxy) {
+        R* H = xy + col0;
+        V5<R> Uold;
+        const bool upd = (role0 & LR_INT) && t >= 1;
+        if (upd) {
+          const R* gin = in + grp * 5 * nS + ((size_t)(t - 1 + g) * S + (jj - 1 + g)) * S + (ii - 1 + g);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) Uold[q] = __ldg(gin + q * nS);
+        }
+        V5<R> dFx, dFy;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { dFx[q] = R(0); dFy[q] = R(0); }
+        if (role0 & LR_INI) {
+          const V5<R> a = ld5(H + LF_FX * 5 * NC + 1, NC), b = ld5(H + LF_FX * 5 * NC, NC);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) dFx[q] = a[q] - b[q];
+        }
+        if (role0 & LR_INJ) {
+          const V5<R> a = ld5(H + LF_FY * 5 * NC + FT, NC), b = ld5(H + LF_FY * 5 * NC, NC);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) dFy[q] = a[q] - b[q];
+        }
+        if (tin && (role0 & LR_INJ)) {  // x states: t1 = y, t2 = z
+          V5<R> dq;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFy[q] + dFz[q]);
+          st5(H + LF_LOX * 5 * NC, NC, Op::correct(ld5(H + LF_LOX * 5 * NC, NC), dq, p, c));
+          st5(H + LF_UPX * 5 * NC, NC, Op::correct(ld5(H + LF_UPX * 5 * NC, NC), dq, p, c));
+        }
+        if (tin && (role0 & LR_INI)) {  // y states: t1 = z, t2 = x
+          V5<R> dq;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFz[q] + dFx[q]);
+          st5(H + LF_LOY * 5 * NC, NC, Op::correct(ld5(H + LF_LOY * 5 * NC, NC), dq, p, c));
+          st5(H + LF_UPY * 5 * NC, NC, Op::correct(ld5(H + LF_UPY * 5 * NC, NC), dq, p, c));
+        }
+        if (role0 & LR_INT) {  // z states: t1 = x, t2 = y; every plane t in [-1,16]
+          V5<R> dq;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFx[q] + dFy[q]);
+          const R* zc = zs + (size_t)(t & 1) * 10 * NT + tid;
+          if (t >= 0) {
+            const V5<R> lzc = Op::correct(ld5(zc, NT), dq, p, c);
+            const V5<R> Fz = Op::template riemann<2>(uzc, lzc, p, c);
+            if (face_flux && (t & 7) == 0)  // stored right after the solve
+              st5(face_flux + grp * 9 * 5 * PS * PS + (size_t)((6 + (t >> 3)) * 5) * 256 + (jj - 1) * PS + (ii - 1), 256, Fz);
+            if (upd) {
+              V5<R> U;
+#pragma unroll
+              for (int q = 0; q < 5; ++q) U[q] = Uold[q] - p.nu * (Dz[q] + Fz[q]);
+              const V5<R> Wn = Op::c2p(U, p, c);
+              if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
+              st5(out + grp * 5 * PS * PS * PS + ((t - 1) * PS + (jj - 1)) * PS + (ii - 1), PS * PS * PS, U);
+            }
+            Dz = Fz;
+          }
+          if (t < PS) uzc = Op::correct(ld5(zc + 5 * NT, NT), dq, p, c);
+        }
+      }
+      __syncthreads();  // barrier 3
+
+      // ================= F: final fluxes of plane t + boundary-flux store ============
+      if (tin) {
+        R* H = xy + col0;
+        R* gff = face_flux ? face_flux + grp * 9 * 5 * PS * PS : nullptr;
+        if ((role0 & (LR_INJ | LR_FX)) == (LR_INJ | LR_FX)) {
+          const V5<R> f = Op::template riemann<0>(ld5(H + LF_UPX * 5 * NC - 1, NC), ld5(H + LF_LOX * 5 * NC, NC), p, c);
+          st5(H + LF_FX * 5 * NC, NC, f);
+          if (gff && ((ii - 1) & 7) == 0) st5(gff + (size_t)(((ii - 1) >> 3) * 5) * 256 + t * PS + (jj - 1), 256, f);
+        }
+        if ((role0 & (LR_INI | LR_FY)) == (LR_INI | LR_FY)) {
+          const V5<R> f = Op::template riemann<1>(ld5(H + LF_UPY * 5 * NC - FT, NC), ld5(H + LF_LOY * 5 * NC, NC), p, c);
+          st5(H + LF_FY * 5 * NC, NC, f);
+          if (gff && ((jj - 1) & 7) == 0) st5(gff + (size_t)((3 + ((jj - 1) >> 3)) * 5) * 256 + t * PS + (ii - 1), 256, f);
+        }
+      }
+      __syncthreads();  // barrier 4
+
+      // ================= G: carried x+y flux difference of plane t minus F_z(t) =================
+      if (tin && (role0 & LR_INT)) {
+        const R* H = xy + col0;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          const R* fx = H + (LF_FX * 5 + q) * NC;
+          const R* fy = H + (LF_FY * 5 + q) * NC;
+          Dz[q] = ((fx[1] - fx[0]) + (fy[FT] - fy[0])) - Dz[q];
+        }
+      }
+    }
+  }
+  flush_counters(c, status);
+}
+
+// persistent grid: SMs x resident CTAs per SM (occupancy API), capped at Ng
+template <class R, int RECON, int RS, int FAST, int MINB> cudaError_t launch_ctu_lean(const SolveArgs<R>& a) {
+  auto kern = ctu_lean_kernel<R, RECON, RS, FAST, MINB>;
+  const size_t smem = lean_smem_bytes(sizeof(R), RECON, a.g);
+  if (smem > SMEM_MAX_OPTIN) return cudaErrorInvalidConfiguration;
+  static int sms = 0;
+  if (!sms) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (sms <= 0) sms = 148;
+  }
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, LEAN_NT, smem);
+  if (e != cudaSuccess) return e;
+  if (per_sm < 1) return cudaErrorInvalidConfiguration;
+  long long grid = (long long)sms * per_sm;
+  if (grid > a.Ng) grid = a.Ng;
+  kern<<<(unsigned)grid, LEAN_NT, smem, a.stream>>>(a.in, a.out, a.face_flux, a.Ng, a.g, a.par, a.max_speed, a.cfl, a.status);
+  return cudaGetLastError();
+}
+
+}  // namespace hydro

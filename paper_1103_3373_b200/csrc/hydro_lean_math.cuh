@@ -1,0 +1,213 @@
+// hydro_lean_math.cuh -- instruction-lean forms of the per-cell / per-face arithmetic for the
+// dominant variants (PLM + van Leer limiter on primitive variables, no floors; Roe and HLLC solvers).
+//
+// Same readings as hydro_math.cuh (S1-S24), algebraically rearranged so that the kernel
+// issues fewer instructions: the profile of the first fused kernels showed the path bound by
+// instruction issue, not by HBM (profiles/r1_ncu_ws_f32_v2.md), so what counts is the number of
+// FP32/FP64 + MUFU instructions per Riemann solve and per reconstruction.
+//   * branch-free limiter and tracing (selects, no divergent control flow);
+//   * the characteristic projection of the tracing written out per component with one rsqrt
+//     (1/(rho c)) instead of rcp + sqrt + rcp;
+//   * Roe wave strengths from the primitive jumps (drho, du, dp with rho~ = sqrt(rhoL rhoR)), which
+//     equal the conserved-jump strengths of S-c4 identically for Roe averages (Roe 1981, sec. 4);
+//     enthalpy from H = gamma/(gamma-1) P/rho + |v|^2/2 and the energy flux as (rho u) H;
+//   * the Roe failure test without divisions: P* > 0  <=>  2 E* rho* - |m*|^2 > 0.
+// Results differ from hydro_math.cuh by rounding only; parity with the oracle is what tests/ checks.
+// Part of the CUDA product path; shares nothing with oracle/.
+#pragma once
+#include "hydro_math.cuh"
+
+namespace hydro {
+
+#if HYDRO_F32_IEEE
+__device__ __forceinline__ float m_rsqrt(float x) { return 1.0f / sqrtf(x); }
+#else
+__device__ __forceinline__ float m_rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#endif
+__device__ __forceinline__ double m_rsqrt(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ float m_fma(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double m_fma(double a, double b, double c) { return fma(a, b, c); }
+
+// ---- c0: conversions --------------------------------------------------------------------------
+// rho |v|^2 is formed as m . v (3 instructions); `bad` counts non-positive rho / P (status[1])
+template <class R> __device__ __forceinline__ V5<R> lean_cons2prim(const V5<R>& U, const Par<R>& p, int& bad) {
+  const R ir = m_rcp(U[0]);
+  V5<R> W;
+  W[0] = U[0];
+  W[1] = U[1] * ir;
+  W[2] = U[2] * ir;
+  W[3] = U[3] * ir;
+  const R mv = m_fma(U[3], W[3], m_fma(U[2], W[2], U[1] * W[1]));
+  W[4] = p.gm1 * m_fma(R(-0.5), mv, U[4]);
+  bad += (U[0] > R(0) && W[4] > R(0)) ? 0 : 1;
+  return W;
+}
+
+// transverse correction of one face state: W <- prim(cons(W) - dq)
+template <class R> __device__ __forceinline__ V5<R> lean_correct(const V5<R>& W, const V5<R>& dq, const Par<R>& p, int& bad) {
+  V5<R> U;
+  U[0] = W[0] - dq[0];
+  U[1] = m_fma(W[0], W[1], -dq[1]);
+  U[2] = m_fma(W[0], W[2], -dq[2]);
+  U[3] = m_fma(W[0], W[3], -dq[3]);
+  const R q2 = m_fma(W[3], W[3], m_fma(W[2], W[2], W[1] * W[1]));
+  U[4] = m_fma(W[4], p.igm1, m_fma(R(0.5) * W[0], q2, -dq[4]));
+  return lean_cons2prim(U, p, bad);
+}
+
+// ---- c1-c3: PLM + van Leer limiter on primitive variables + CTU tracing (normal frame) ---------
+template <class R> __device__ __forceinline__ R vl_slope(R dL, R dR) {
+  const R prod = dL * dR;
+  const R s = m_div(prod + prod, dL + dR);
+  return prod > R(0) ? s : R(0);  // S19; the select also discards inf/NaN of the unused quotient
+}
+
+template <class R>
+__device__ __forceinline__ void lean_plm_trace(const V5<R>& Wm, const V5<R>& W0, const V5<R>& Wp, const Par<R>& p, R nu, R hnu,
+                                               V5<R>& lo, V5<R>& up) {
+  V5<R> s;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) s[q] = vl_slope(W0[q] - Wm[q], Wp[q] - W0[q]);
+  // eigen-system scalars from one rsqrt: irc = 1/(rho c), c = gamma P irc, 1/c = rho irc
+  const R gP = p.gamma * W0[4], x = gP * W0[0];
+  const R irc = m_rsqrt(x);
+  const R c = gP * irc, ic = W0[0] * irc, ic2 = ic * ic, rc = x * irc;
+  const R u = W0[1], lamM = u + c, lam0 = u - c;
+  const R nc = nu * c, hnc = R(0.5) * nc;
+  // S5 / S19: only waves approaching the face, lambda = 0 contributes to neither
+  const R b0 = lam0 > R(0) ? nc : R(0);     // (nu/2)(lamM - lam0)
+  const R b1 = u > R(0) ? hnc : R(0);       // (nu/2)(lamM - u)
+  const R g1 = u < R(0) ? -hnc : R(0);      // (nu/2)(lam0 - u)
+  const R g4 = lamM < R(0) ? -nc : R(0);    // (nu/2)(lam0 - lamM)
+  const R kp = m_fma(-hnu, m_max(lamM, R(0)), R(0.5));
+  const R km = m_fma(-hnu, m_min(lam0, R(0)), R(-0.5));
+  const R Z = rc * s[1];                          // rho c du
+  const R B0 = b0 * (R(0.5) * (s[4] - Z));        // coefficient x (L_0 . s) c^2
+  const R B4 = g4 * (R(0.5) * (s[4] + Z));
+  const R e1 = m_fma(-s[4], ic2, s[0]);           // entropy-wave amplitude
+  up[0] = m_fma(B0, ic2, m_fma(b1, e1, m_fma(kp, s[0], W0[0])));
+  up[1] = m_fma(-B0, irc, m_fma(kp, s[1], W0[1]));
+  up[2] = m_fma(kp + b1, s[2], W0[2]);
+  up[3] = m_fma(kp + b1, s[3], W0[3]);
+  up[4] = m_fma(kp, s[4], W0[4]) + B0;
+  lo[0] = m_fma(B4, ic2, m_fma(g1, e1, m_fma(km, s[0], W0[0])));
+  lo[1] = m_fma(B4, irc, m_fma(km, s[1], W0[1]));
+  lo[2] = m_fma(km + g1, s[2], W0[2]);
+  lo[3] = m_fma(km + g1, s[3], W0[3]);
+  lo[4] = m_fma(km, s[4], W0[4]) + B4;
+}
+
+// ---- c4: Roe's solver, primitive-jump form (normal frame in, normal-frame flux out) ------------
+template <class R> struct LeanState { R ir, H, m, F1, F2, F3, F4; };
+template <class R> __device__ __forceinline__ LeanState<R> lean_state(const V5<R>& W, R g1) {
+  LeanState<R> s;
+  s.ir = m_rcp(W[0]);
+  const R q2 = m_fma(W[3], W[3], m_fma(W[2], W[2], W[1] * W[1]));
+  s.H = m_fma(R(0.5), q2, (g1 * W[4]) * s.ir);
+  s.m = W[0] * W[1];
+  s.F1 = m_fma(s.m, W[1], W[4]);
+  s.F2 = s.m * W[2];
+  s.F3 = s.m * W[3];
+  s.F4 = s.m * s.H;
+  return s;
+}
+
+// the rare path: Roe failed at this face -> HLLE / HLLC / exact flux of the same states
+template <class R> __device__ __noinline__ void roe_fallback_flux(const V5<R>* WL, const V5<R>* WR, const Par<R>* p, int* cnt_exact, V5<R>* F) {
+  Cnt c = {0, 0, 0};
+  if (p->roe_fallback == 2) *F = hllc(*WL, *WR, *p);
+  else if (p->roe_fallback == 3) *F = exact(*WL, *WR, *p, c);
+  else *F = hlle(*WL, *WR, *p);
+  *cnt_exact += c.exact;
+}
+
+template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
+  const R g1 = p.gamma * p.igm1;
+  const LeanState<R> L = lean_state(WL, g1), Rr = lean_state(WR, g1);
+  // Roe averages with weights wL = sqrt(rhoL)/(sqrt(rhoL)+sqrt(rhoR)), wR = 1 - wL; rho~ = sqrt(rhoL rhoR)
+  const R r = m_sqrt(WR[0] * L.ir);
+  const R wR = r * m_rcp(R(1) + r);
+  const R rt = WL[0] * r;
+  const R du = WR[1] - WL[1], dv = WR[2] - WL[2], dw = WR[3] - WL[3];
+  const R ut = m_fma(wR, du, WL[1]), vt = m_fma(wR, dv, WL[2]), wt = m_fma(wR, dw, WL[3]);
+  const R Ht = m_fma(wR, Rr.H - L.H, L.H);
+  const R hq = R(0.5) * m_fma(wt, wt, m_fma(vt, vt, ut * ut));
+  const R a2 = p.gm1 * (Ht - hq);
+  const R a = m_sqrt(a2), ia2 = m_rcp(a2);
+  // wave strengths from the primitive jumps
+  const R dp = WR[4] - WL[4], dr = WR[0] - WL[0];
+  const R y = (rt * a) * du, h = R(0.5) * ia2;
+  const R al1 = (dp - y) * h, al5 = (dp + y) * h, al2 = m_fma(-dp, ia2, dr);
+  const R al3 = rt * dv, al4 = rt * dw;
+  const R um = ut - a, up = ut + a, ua = ut * a, H1 = Ht - ua, H5 = Ht + ua;
+  // failure test on U_L + al1 K1 and U_R - al5 K5 (rho > 0 and P > 0, the latter without a division)
+  {
+    const R A0 = WL[0] + al1, B0 = WR[0] - al5;
+    const R A1 = m_fma(al1, um, L.m), B1 = m_fma(-al5, up, Rr.m);
+    const R A2 = m_fma(al1, vt, WL[0] * WL[2]), B2 = m_fma(-al5, vt, WR[0] * WR[2]);
+    const R A3 = m_fma(al1, wt, WL[0] * WL[3]), B3 = m_fma(-al5, wt, WR[0] * WR[3]);
+    const R A4 = m_fma(al1, H1, m_fma(WL[0], L.H, -WL[4])), B4 = m_fma(-al5, H5, m_fma(WR[0], Rr.H, -WR[4]));
+    const R mA = m_fma(A3, A3, m_fma(A2, A2, A1 * A1)), mB = m_fma(B3, B3, m_fma(B2, B2, B1 * B1));
+    const R tA = m_fma(A4 + A4, A0, -mA), tB = m_fma(B4 + B4, B0, -mB);
+    if (!(A0 > R(0) && B0 > R(0) && tA > R(0) && tB > R(0))) {  // NaN fails the test
+      c.roe_fb++;
+      V5<R> F;
+      roe_fallback_flux(&WL, &WR, &p, &c.exact, &F);
+      return F;
+    }
+  }
+  const R w1 = al1 * m_abs(um), w2 = al2 * m_abs(ut), w5 = al5 * m_abs(up);
+  const R w3 = al3 * m_abs(ut), w4 = al4 * m_abs(ut);
+  const R d0 = (w1 + w2) + w5;
+  const R d1 = m_fma(w5, up, m_fma(w2, ut, w1 * um));
+  const R d2 = m_fma(d0, vt, w3);
+  const R d3 = m_fma(d0, wt, w4);
+  const R d4 = m_fma(w5, H5, m_fma(w4, wt, m_fma(w3, vt, m_fma(w2, hq, w1 * H1))));
+  V5<R> F;
+  F[0] = R(0.5) * ((L.m + Rr.m) - d0);
+  F[1] = R(0.5) * ((L.F1 + Rr.F1) - d1);
+  F[2] = R(0.5) * ((L.F2 + Rr.F2) - d2);
+  F[3] = R(0.5) * ((L.F3 + Rr.F3) - d3);
+  F[4] = R(0.5) * ((L.F4 + Rr.F4) - d4);
+  return F;
+}
+
+// ---- c4: HLLC, Toro's pressure-based speeds (S9), select form ----------------------------------
+template <class R> __device__ __forceinline__ V5<R> lean_hllc(const V5<R>& WL, const V5<R>& WR, const Par<R>& p) {
+  const R g = p.gamma;
+  const R irL = m_rcp(WL[0]), irR = m_rcp(WR[0]);
+  const R cL = m_sqrt(g * WL[4] * irL), cR = m_sqrt(g * WR[4] * irR);
+  const R ppv = R(0.5) * (WL[4] + WR[4]) - R(0.125) * (WR[1] - WL[1]) * (WL[0] + WR[0]) * (cL + cR);
+  const R ps = m_max(R(0), ppv);
+  const R gf = (g + R(1)) * (R(0.5) * m_rcp(g));
+  const R qL = (ps <= WL[4]) ? R(1) : m_sqrt(m_fma(gf, m_div(ps, WL[4]) - R(1), R(1)));
+  const R qR = (ps <= WR[4]) ? R(1) : m_sqrt(m_fma(gf, m_div(ps, WR[4]) - R(1), R(1)));
+  const R SL = m_fma(-cL, qL, WL[1]), SR = m_fma(cR, qR, WR[1]);
+  const R mL = WL[0] * (SL - WL[1]), mR = WR[0] * (SR - WR[1]);
+  const R Ss = m_div((WR[4] - WL[4]) + WL[1] * mL - WR[1] * mR, mL - mR);
+  // F_L if S_L >= 0, F_R if S_R <= 0, else the star state on the side of the contact (S19: S* = 0 -> left)
+  const bool supL = SL >= R(0), supR = SR <= R(0);
+  const bool left = supL || (!supR && Ss >= R(0));
+  const bool star = !supL && !supR;
+  const R rK = left ? WL[0] : WR[0], uK = left ? WL[1] : WR[1], vK = left ? WL[2] : WR[2], wK = left ? WL[3] : WR[3];
+  const R pK = left ? WL[4] : WR[4], SK = left ? SL : SR, mK = left ? mL : mR;
+  // physical flux and conserved vector of the chosen side
+  const R q2 = m_fma(wK, wK, m_fma(vK, vK, uK * uK));
+  const R E = m_fma(pK, p.igm1, R(0.5) * rK * q2);
+  const R mom = rK * uK;
+  V5<R> U, F;
+  U[0] = rK; U[1] = mom; U[2] = rK * vK; U[3] = rK * wK; U[4] = E;
+  F[0] = mom; F[1] = m_fma(mom, uK, pK); F[2] = mom * vK; F[3] = mom * wK; F[4] = (E + pK) * uK;
+  const R f = m_div(mK, SK - Ss);
+  V5<R> Us;
+  Us[0] = f;
+  Us[1] = f * Ss;
+  Us[2] = f * vK;
+  Us[3] = f * wK;
+  Us[4] = f * (m_div(E, rK) + (Ss - uK) * (Ss + m_div(pK, mK)));
+#pragma unroll
+  for (int q = 0; q < 5; ++q) F[q] = star ? m_fma(SK, Us[q] - U[q], F[q]) : F[q];
+  return F;
+}
+
+}  // namespace hydro

@@ -31,27 +31,6 @@
 
 namespace hydro {
 
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  while (!mbar_try_wait(bar, parity)) {}
-}
-template <int ID, int N> __device__ __forceinline__ void group_bar() {
-  asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(N) : "memory");
-}
-
-template <class R> __device__ __forceinline__ V5<R> ld5(const R* p, int stride) {
-  V5<R> x;
-#pragma unroll
-  for (int q = 0; q < 5; ++q) x[q] = p[q * stride];
-  return x;
-}
-template <class R> __device__ __forceinline__ void st5(R* p, int stride, const V5<R>& x) {
-#pragma unroll
-  for (int q = 0; q < 5; ++q) p[q * stride] = x[q];
-}
-
 // transverse correction of one face state: W <- prim(cons(W) - dq)
 template <class R> __device__ __forceinline__ V5<R> ctu_correct(const V5<R>& W, const V5<R>& dq, const Par<R>& p, Cnt& c) {
   V5<R> U = prim2cons(W, p);

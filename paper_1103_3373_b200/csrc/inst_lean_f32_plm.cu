@@ -1,0 +1,7 @@
+// explicit instantiations of the lean fused CTU kernel: float, RECON_PLM, four Riemann solvers (x fast / generic options)
+#include "hydro_lean.cuh"
+namespace hydro {
+#define INST(RS) template cudaError_t launch_lean<float, SCHEME_CTU, RECON_PLM, RS>(const SolveArgs<float>&);
+INST(RS_EXACT) INST(RS_HLLE) INST(RS_HLLC) INST(RS_ROE)
+#undef INST
+}  // namespace hydro

@@ -18,7 +18,7 @@ MHM, VL, CTU = 0, 1, 2
 EXACT, HLLE, HLLC, ROE = 0, 1, 2, 3
 GMINMOD, VANLEER, VANALBADA, HYBRID = 0, 1, 2, 3
 PLM, PPM = 0, 1
-AUTO, STAGED, FUSED, WS = 0, 1, 2, 3
+AUTO, STAGED, FUSED, WS, LEAN = 0, 1, 2, 3, 4
 PS = 16
 TOL64, TOL32 = 1e-12, 1e-5
 
@@ -74,6 +74,8 @@ def impls(B, dtype, scheme, recon, g=0):
         r += (FUSED,)
     if B.hydro_ws_fits(t, scheme, recon, g):
         r += (WS,)
+    if B.hydro_lean_fits(t, scheme, recon, g):
+        r += (LEAN,)
     return r
 
 
