@@ -6,11 +6,14 @@
 // the column-per-thread z-march but holds only 15 carried values per thread in registers; everything
 // that crosses a phase boundary lives in shared memory, so that a 320-thread CTA fits in 96 registers and
 // about 108 KB of shared memory (fp32, PLM) and TWO CTAs (two patch groups) are resident per SM, each
-// hiding the other's barriers.  The arithmetic is the instruction-lean form of hydro_lean_math.cuh.
+// hiding the other's barriers.  The arithmetic is the instruction-lean form of hydro_lean_math.cuh;
+// shared-memory fields use the packed "4+1" layout of hydro_ptx.cuh (2 instructions per 5-vector).
 //
 // Thread -> column of the 18 x 18 tile (interior + one-cell ring): warps 0-8 own rows j = 0..15 (18
-// columns each, i = -1..16), warp 9 owns the rows j = -1 and j = 16 (i = 0..15) and, in a second pass of
-// phases C and D, the four corner columns (which only feed F*_x / F*_y of the ring).
+// columns each, i = -1..16), warp 9 owns the rows j = -1 and j = 16 (i = 0..15).  The four corner columns
+// only feed F*_x / F*_y of the ring; their work rides on lanes that would otherwise idle: their traced
+// states are formed by 8 lanes of warp 9 during phase F of the previous step, their four first-pass
+// Riemann problems by the i = -1 lanes of warp 0 (F*_x) and the j = -1 lanes of warp 9 (F*_y) in phase D.
 //
 // Step t = -2 .. 16 of a group (plane index; W = primitive planes in a ring, one plane converted per step):
 //   B  z: traced states of plane t+1 (own column of the ring planes) -> private slots;
@@ -19,7 +22,7 @@
 //   D  F*_x(t), F*_y(t) -> FX, FY;  con->prim of the next raw plane into the ring           | barrier 2
 //   E  transverse correction (half nu, S4) of the x,y states in place and of the z states;
 //      F_z(t) = RS(up_z'(t-1), lo_z'(t)); conservative update + store of plane t-1          | barrier 3
-//   F  F_x(t), F_y(t) -> FX, FY; patch-boundary flux stores                                 | barrier 4
+//   F  F_x(t), F_y(t) -> FX, FY; patch-boundary flux stores; corner states of plane t+1     | barrier 4
 //   G  carried D_z = (dF_x + dF_y)(t) - F_z(t), so that the update is U - nu (D_z + F_z(t+1))
 // Input planes arrive by 1-D bulk async copies (cp.async.bulk + mbarrier), two planes in flight, running
 // ahead across group boundaries.
@@ -31,7 +34,6 @@
 
 namespace hydro {
 
-enum : int { LR_Z = 1, LR_FX = 2, LR_FY = 4, LR_INI = 8, LR_INJ = 16, LR_INT = 32, LR_RC = 64 };
 enum : int { LF_LOX = 0, LF_UPX, LF_LOY, LF_UPY, LF_FX, LF_FY };
 
 // variant seams: FAST = van Leer limiter on primitive variables, no floors (compile time)
@@ -75,28 +77,35 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   const size_t nS = (size_t)SS * S;
   const int off = g - GW;  // unused outer ghost layers
 
+  // shared memory: everything at compile-time offsets; the raw planes, whose size depends on g, come last
   extern __shared__ __align__(16) unsigned char smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
-  R* raw = reinterpret_cast<R*>(smem + 64);            // [2][5][SS]      landing zone of the bulk copies
-  R* ring = raw + (size_t)2 * 5 * SS;                  // [NW][5][WPL]    primitive planes
-  R* zs = ring + (size_t)NW * 5 * WPL;                 // [2][2][5][NT]   private traced z states (lo, up) of planes t, t+1
-  R* xy = zs + (size_t)2 * 2 * 5 * NT;                 // [6][5][NC]      LOX UPX LOY UPY FX FY
+  R* ring = reinterpret_cast<R*>(smem + 64);           // [NW] fields of WPL cells: primitive planes
+  R* zs = ring + NW * 5 * WPL;                         // [2][2] fields of NT cells: private traced z states (lo, up) of planes t, t+1
+  R* xy = zs + 4 * 5 * NT;                             // [6] fields of NC cells: LOX UPX LOY UPY FX FY
+  R* raw = xy + 6 * 5 * NC;                            // [2][5][SS] landing zone of the bulk copies (SoA as in HBM)
+  auto fld = [&](int k) { return xy + k * 5 * NC; };
 
   const int tid = threadIdx.x;
-  // ---- column and role of this thread (pass 0) and, for warp 9, of its corner column (pass 1)
+  // ---- column and role of this thread
   int ii, jj;
   if (tid < PS * FT) { jj = 1 + tid / FT; ii = tid - (jj - 1) * FT; }
   else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
-  const int col0 = jj * FT + ii;
-  const bool in_i = ii >= 1 && ii <= PS, in_j = jj >= 1 && jj <= PS;
-  const int role0 = LR_Z | LR_RC | (ii >= 1 ? LR_FX : 0) | (jj >= 1 ? LR_FY : 0) | (in_i ? LR_INI : 0) | (in_j ? LR_INJ : 0) |
-                    ((in_i && in_j) ? LR_INT : 0);
-  const int npass = (tid >= PS * FT) ? 2 : 1;  // warp-uniform
-  const int cl = tid - PS * FT;                // corner id for lanes 0..3 of warp 9
-  const int ci = (cl & 1) ? FT - 1 : 0, cj = (cl & 2) ? FT - 1 : 0;
-  const int col1 = cj * FT + ci;
-  const int role1 = (cl >= 0 && cl < 4) ? (LR_RC | (ci >= 1 ? LR_FX : 0) | (cj >= 1 ? LR_FY : 0)) : 0;
-  const int wb0 = (jj + GW - 1) * SWP + (ii + GW - 1);  // own index in a primitive plane
+  const int col = jj * FT + ii;
+  const bool in_i = ii >= 1 && ii <= PS, in_j = jj >= 1 && jj <= PS, interior = in_i && in_j;
+  const int wb = (jj + GW - 1) * SWP + (ii + GW - 1);  // own index in a primitive plane
+  // first-pass face jobs of phase D: own lower faces, plus the corner faces on lanes that have none
+  int fxc = (ii >= 1) ? col : -1, fyc = (jj >= 1) ? col : -1;
+  if (tid == 0) fxc = FT - 1;                         // F*_x(f = 16, j = -1)
+  if (tid == FT) fxc = FT * FT - 1;                   // F*_x(f = 16, j = 16)
+  if (tid == PS * FT) fyc = (FT - 1) * FT;            // F*_y(i = -1, f = 16)
+  if (tid == PS * FT + 1) fyc = FT * FT - 1;          // F*_y(i = 16, f = 16)
+  // corner-state job of phase F: lanes 0..7 of warp 9: corner (l & 3), direction (l >> 2)
+  const int cl = tid - PS * FT;
+  const bool cjob = cl >= 0 && cl < 8;
+  const int cdir = (cl >> 2) & 1;
+  const int cci = (cl & 1) ? FT - 1 : 0, ccj = (cl & 2) ? FT - 1 : 0;
+  const int ccol = ccj * FT + cci, cwb = (ccj + GW - 1) * SWP + (cci + GW - 1);
 
   // ---- plane pipeline: sequence number n = m * NPL + (plane + GW) over this CTA's groups m
   const int my_groups = (Ng - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
@@ -128,16 +137,37 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     const int st = nseq & 1;
     mbar_wait(bar + st, (uint32_t)((nseq >> 1) & 1));
     const R* rp = raw + (size_t)st * 5 * SS;
-    R* wp = ring + (size_t)slot * 5 * WPL;
+    R* wp = ring + slot * 5 * WPL;
     for (int idx = tid; idx < WPL; idx += NT) {
       const int b = idx / SWP, a = idx - b * SWP;
-      st5(wp + idx, WPL, Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c));
+      stv(wp, WPL, idx, Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c));
     }
   };
   // after the barrier that follows a conversion: refill the raw stage it consumed
   auto refill = [&]() {
     if (tid == 0) { fence_async_smem(); issue(nseq + 2); }
     ++nseq;
+  };
+  // traced states of a corner column of primitive plane `wpl` along x (cdir 0) or y (cdir 1)
+  auto corner_states = [&](const R* wpl) {
+    const int st = cdir ? SWP : 1;
+    V5<R> W[2 * RW + 1];
+#pragma unroll
+    for (int s = 0; s < 2 * RW + 1; ++s) {
+      const V5<R> w = ldv(wpl, WPL, cwb + (s - RW) * st);
+      W[s][0] = w[0]; W[s][4] = w[4];
+      W[s][1] = cdir ? w[2] : w[1];
+      W[s][2] = cdir ? w[3] : w[2];
+      W[s][3] = cdir ? w[1] : w[3];
+    }
+    V5<R> l, u, lo, up;
+    Op::recon(W[0], W[RW - 1], W[RW], W[RW + 1], W[2 * RW], p, l, u);
+    lo[0] = l[0]; lo[4] = l[4]; up[0] = u[0]; up[4] = u[4];
+    lo[1] = cdir ? l[3] : l[1]; up[1] = cdir ? u[3] : u[1];
+    lo[2] = cdir ? l[1] : l[2]; up[2] = cdir ? u[1] : u[2];
+    lo[3] = cdir ? l[2] : l[3]; up[3] = cdir ? u[2] : u[3];
+    stv(fld(LF_LOX + 2 * cdir), NC, ccol, lo);
+    stv(fld(LF_UPX + 2 * cdir), NC, ccol, up);
   };
 
   V5<R> f1z, uzc, Dz;  // F*_z at the lower face of plane t+1; corrected up_z of plane t-1; (dF_x + dF_y) - F_z of plane t-1
@@ -152,90 +182,78 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
       __syncthreads();
       refill();
     }
+    int sl = 0;  // ring slot of plane t+1-RW (the oldest plane held)
 
 #pragma unroll 1
     for (int t = -2; t <= PS; ++t) {
       const bool doxy = t >= -1;
       const bool tin = t >= 0 && t < PS;
+      // ring slots of the planes this step touches
+      int slot[NW];
+#pragma unroll
+      for (int s = 0; s < NW; ++s) slot[s] = (sl + s < NW) ? sl + s : sl + s - NW;
       // ================= B: z states of plane t+1, F*_z(t+1) =================
       V5<R> dFz;
 #pragma unroll
       for (int q = 0; q < 5; ++q) dFz[q] = R(0);
       if (t < PS) {
-        const int kz = t + 1;
-        V5<R> Wz[2 * RW + 1];
+        V5<R> Wz[NW];
 #pragma unroll
-        for (int s = 0; s < 2 * RW + 1; ++s)
-          Wz[s] = to_normal<2>(ld5(ring + (size_t)((kz - RW + s + GW) % NW) * 5 * WPL + wb0, WPL));
+        for (int s = 0; s < NW; ++s) Wz[s] = to_normal<2>(ldv(ring + slot[s] * 5 * WPL, WPL, wb));
         V5<R> l, u;
         Op::recon(Wz[0], Wz[RW - 1], Wz[RW], Wz[RW + 1], Wz[2 * RW], p, l, u);
         const V5<R> lz = from_normal<2>(l), uz = from_normal<2>(u);
-        R* zn = zs + (size_t)(kz & 1) * 10 * NT + tid;
-        st5(zn, NT, lz);
-        st5(zn + 5 * NT, NT, uz);
-        if (kz >= 0) {
-          const V5<R> uzp = ld5(zs + (size_t)(t & 1) * 10 * NT + 5 * NT + tid, NT);
+        R* zn = zs + ((t + 1) & 1) * 10 * NT;
+        stv(zn, NT, tid, lz);
+        stv(zn + 5 * NT, NT, tid, uz);
+        if (t >= -1) {
+          const V5<R> uzp = ldv(zs + (t & 1) * 10 * NT + 5 * NT, NT, tid);
           const V5<R> f = Op::template riemann<2>(uzp, lz, p, c);
 #pragma unroll
           for (int q = 0; q < 5; ++q) { dFz[q] = f[q] - f1z[q]; f1z[q] = f[q]; }
         }
       }
-      // ================= C: x,y traced states of plane t =================
+      // ================= C: x,y traced states of plane t (slot RW-1 of the held planes) =================
       if (doxy) {
-        const R* wpl = ring + (size_t)((t + GW) % NW) * 5 * WPL;
-        for (int ps = 0; ps < npass; ++ps) {
-          const int col = ps ? col1 : col0, role = ps ? role1 : role0;
-          if (role & LR_RC) {
-            const int cjj = col / FT, cii = col - cjj * FT;
-            const R* wt = wpl + (cjj + GW - 1) * SWP + (cii + GW - 1);
-            const V5<R> W0 = ld5(wt, WPL);
-            R* H = xy + col;
-            {
-              const V5<R> Wb = ld5(wt - 1, WPL), Wc = ld5(wt + 1, WPL);
-              V5<R> Wa = Wb, Wd = Wc;
-              if (RECON == RECON_PPM) { Wa = ld5(wt - 2, WPL); Wd = ld5(wt + 2, WPL); }
-              V5<R> l, u;
-              Op::recon(to_normal<0>(Wa), to_normal<0>(Wb), to_normal<0>(W0), to_normal<0>(Wc), to_normal<0>(Wd), p, l, u);
-              st5(H + LF_LOX * 5 * NC, NC, from_normal<0>(l));
-              st5(H + LF_UPX * 5 * NC, NC, from_normal<0>(u));
-            }
-            {
-              const V5<R> Wb = ld5(wt - SWP, WPL), Wc = ld5(wt + SWP, WPL);
-              V5<R> Wa = Wb, Wd = Wc;
-              if (RECON == RECON_PPM) { Wa = ld5(wt - 2 * SWP, WPL); Wd = ld5(wt + 2 * SWP, WPL); }
-              V5<R> l, u;
-              Op::recon(to_normal<1>(Wa), to_normal<1>(Wb), to_normal<1>(W0), to_normal<1>(Wc), to_normal<1>(Wd), p, l, u);
-              st5(H + LF_LOY * 5 * NC, NC, from_normal<1>(l));
-              st5(H + LF_UPY * 5 * NC, NC, from_normal<1>(u));
-            }
-          }
+        const R* wpl = ring + slot[RW - 1] * 5 * WPL;
+        const V5<R> W0 = ldv(wpl, WPL, wb);
+        {
+          const V5<R> Wb = ldv(wpl, WPL, wb - 1), Wc = ldv(wpl, WPL, wb + 1);
+          V5<R> Wa = Wb, Wd = Wc;
+          if (RECON == RECON_PPM) { Wa = ldv(wpl, WPL, wb - 2); Wd = ldv(wpl, WPL, wb + 2); }
+          V5<R> l, u;
+          Op::recon(to_normal<0>(Wa), to_normal<0>(Wb), to_normal<0>(W0), to_normal<0>(Wc), to_normal<0>(Wd), p, l, u);
+          stv(fld(LF_LOX), NC, col, from_normal<0>(l));
+          stv(fld(LF_UPX), NC, col, from_normal<0>(u));
+        }
+        {
+          const V5<R> Wb = ldv(wpl, WPL, wb - SWP), Wc = ldv(wpl, WPL, wb + SWP);
+          V5<R> Wa = Wb, Wd = Wc;
+          if (RECON == RECON_PPM) { Wa = ldv(wpl, WPL, wb - 2 * SWP); Wd = ldv(wpl, WPL, wb + 2 * SWP); }
+          V5<R> l, u;
+          Op::recon(to_normal<1>(Wa), to_normal<1>(Wb), to_normal<1>(W0), to_normal<1>(Wc), to_normal<1>(Wd), p, l, u);
+          stv(fld(LF_LOY), NC, col, from_normal<1>(l));
+          stv(fld(LF_UPY), NC, col, from_normal<1>(u));
         }
       }
       __syncthreads();  // barrier 1
 
       // ================= D: F*_x(t), F*_y(t); con->prim of the next plane =================
       if (doxy) {
-        for (int ps = 0; ps < npass; ++ps) {
-          const int col = ps ? col1 : col0, role = ps ? role1 : role0;
-          R* H = xy + col;
-          if (role & LR_FX)
-            st5(H + LF_FX * 5 * NC, NC,
-                Op::template riemann<0>(ld5(H + LF_UPX * 5 * NC - 1, NC), ld5(H + LF_LOX * 5 * NC, NC), p, c));
-          if (role & LR_FY)
-            st5(H + LF_FY * 5 * NC, NC,
-                Op::template riemann<1>(ld5(H + LF_UPY * 5 * NC - FT, NC), ld5(H + LF_LOY * 5 * NC, NC), p, c));
-        }
+        if (fxc >= 0)
+          stv(fld(LF_FX), NC, fxc, Op::template riemann<0>(ldv(fld(LF_UPX), NC, fxc - 1), ldv(fld(LF_LOX), NC, fxc), p, c));
+        if (fyc >= 0)
+          stv(fld(LF_FY), NC, fyc, Op::template riemann<1>(ldv(fld(LF_UPY), NC, fyc - FT), ldv(fld(LF_LOY), NC, fyc), p, c));
       }
-      const bool conv = t + 2 + RW <= PS - 1 + GW;  // plane t+2+RW replaces plane t+1-RW (read for the last time in B)
-      if (conv) convert((t + 2 + RW + GW) % NW);
+      const bool conv = t + 2 + RW <= PS - 1 + GW;  // plane t+2+RW replaces plane t+1-RW (read for the last time in B / C)
+      if (conv) convert(sl);
       __syncthreads();  // barrier 2
       if (conv) refill();
 
       // ================= E: transverse correction, F_z(t), update of plane t-1 =========
       if (doxy) {
-        R* H = xy + col0;
         V5<R> Uold;
-        const bool upd = (role0 & LR_INT) && t >= 1;
+        const bool upd = interior && t >= 1;
         if (upd) {
           const R* gin = in + grp * 5 * nS + ((size_t)(t - 1 + g) * S + (jj - 1 + g)) * S + (ii - 1 + g);
 #pragma unroll
@@ -244,37 +262,37 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
         V5<R> dFx, dFy;
 #pragma unroll
         for (int q = 0; q < 5; ++q) { dFx[q] = R(0); dFy[q] = R(0); }
-        if (role0 & LR_INI) {
-          const V5<R> a = ld5(H + LF_FX * 5 * NC + 1, NC), b = ld5(H + LF_FX * 5 * NC, NC);
+        if (in_i) {
+          const V5<R> a = ldv(fld(LF_FX), NC, col + 1), b = ldv(fld(LF_FX), NC, col);
 #pragma unroll
           for (int q = 0; q < 5; ++q) dFx[q] = a[q] - b[q];
         }
-        if (role0 & LR_INJ) {
-          const V5<R> a = ld5(H + LF_FY * 5 * NC + FT, NC), b = ld5(H + LF_FY * 5 * NC, NC);
+        if (in_j) {
+          const V5<R> a = ldv(fld(LF_FY), NC, col + FT), b = ldv(fld(LF_FY), NC, col);
 #pragma unroll
           for (int q = 0; q < 5; ++q) dFy[q] = a[q] - b[q];
         }
-        if (tin && (role0 & LR_INJ)) {  // x states: t1 = y, t2 = z
+        if (tin && in_j) {  // x states: t1 = y, t2 = z
           V5<R> dq;
 #pragma unroll
           for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFy[q] + dFz[q]);
-          st5(H + LF_LOX * 5 * NC, NC, Op::correct(ld5(H + LF_LOX * 5 * NC, NC), dq, p, c));
-          st5(H + LF_UPX * 5 * NC, NC, Op::correct(ld5(H + LF_UPX * 5 * NC, NC), dq, p, c));
+          stv(fld(LF_LOX), NC, col, Op::correct(ldv(fld(LF_LOX), NC, col), dq, p, c));
+          stv(fld(LF_UPX), NC, col, Op::correct(ldv(fld(LF_UPX), NC, col), dq, p, c));
         }
-        if (tin && (role0 & LR_INI)) {  // y states: t1 = z, t2 = x
+        if (tin && in_i) {  // y states: t1 = z, t2 = x
           V5<R> dq;
 #pragma unroll
           for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFz[q] + dFx[q]);
-          st5(H + LF_LOY * 5 * NC, NC, Op::correct(ld5(H + LF_LOY * 5 * NC, NC), dq, p, c));
-          st5(H + LF_UPY * 5 * NC, NC, Op::correct(ld5(H + LF_UPY * 5 * NC, NC), dq, p, c));
+          stv(fld(LF_LOY), NC, col, Op::correct(ldv(fld(LF_LOY), NC, col), dq, p, c));
+          stv(fld(LF_UPY), NC, col, Op::correct(ldv(fld(LF_UPY), NC, col), dq, p, c));
         }
-        if (role0 & LR_INT) {  // z states: t1 = x, t2 = y; every plane t in [-1,16]
+        if (interior) {  // z states: t1 = x, t2 = y; every plane t in [-1,16]
           V5<R> dq;
 #pragma unroll
           for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFx[q] + dFy[q]);
-          const R* zc = zs + (size_t)(t & 1) * 10 * NT + tid;
+          const R* zc = zs + (t & 1) * 10 * NT;
           if (t >= 0) {
-            const V5<R> lzc = Op::correct(ld5(zc, NT), dq, p, c);
+            const V5<R> lzc = Op::correct(ldv(zc, NT, tid), dq, p, c);
             const V5<R> Fz = Op::template riemann<2>(uzc, lzc, p, c);
             if (face_flux && (t & 7) == 0)  // stored right after the solve
               st5(face_flux + grp * 9 * 5 * PS * PS + (size_t)((6 + (t >> 3)) * 5) * 256 + (jj - 1) * PS + (ii - 1), 256, Fz);
@@ -288,38 +306,37 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
             }
             Dz = Fz;
           }
-          if (t < PS) uzc = Op::correct(ld5(zc + 5 * NT, NT), dq, p, c);
+          if (t < PS) uzc = Op::correct(ldv(zc + 5 * NT, NT, tid), dq, p, c);
         }
       }
       __syncthreads();  // barrier 3
 
       // ================= F: final fluxes of plane t + boundary-flux store ============
       if (tin) {
-        R* H = xy + col0;
         R* gff = face_flux ? face_flux + grp * 9 * 5 * PS * PS : nullptr;
-        if ((role0 & (LR_INJ | LR_FX)) == (LR_INJ | LR_FX)) {
-          const V5<R> f = Op::template riemann<0>(ld5(H + LF_UPX * 5 * NC - 1, NC), ld5(H + LF_LOX * 5 * NC, NC), p, c);
-          st5(H + LF_FX * 5 * NC, NC, f);
+        if (in_j && ii >= 1) {
+          const V5<R> f = Op::template riemann<0>(ldv(fld(LF_UPX), NC, col - 1), ldv(fld(LF_LOX), NC, col), p, c);
+          stv(fld(LF_FX), NC, col, f);
           if (gff && ((ii - 1) & 7) == 0) st5(gff + (size_t)(((ii - 1) >> 3) * 5) * 256 + t * PS + (jj - 1), 256, f);
         }
-        if ((role0 & (LR_INI | LR_FY)) == (LR_INI | LR_FY)) {
-          const V5<R> f = Op::template riemann<1>(ld5(H + LF_UPY * 5 * NC - FT, NC), ld5(H + LF_LOY * 5 * NC, NC), p, c);
-          st5(H + LF_FY * 5 * NC, NC, f);
+        if (in_i && jj >= 1) {
+          const V5<R> f = Op::template riemann<1>(ldv(fld(LF_UPY), NC, col - FT), ldv(fld(LF_LOY), NC, col), p, c);
+          stv(fld(LF_FY), NC, col, f);
           if (gff && ((jj - 1) & 7) == 0) st5(gff + (size_t)((3 + ((jj - 1) >> 3)) * 5) * 256 + t * PS + (ii - 1), 256, f);
         }
       }
+      // corner columns of plane t+1 (held in ring slot RW); their entries of LOX..UPY were last read in D
+      if (cjob && t < PS) corner_states(ring + slot[RW] * 5 * WPL);
       __syncthreads();  // barrier 4
 
       // ================= G: carried x+y flux difference of plane t minus F_z(t) =================
-      if (tin && (role0 & LR_INT)) {
-        const R* H = xy + col0;
+      if (tin && interior) {
+        const V5<R> x1 = ldv(fld(LF_FX), NC, col + 1), x0 = ldv(fld(LF_FX), NC, col);
+        const V5<R> y1 = ldv(fld(LF_FY), NC, col + FT), y0 = ldv(fld(LF_FY), NC, col);
 #pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          const R* fx = H + (LF_FX * 5 + q) * NC;
-          const R* fy = H + (LF_FY * 5 + q) * NC;
-          Dz[q] = ((fx[1] - fx[0]) + (fy[FT] - fy[0])) - Dz[q];
-        }
+        for (int q = 0; q < 5; ++q) Dz[q] = ((x1[q] - x0[q]) + (y1[q] - y0[q])) - Dz[q];
       }
+      sl = (sl + 1 < NW) ? sl + 1 : 0;
     }
   }
   flush_counters(c, status);

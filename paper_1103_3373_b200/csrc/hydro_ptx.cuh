@@ -52,4 +52,30 @@ template <class R> __device__ __forceinline__ void st5(R* p, int stride, const V
   for (int q = 0; q < 5; ++q) p[q * stride] = x[q];
 }
 
+
+// Packed 5-vector fields in shared memory ("4+1" layout): a field of N cells is [N] 16-byte vectors holding
+// components 0..3 followed by [N] scalars holding component 4 (float), or [N] (q0,q1) | [N] (q2,q3) | [N] q4
+// (double), so that a state moves with 2 (3) shared-memory instructions instead of 5.  N even, base 16-byte aligned.
+__device__ __forceinline__ V5<float> ldv(const float* f, int N, int i) {
+  const float4 a = reinterpret_cast<const float4*>(f)[i];
+  V5<float> x;
+  x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = f[4 * N + i];
+  return x;
+}
+__device__ __forceinline__ void stv(float* f, int N, int i, const V5<float>& x) {
+  reinterpret_cast<float4*>(f)[i] = make_float4(x[0], x[1], x[2], x[3]);
+  f[4 * N + i] = x[4];
+}
+__device__ __forceinline__ V5<double> ldv(const double* f, int N, int i) {
+  const double2 a = reinterpret_cast<const double2*>(f)[i], b = reinterpret_cast<const double2*>(f + 2 * N)[i];
+  V5<double> x;
+  x[0] = a.x; x[1] = a.y; x[2] = b.x; x[3] = b.y; x[4] = f[4 * N + i];
+  return x;
+}
+__device__ __forceinline__ void stv(double* f, int N, int i, const V5<double>& x) {
+  reinterpret_cast<double2*>(f)[i] = make_double2(x[0], x[1]);
+  reinterpret_cast<double2*>(f + 2 * N)[i] = make_double2(x[2], x[3]);
+  f[4 * N + i] = x[4];
+}
+
 }  // namespace hydro
