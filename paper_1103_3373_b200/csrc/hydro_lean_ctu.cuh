@@ -176,6 +176,9 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
 
   for (int m = 0; m < my_groups; ++m) {
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
+    // own cell of plane 0 in `in` / `out` (interior columns only)
+    const R* gin0 = in + grp * 5 * nS + ((size_t)g * S + (jj - 1 + g)) * S + (ii - 1 + g);
+    R* gout0 = out + grp * 5 * PS * PS * PS + (jj - 1) * PS + (ii - 1);
     // ---- prologue: the first NW primitive planes (-GW .. -GW+NW-1)
     for (int k = 0; k < NW; ++k) {
       convert(k);
@@ -255,9 +258,9 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
         V5<R> Uold;
         const bool upd = interior && t >= 1;
         if (upd) {
-          const R* gin = in + grp * 5 * nS + ((size_t)(t - 1 + g) * S + (jj - 1 + g)) * S + (ii - 1 + g);
+          const R* gin = gin0 + (t - 1) * SS;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) Uold[q] = __ldg(gin + q * nS);
+          for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += nS; }
         }
         V5<R> dFx, dFy;
 #pragma unroll
@@ -302,7 +305,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
               for (int q = 0; q < 5; ++q) U[q] = Uold[q] - p.nu * (Dz[q] + Fz[q]);
               const V5<R> Wn = Op::c2p(U, p, c);
               if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
-              st5(out + grp * 5 * PS * PS * PS + ((t - 1) * PS + (jj - 1)) * PS + (ii - 1), PS * PS * PS, U);
+              st5(gout0 + (t - 1) * PS * PS, PS * PS * PS, U);
             }
             Dz = Fz;
           }

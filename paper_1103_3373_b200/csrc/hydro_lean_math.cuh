@@ -151,8 +151,10 @@ template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, co
     const R tA = m_fma(A4 + A4, A0, -mA), tB = m_fma(B4 + B4, B0, -mB);
     if (!(A0 > R(0) && B0 > R(0) && tA > R(0) && tB > R(0))) {  // NaN fails the test
       c.roe_fb++;
-      V5<R> F, l = WL, r = WR;  // copies: only this branch spills its arguments to the stack
-      roe_fallback_flux(&l, &r, &p, &c.exact, &F);
+      V5<R> F, l = WL, r = WR;  // copies: only this branch puts its arguments on the stack
+      int ex = 0;
+      roe_fallback_flux(&l, &r, &p, &ex, &F);
+      c.exact += ex;
       return F;
     }
   }
