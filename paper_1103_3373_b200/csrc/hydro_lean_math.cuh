@@ -24,7 +24,7 @@ __device__ __forceinline__ float m_rsqrt(float x) { return 1.0f / sqrtf(x); }
 #else
 __device__ __forceinline__ float m_rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 #endif
-__device__ __forceinline__ double m_rsqrt(double x) { return 1.0 / sqrt(x); }
+__device__ __forceinline__ double m_rsqrt(double x) { return rsqrt(x); }  // <= 1 ulp, no division
 __device__ __forceinline__ float m_fma(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ double m_fma(double a, double b, double c) { return fma(a, b, c); }
 
@@ -98,10 +98,18 @@ __device__ __forceinline__ void lean_plm_trace(const V5<R>& Wm, const V5<R>& W0,
 }
 
 // ---- c4: Roe's solver, primitive-jump form (normal frame in, normal-frame flux out) ------------
-template <class R> struct LeanState { R ir, H, m, F1, F2, F3, F4; };
+// per-state quantities of a Riemann problem
+template <class R> struct LeanState { R ir, sq, H, m, F1, F2, F3, F4; };
 template <class R> __device__ __forceinline__ LeanState<R> lean_state(const V5<R>& W, R g1) {
   LeanState<R> s;
-  s.ir = m_rcp(W[0]);
+  if (sizeof(R) == 4) {  // fp32: two SFU instructions are cheaper than the extra multiplies
+    s.ir = m_rcp(W[0]);
+    s.sq = m_sqrt(W[0]);
+  } else {               // fp64: one rsqrt instead of a division and a square root
+    const R is = m_rsqrt(W[0]);
+    s.ir = is * is;
+    s.sq = W[0] * is;
+  }
   const R q2 = m_fma(W[3], W[3], m_fma(W[2], W[2], W[1] * W[1]));
   s.H = m_fma(R(0.5), q2, (g1 * W[4]) * s.ir);
   s.m = W[0] * W[1];
@@ -121,19 +129,22 @@ template <class R> __device__ __noinline__ void roe_fallback_flux(const V5<R>* W
   *cnt_exact += c.exact;
 }
 
-template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
+// branch-free core: the Roe flux and whether both intermediate states passed the failure test.  Keeping the
+// (rare) fallback out of it lets two independent solves share one basic block and interleave.
+template <class R> __device__ __forceinline__ bool lean_roe_core(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, V5<R>& F) {
   const R g1 = p.gamma * p.igm1;
   const LeanState<R> L = lean_state(WL, g1), Rr = lean_state(WR, g1);
   // Roe averages with weights wL = sqrt(rhoL)/(sqrt(rhoL)+sqrt(rhoR)), wR = 1 - wL; rho~ = sqrt(rhoL rhoR)
-  const R r = m_sqrt(WR[0] * L.ir);
-  const R wR = r * m_rcp(R(1) + r);
-  const R rt = WL[0] * r;
+  const R wR = Rr.sq * m_rcp(L.sq + Rr.sq);
+  const R rt = L.sq * Rr.sq;
   const R du = WR[1] - WL[1], dv = WR[2] - WL[2], dw = WR[3] - WL[3];
   const R ut = m_fma(wR, du, WL[1]), vt = m_fma(wR, dv, WL[2]), wt = m_fma(wR, dw, WL[3]);
   const R Ht = m_fma(wR, Rr.H - L.H, L.H);
   const R hq = R(0.5) * m_fma(wt, wt, m_fma(vt, vt, ut * ut));
   const R a2 = p.gm1 * (Ht - hq);
-  const R a = m_sqrt(a2), ia2 = m_rcp(a2);
+  R a, ia2;
+  if (sizeof(R) == 4) { a = m_sqrt(a2); ia2 = m_rcp(a2); }
+  else { const R ia = m_rsqrt(a2); a = a2 * ia; ia2 = ia * ia; }
   // wave strengths from the primitive jumps
   const R dp = WR[4] - WL[4], dr = WR[0] - WL[0];
   const R y = (rt * a) * du, h = R(0.5) * ia2;
@@ -141,23 +152,14 @@ template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, co
   const R al3 = rt * dv, al4 = rt * dw;
   const R um = ut - a, up = ut + a, ua = ut * a, H1 = Ht - ua, H5 = Ht + ua;
   // failure test on U_L + al1 K1 and U_R - al5 K5 (rho > 0 and P > 0, the latter without a division)
-  {
-    const R A0 = WL[0] + al1, B0 = WR[0] - al5;
-    const R A1 = m_fma(al1, um, L.m), B1 = m_fma(-al5, up, Rr.m);
-    const R A2 = m_fma(al1, vt, WL[0] * WL[2]), B2 = m_fma(-al5, vt, WR[0] * WR[2]);
-    const R A3 = m_fma(al1, wt, WL[0] * WL[3]), B3 = m_fma(-al5, wt, WR[0] * WR[3]);
-    const R A4 = m_fma(al1, H1, m_fma(WL[0], L.H, -WL[4])), B4 = m_fma(-al5, H5, m_fma(WR[0], Rr.H, -WR[4]));
-    const R mA = m_fma(A3, A3, m_fma(A2, A2, A1 * A1)), mB = m_fma(B3, B3, m_fma(B2, B2, B1 * B1));
-    const R tA = m_fma(A4 + A4, A0, -mA), tB = m_fma(B4 + B4, B0, -mB);
-    if (!(A0 > R(0) && B0 > R(0) && tA > R(0) && tB > R(0))) {  // NaN fails the test
-      c.roe_fb++;
-      V5<R> F, l = WL, r = WR;  // copies: only this branch puts its arguments on the stack
-      int ex = 0;
-      roe_fallback_flux(&l, &r, &p, &ex, &F);
-      c.exact += ex;
-      return F;
-    }
-  }
+  const R A0 = WL[0] + al1, B0 = WR[0] - al5;
+  const R A1 = m_fma(al1, um, L.m), B1 = m_fma(-al5, up, Rr.m);
+  const R A2 = m_fma(al1, vt, WL[0] * WL[2]), B2 = m_fma(-al5, vt, WR[0] * WR[2]);
+  const R A3 = m_fma(al1, wt, WL[0] * WL[3]), B3 = m_fma(-al5, wt, WR[0] * WR[3]);
+  const R A4 = m_fma(al1, H1, m_fma(WL[0], L.H, -WL[4])), B4 = m_fma(-al5, H5, m_fma(WR[0], Rr.H, -WR[4]));
+  const R mA = m_fma(A3, A3, m_fma(A2, A2, A1 * A1)), mB = m_fma(B3, B3, m_fma(B2, B2, B1 * B1));
+  const R tA = m_fma(A4 + A4, A0, -mA), tB = m_fma(B4 + B4, B0, -mB);
+  const bool ok = A0 > R(0) && B0 > R(0) && tA > R(0) && tB > R(0);  // NaN fails the test
   const R w1 = al1 * m_abs(um), w2 = al2 * m_abs(ut), w5 = al5 * m_abs(up);
   const R w3 = al3 * m_abs(ut), w4 = al4 * m_abs(ut);
   const R d0 = (w1 + w2) + w5;
@@ -165,12 +167,24 @@ template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, co
   const R d2 = m_fma(d0, vt, w3);
   const R d3 = m_fma(d0, wt, w4);
   const R d4 = m_fma(w5, H5, m_fma(w4, wt, m_fma(w3, vt, m_fma(w2, hq, w1 * H1))));
-  V5<R> F;
   F[0] = R(0.5) * ((L.m + Rr.m) - d0);
   F[1] = R(0.5) * ((L.F1 + Rr.F1) - d1);
   F[2] = R(0.5) * ((L.F2 + Rr.F2) - d2);
   F[3] = R(0.5) * ((L.F3 + Rr.F3) - d3);
   F[4] = R(0.5) * ((L.F4 + Rr.F4) - d4);
+  return ok;
+}
+// Roe failed at this face: count it and replace the flux by the fallback solver's
+template <class R> __device__ __forceinline__ void lean_roe_failed(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c, V5<R>& F) {
+  c.roe_fb++;
+  V5<R> l = WL, r = WR;  // copies: only this branch puts its arguments on the stack
+  int ex = 0;
+  roe_fallback_flux(&l, &r, &p, &ex, &F);
+  c.exact += ex;
+}
+template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
+  V5<R> F;
+  if (!lean_roe_core(WL, WR, p, F)) lean_roe_failed(WL, WR, p, c, F);
   return F;
 }
 
