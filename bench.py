@@ -182,7 +182,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--dtype", default="f32", choices=("f32", "f64"))
     ap.add_argument("--ng", type=int, default=NG, help="patch groups per GPU (default: the config's 8192)")
-    ap.add_argument("--kernel", default="auto", choices=("auto", "staged", "fused", "ws", "lean"))
+    ap.add_argument("--kernel", default="auto", choices=("auto", "staged", "fused"))
     ap.add_argument("--no-extras", action="store_true", help="skip the e2e / cpu_baseline / f64 legs (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -204,7 +204,7 @@ def main():
     B.lib()
     warmup = max(3, args.warmup)
     steps = max(1, args.steps)
-    impl = {"auto": B.IMPL_AUTO, "staged": B.IMPL_STAGED, "fused": B.IMPL_FUSED, "ws": B.IMPL_WS, "lean": B.IMPL_LEAN}[args.kernel]
+    impl = {"auto": B.IMPL_AUTO, "staged": B.IMPL_STAGED, "fused": B.IMPL_FUSED}[args.kernel]
     Ng = args.ng
 
     def barrier():
@@ -280,12 +280,8 @@ def main():
     hbm = float(peaks.get("hbm_gbs") or 6650.0)
     hbm_src = "measured (MEASURED_PEAKS.json)" if peaks.get("hbm_gbs") else "fallback (B200_PROFILING.md)"
     traffic = ncu_traffic(f"solve_{args.dtype}_{args.kernel}")
-    if impl in (B.IMPL_AUTO, B.IMPL_LEAN) and B.hydro_lean_fits(main_dtype, SCHEME, B.PLM, GHOST):
-        kernel_name = "hydro_solve (ctu_lean_kernel: lean fused, two CTAs per SM)"
-    elif impl in (B.IMPL_AUTO, B.IMPL_WS) and B.hydro_ws_fits(main_dtype, SCHEME, B.PLM, GHOST):
-        kernel_name = "hydro_solve (ctu_ws_kernel: warp-specialised fused)"
-    elif impl != B.IMPL_STAGED and B.hydro_fused_fits(main_dtype, SCHEME, B.PLM, GHOST):
-        kernel_name = "hydro_solve (ctu_fused_kernel)"
+    if impl != B.IMPL_STAGED and B.hydro_fused_fits(main_dtype, SCHEME, B.PLM, GHOST):
+        kernel_name = "hydro_solve (ctu_lean_kernel: fused z-marching CTU, phase-crossing state in shared memory)"
     else:
         kernel_name = "hydro_solve (staged_kernel)"
     roofline = {

@@ -57,11 +57,10 @@ enum { HYDRO_MHM = 0, HYDRO_VL = 1, HYDRO_CTU = 2 };                       /* sc
 enum { HYDRO_EXACT = 0, HYDRO_HLLE = 1, HYDRO_HLLC = 2, HYDRO_ROE = 3 };   /* riemann */
 enum { HYDRO_GMINMOD = 0, HYDRO_VANLEER = 1, HYDRO_VANALBADA = 2, HYDRO_HYBRID = 3 }; /* limiter PAPER.md:48 */
 enum { HYDRO_PLM = 0, HYDRO_PPM = 1 };                                     /* recon */
-/* kernel organisation (all compute the same update): staged = one phase per stage with global scratch (any
- * variant, any ghost width); fused = z-marching, single-role CTAs; ws = z-marching, warp-specialised
- * predictor / corrector groups; lean = z-marching, phase-crossing state in shared memory, two CTAs per SM.
- * AUTO picks lean, else ws, else fused, else staged, by availability and shared-memory fit. */
-enum { HYDRO_IMPL_AUTO = 0, HYDRO_IMPL_STAGED = 1, HYDRO_IMPL_FUSED = 2, HYDRO_IMPL_WS = 3, HYDRO_IMPL_LEAN = 4 };
+/* kernel organisation (both compute the same update): staged = one phase per stage with global scratch (any
+ * variant, any ghost width); fused = z-marching, every intermediate on chip, phase-crossing state in shared
+ * memory (CTU; two CTAs per SM where the tiles allow).  AUTO picks fused when it exists and its tiles fit. */
+enum { HYDRO_IMPL_AUTO = 0, HYDRO_IMPL_STAGED = 1, HYDRO_IMPL_FUSED = 2 };
 
 enum {
   HYDRO_OK = 0,
@@ -72,7 +71,7 @@ enum {
   HYDRO_E_GHOST = -5,     /* nghost < hydro_min_ghost(scheme, recon), or > 8 */
   HYDRO_E_WORKSPACE = -6, /* staged path selected and workspace missing / smaller than one slot */
   HYDRO_E_VALUE = -7,     /* gamma <= 1, dh <= 0, dt < 0, minmod_coeff outside [1,2], negative floor, cfl <= 0 */
-  HYDRO_E_NOFUSED = -8    /* impl == HYDRO_IMPL_FUSED / _WS / _LEAN and no such kernel exists (or fits) for this variant */
+  HYDRO_E_NOFUSED = -8    /* impl == HYDRO_IMPL_FUSED and no such kernel exists (or fits) for this variant */
 };
 
 typedef struct hydro_opts {      /* NULL => all defaults */
@@ -133,10 +132,6 @@ HYDRO_API int hydro_min_ghost(int scheme, int recon);                 /* 2/3 (MH
 HYDRO_API int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann); /* 1 if a fused kernel exists */
 /* 1 if that fused kernel's tiles fit in shared memory for ghost width nghost (else AUTO uses the staged path) */
 HYDRO_API int hydro_fused_fits(int precision_bytes, int scheme, int recon, int nghost);
-/* 1 if a warp-specialised fused kernel exists for (precision, scheme, recon) and fits for ghost width nghost */
-HYDRO_API int hydro_ws_fits(int precision_bytes, int scheme, int recon, int nghost);
-/* 1 if a lean fused kernel exists for (precision, scheme, recon) and fits for ghost width nghost */
-HYDRO_API int hydro_lean_fits(int precision_bytes, int scheme, int recon, int nghost);
 /* bytes of opts->workspace that hydro_solve_* may need in HYDRO_IMPL_AUTO mode for any ghost width
  * (0 only when the fused kernel runs for every nghost <= 8) */
 HYDRO_API size_t hydro_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon);

@@ -16,12 +16,12 @@ MHM, VL, CTU = 0, 1, 2
 EXACT, HLLE, HLLC, ROE = 0, 1, 2, 3
 GMINMOD, VANLEER, VANALBADA, HYBRID = 0, 1, 2, 3
 PLM, PPM = 0, 1
-IMPL_AUTO, IMPL_STAGED, IMPL_FUSED, IMPL_WS, IMPL_LEAN = 0, 1, 2, 3, 4
+IMPL_AUTO, IMPL_STAGED, IMPL_FUSED = 0, 1, 2
 PS = 16
 
 EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64", "hydro_pipeline_create",
            "hydro_pipeline_destroy", "hydro_pipeline_solve_f32", "hydro_pipeline_solve_f64", "hydro_min_ghost",
-           "hydro_has_fused", "hydro_fused_fits", "hydro_ws_fits", "hydro_lean_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror")
+           "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror")
 
 
 class HydroOpts(C.Structure):
@@ -60,8 +60,6 @@ def lib():
         L.hydro_min_ghost.argtypes = [i, i]
         L.hydro_has_fused.argtypes = [i, i, i, i]
         L.hydro_fused_fits.argtypes = [i, i, i, i]
-        L.hydro_ws_fits.argtypes = [i, i, i, i]
-        L.hydro_lean_fits.argtypes = [i, i, i, i]
         L.hydro_workspace_bytes.argtypes = [i, i, i, i]
         L.hydro_workspace_bytes.restype = sz
         L.hydro_staged_workspace_bytes.argtypes = [i, i, i, i]
@@ -88,20 +86,10 @@ def hydro_fused_fits(dtype, scheme, recon=PLM, nghost=0):
     return bool(lib().hydro_fused_fits(torch.empty((), dtype=dtype).element_size(), scheme, recon, nghost))
 
 
-def hydro_ws_fits(dtype, scheme, recon=PLM, nghost=0):
-    return bool(lib().hydro_ws_fits(torch.empty((), dtype=dtype).element_size(), scheme, recon, nghost))
-
-
-def hydro_lean_fits(dtype, scheme, recon=PLM, nghost=0):
-    return bool(lib().hydro_lean_fits(torch.empty((), dtype=dtype).element_size(), scheme, recon, nghost))
-
-
 def hydro_workspace_bytes(Ng, dtype, scheme, recon=PLM, impl=IMPL_AUTO, nghost=0):
     """Scratch bytes hydro_solve needs: 0 when the fused kernel runs for this ghost width."""
     es = torch.empty((), dtype=dtype).element_size()
-    if impl == IMPL_STAGED or (impl == IMPL_AUTO and not lib().hydro_fused_fits(es, scheme, recon, nghost)
-                               and not lib().hydro_ws_fits(es, scheme, recon, nghost)
-                               and not lib().hydro_lean_fits(es, scheme, recon, nghost)):
+    if impl == IMPL_STAGED or (impl == IMPL_AUTO and not lib().hydro_fused_fits(es, scheme, recon, nghost)):
         return lib().hydro_staged_workspace_bytes(Ng, es, scheme, recon)
     return 0
 

@@ -14,18 +14,12 @@ namespace hydro {
 
 // ---- dispatch tables ---------------------------------------------------------------------------
 #define DECL_STAGED(R, S, RC, RS) extern template cudaError_t launch_staged<R, S, RC, RS>(const SolveArgs<R>&);
-#define DECL_FUSED(R, S, RC, RS) extern template cudaError_t launch_fused<R, S, RC, RS>(const SolveArgs<R>&);
-#define DECL_WS(R, S, RC, RS) extern template cudaError_t launch_ws<R, S, RC, RS>(const SolveArgs<R>&);
 #define DECL_LEAN(R, S, RC, RS) extern template cudaError_t launch_lean<R, S, RC, RS>(const SolveArgs<R>&);
 #define FOR_RS(M, R, S, RC) M(R, S, RC, RS_EXACT) M(R, S, RC, RS_HLLE) M(R, S, RC, RS_HLLC) M(R, S, RC, RS_ROE)
 #define FOR_RC(M, R, S) FOR_RS(M, R, S, RECON_PLM) FOR_RS(M, R, S, RECON_PPM)
 #define FOR_S(M, R) FOR_RC(M, R, SCHEME_MHM) FOR_RC(M, R, SCHEME_VL) FOR_RC(M, R, SCHEME_CTU)
 FOR_S(DECL_STAGED, float)
 FOR_S(DECL_STAGED, double)
-FOR_S(DECL_FUSED, float)
-FOR_S(DECL_FUSED, double)
-FOR_S(DECL_WS, float)
-FOR_S(DECL_WS, double)
 FOR_S(DECL_LEAN, float)
 FOR_S(DECL_LEAN, double)
 
@@ -39,27 +33,6 @@ template <class R> static LaunchFn<R> staged_fn(int scheme, int recon, int rs) {
 #undef ROW
   return t[scheme][recon][rs];
 }
-template <class R> static LaunchFn<R> fused_fn(int scheme, int recon, int rs) {
-#define ROW(R_, S, RC) {&launch_fused<R_, S, RC, RS_EXACT>, &launch_fused<R_, S, RC, RS_HLLE>, \
-                        &launch_fused<R_, S, RC, RS_HLLC>, &launch_fused<R_, S, RC, RS_ROE>}
-  static const LaunchFn<R> t[3][2][4] = {
-      {ROW(R, SCHEME_MHM, RECON_PLM), ROW(R, SCHEME_MHM, RECON_PPM)},
-      {ROW(R, SCHEME_VL, RECON_PLM), ROW(R, SCHEME_VL, RECON_PPM)},
-      {ROW(R, SCHEME_CTU, RECON_PLM), ROW(R, SCHEME_CTU, RECON_PPM)}};
-#undef ROW
-  return t[scheme][recon][rs];
-}
-template <class R> static LaunchFn<R> ws_fn(int scheme, int recon, int rs) {
-#define ROW(R_, S, RC) {&launch_ws<R_, S, RC, RS_EXACT>, &launch_ws<R_, S, RC, RS_HLLE>, \
-                        &launch_ws<R_, S, RC, RS_HLLC>, &launch_ws<R_, S, RC, RS_ROE>}
-  static const LaunchFn<R> t[3][2][4] = {
-      {ROW(R, SCHEME_MHM, RECON_PLM), ROW(R, SCHEME_MHM, RECON_PPM)},
-      {ROW(R, SCHEME_VL, RECON_PLM), ROW(R, SCHEME_VL, RECON_PPM)},
-      {ROW(R, SCHEME_CTU, RECON_PLM), ROW(R, SCHEME_CTU, RECON_PPM)}};
-#undef ROW
-  return t[scheme][recon][rs];
-}
-
 template <class R> static LaunchFn<R> lean_fn(int scheme, int recon, int rs) {
 #define ROW(R_, S, RC) {&launch_lean<R_, S, RC, RS_EXACT>, &launch_lean<R_, S, RC, RS_HLLE>, \
                         &launch_lean<R_, S, RC, RS_HLLC>, &launch_lean<R_, S, RC, RS_ROE>}
@@ -180,7 +153,7 @@ static int dt_impl(const R* u, int Ng, int nghost, R gamma, int norm, R* max_spe
 
 // ---- hydro_solve ---------------------------------------------------------------------------------
 struct Plan {
-  int recon, g, impl;  // impl resolved to STAGED, FUSED or WS
+  int recon, g, impl;  // impl resolved to STAGED or FUSED
 };
 
 template <class R>
@@ -190,7 +163,7 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   const int recon = o ? o->recon : 0;
   const int fb = (o && o->roe_fallback) ? o->roe_fallback : 1;
   const int impl = o ? o->impl : 0;
-  if (recon < 0 || recon > 1 || fb < 1 || fb > 3 || impl < 0 || impl > 4) return HYDRO_E_ENUM;
+  if (recon < 0 || recon > 1 || fb < 1 || fb > 3 || impl < 0 || impl > 2) return HYDRO_E_ENUM;
   if (o && (o->char_limit < 0 || o->char_limit > 1)) return HYDRO_E_ENUM;
   if (Ng < 0) return HYDRO_E_COUNT;
   if (Ng > 0 && (!in || !out)) return HYDRO_E_NULL;
@@ -214,18 +187,11 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   par.limiter = limiter;
   par.char_limit = o ? o->char_limit : 0;
   par.roe_fallback = fb;
-  const bool has = fused_fits((int)sizeof(R), scheme, recon, g);  // kernel exists and its tiles fit in shared memory
-  const bool has_ws = ws_fits((int)sizeof(R), scheme, recon, g);
-  const bool has_lean = lean_fits((int)sizeof(R), scheme, recon, g);
-  if (impl == HYDRO_IMPL_FUSED && !has) return HYDRO_E_NOFUSED;  // no kernel, or its tiles do not fit for this g
-  if (impl == HYDRO_IMPL_WS && !has_ws) return HYDRO_E_NOFUSED;
-  if (impl == HYDRO_IMPL_LEAN && !has_lean) return HYDRO_E_NOFUSED;
+  const bool has = lean_fits((int)sizeof(R), scheme, recon, g);  // kernel exists and its tiles fit in shared memory
+  if (impl == HYDRO_IMPL_FUSED && !has) return HYDRO_E_NOFUSED;
   pl.recon = recon;
   pl.g = g;
-  if (impl == HYDRO_IMPL_STAGED) pl.impl = HYDRO_IMPL_STAGED;
-  else if (impl == HYDRO_IMPL_LEAN || (impl == HYDRO_IMPL_AUTO && has_lean)) pl.impl = HYDRO_IMPL_LEAN;
-  else if (impl == HYDRO_IMPL_WS || (impl == HYDRO_IMPL_AUTO && has_ws)) pl.impl = HYDRO_IMPL_WS;
-  else pl.impl = has ? HYDRO_IMPL_FUSED : HYDRO_IMPL_STAGED;
+  pl.impl = (impl != HYDRO_IMPL_STAGED && has) ? HYDRO_IMPL_FUSED : HYDRO_IMPL_STAGED;
   return HYDRO_OK;
 }
 
@@ -253,9 +219,7 @@ static int solve_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, i
       return HYDRO_E_WORKSPACE;
     return (int)staged_fn<R>(scheme, pl.recon, riemann)(a);
   }
-  if (pl.impl == HYDRO_IMPL_LEAN) return (int)lean_fn<R>(scheme, pl.recon, riemann)(a);
-  if (pl.impl == HYDRO_IMPL_WS) return (int)ws_fn<R>(scheme, pl.recon, riemann)(a);
-  return (int)fused_fn<R>(scheme, pl.recon, riemann)(a);
+  return (int)lean_fn<R>(scheme, pl.recon, riemann)(a);
 }
 
 }  // namespace hydro
@@ -357,27 +321,11 @@ int hydro_min_ghost(int scheme, int recon) {
 int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann) {
   if (scheme < 0 || scheme > 2 || recon < 0 || recon > 1 || riemann < 0 || riemann > 3) return 0;
   if (precision_bytes != 4 && precision_bytes != 8) return 0;
-  return hydro::fused_available(precision_bytes, scheme, recon) ? 1 : 0;
+  return hydro::lean_available(precision_bytes, scheme, recon) ? 1 : 0;
 }
 
 int hydro_fused_fits(int precision_bytes, int scheme, int recon, int nghost) {
   if (!hydro_has_fused(precision_bytes, scheme, recon, 0)) return 0;
-  if (nghost == 0) nghost = hydro::min_ghost(scheme, recon);
-  if (nghost < hydro::min_ghost(scheme, recon) || nghost > 8) return 0;
-  return hydro::fused_fits(precision_bytes, scheme, recon, nghost) ? 1 : 0;
-}
-
-int hydro_ws_fits(int precision_bytes, int scheme, int recon, int nghost) {
-  if (scheme < 0 || scheme > 2 || recon < 0 || recon > 1) return 0;
-  if (precision_bytes != 4 && precision_bytes != 8) return 0;
-  if (nghost == 0) nghost = hydro::min_ghost(scheme, recon);
-  if (nghost < hydro::min_ghost(scheme, recon) || nghost > 8) return 0;
-  return hydro::ws_fits(precision_bytes, scheme, recon, nghost) ? 1 : 0;
-}
-
-int hydro_lean_fits(int precision_bytes, int scheme, int recon, int nghost) {
-  if (scheme < 0 || scheme > 2 || recon < 0 || recon > 1) return 0;
-  if (precision_bytes != 4 && precision_bytes != 8) return 0;
   if (nghost == 0) nghost = hydro::min_ghost(scheme, recon);
   if (nghost < hydro::min_ghost(scheme, recon) || nghost > 8) return 0;
   return hydro::lean_fits(precision_bytes, scheme, recon, nghost) ? 1 : 0;
@@ -391,8 +339,7 @@ size_t hydro_staged_workspace_bytes(int Ng, int precision_bytes, int scheme, int
 }
 
 size_t hydro_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon) {
-  if (hydro_fused_fits(precision_bytes, scheme, recon, 8) || hydro_ws_fits(precision_bytes, scheme, recon, 8) ||
-      hydro_lean_fits(precision_bytes, scheme, recon, 8)) return 0;
+  if (hydro_fused_fits(precision_bytes, scheme, recon, 8)) return 0;
   return hydro_staged_workspace_bytes(Ng, precision_bytes, scheme, recon);
 }
 

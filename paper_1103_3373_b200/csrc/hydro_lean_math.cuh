@@ -3,7 +3,7 @@
 //
 // Same readings as hydro_math.cuh (S1-S24), algebraically rearranged so that the kernel
 // issues fewer instructions: the profile of the first fused kernels showed the path bound by
-// instruction issue, not by HBM (profiles/r1_ncu_ws_f32_v2.md), so what counts is the number of
+// instruction issue, not by HBM (profiles/r1_ncu_fused_f32_v1.md), so what counts is the number of
 // FP32/FP64 + MUFU instructions per Riemann solve and per reconstruction.
 //   * branch-free limiter and tracing (selects, no divergent control flow);
 //   * the characteristic projection of the tracing written out per component with one rsqrt

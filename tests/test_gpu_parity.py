@@ -18,7 +18,7 @@ MHM, VL, CTU = 0, 1, 2
 EXACT, HLLE, HLLC, ROE = 0, 1, 2, 3
 GMINMOD, VANLEER, VANALBADA, HYBRID = 0, 1, 2, 3
 PLM, PPM = 0, 1
-AUTO, STAGED, FUSED, WS, LEAN = 0, 1, 2, 3, 4
+AUTO, STAGED, FUSED = 0, 1, 2
 PS = 16
 TOL64, TOL32 = 1e-12, 1e-5
 
@@ -72,10 +72,6 @@ def impls(B, dtype, scheme, recon, g=0):
     r = (STAGED,)
     if B.hydro_fused_fits(t, scheme, recon, g):
         r += (FUSED,)
-    if B.hydro_ws_fits(t, scheme, recon, g):
-        r += (WS,)
-    if B.hydro_lean_fits(t, scheme, recon, g):
-        r += (LEAN,)
     return r
 
 
