@@ -45,12 +45,19 @@ constexpr size_t lean_smem_bytes(size_t elem, int recon, int g) {
   const size_t S = PS + 2 * g, SWP = PS + 2 * (2 + recon), NW = 2 * (1 + recon) + 1;
   return 64 + elem * (2 * 5 * S * S + NW * 5 * SWP * SWP + (size_t)20 * LEAN_NT + (size_t)30 * LEAN_COLS);
 }
+// fused MHM kernel (hydro_lean_mhm.cuh): mbarriers | raw planes | W ring | LOX UPX LOY UPY FX FY
+constexpr size_t mhm_smem_bytes(size_t elem, int recon, int g) {
+  const size_t S = PS + 2 * g, SWP = PS + 2 * (2 + recon), NW = 2 * (1 + recon) + 1;
+  return 64 + elem * (2 * 5 * S * S + NW * 5 * SWP * SWP + (size_t)30 * LEAN_COLS);
+}
 constexpr bool lean_available(int precision_bytes, int scheme, int recon) {
   (void)precision_bytes; (void)recon;
-  return scheme == SCHEME_CTU;
+  return scheme == SCHEME_CTU || scheme == SCHEME_MHM;
 }
 constexpr bool lean_fits(int precision_bytes, int scheme, int recon, int g) {
-  return lean_available(precision_bytes, scheme, recon) && lean_smem_bytes((size_t)precision_bytes, recon, g) <= SMEM_MAX_OPTIN;
+  return lean_available(precision_bytes, scheme, recon) &&
+         (scheme == SCHEME_MHM ? mhm_smem_bytes((size_t)precision_bytes, recon, g) : lean_smem_bytes((size_t)precision_bytes, recon, g)) <=
+             SMEM_MAX_OPTIN;
 }
 
 template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_lean(const SolveArgs<R>& a);

@@ -3,6 +3,7 @@
 #pragma once
 #include "hydro_launch.cuh"
 #include "hydro_lean_ctu.cuh"
+#include "hydro_lean_mhm.cuh"
 
 namespace hydro {
 
@@ -15,6 +16,11 @@ template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_lean(const 
     const bool fast = a.par.limiter == LIM_VANLEER && !a.par.char_limit && !(a.par.min_dens > R(0)) && !(a.par.min_pres > R(0));
     if (fast) return launch_ctu_lean<R, RECON, RS, 1, LeanTune<R, RECON>::MINB>(a);
     return launch_ctu_lean<R, RECON, RS, 0, LeanTune<R, RECON>::MINB>(a);
+  } else if constexpr (SCHEME == SCHEME_MHM) {
+    const bool fast = a.par.limiter == LIM_VANLEER && !a.par.char_limit && !(a.par.min_dens > R(0)) && !(a.par.min_pres > R(0));
+    constexpr int MINB = sizeof(R) == 4 ? 2 : 1;
+    if (fast) return launch_mhm_lean<R, RECON, RS, 1, MINB>(a);
+    return launch_mhm_lean<R, RECON, RS, 0, MINB>(a);
   } else {
     (void)a;
     return cudaErrorNotSupported;

@@ -1,0 +1,276 @@
+// hydro_lean_mhm.cuh -- fused z-marching MHM (MUSCL-Hancock) kernel: PAPER.md:35, 46, 93 -- steps (1)-(5) of
+// PAPER.md:39-44 with the half-step of the face values taken from cell-local flux differences of all three
+// directions, no Riemann solver in the predictor, three Riemann solves per cell.
+//
+// Same organisation as hydro_lean_ctu.cuh: persistent 320-thread CTAs (two per SM where the tiles allow),
+// one thread per column of the 18 x 18 tile (MHM never touches the four corner columns), primitive planes in
+// a ring fed by 1-D bulk async copies, packed "4+1" shared-memory fields.  MHM needs only two barriers per plane:
+//   P1  untraced face states of plane t in x, y, z (S6/S7); Hancock increment (hnu * sum_d [F_d(W+_d) - F_d(W-_d)],
+//       S13: one increment for the six face values of the cell); advanced x,y states -> LOX UPX LOY UPY;
+//       z is column-local: F_z(t) = RS(up_z(t-1), lo_z(t)), boundary-flux store, conservative update and
+//       store of plane t-1 as U - nu (D_z + F_z(t))                                               | barrier A
+//   P2  F_x(t), F_y(t) -> FX, FY; patch-boundary flux stores; con->prim of the next raw plane     | barrier B
+//   P3  carried D_z = (dF_x + dF_y)(t) - F_z(t)
+#pragma once
+#include <cstdint>
+#include "hydro_launch.cuh"
+#include "hydro_lean_ctu.cuh"
+
+namespace hydro {
+
+// untraced PLM face values, van Leer limiter on primitive variables (normal frame irrelevant: per component)
+template <class R> __device__ __forceinline__ void lean_plm(const V5<R>& Wm, const V5<R>& W0, const V5<R>& Wp, V5<R>& lo, V5<R>& up) {
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    const R h = R(0.5) * vl_slope(W0[q] - Wm[q], Wp[q] - W0[q]);
+    lo[q] = W0[q] - h;
+    up[q] = W0[q] + h;
+  }
+}
+// physical flux along D of an xyz-frame primitive state; (E + P) = gamma/(gamma-1) P + rho |v|^2 / 2
+template <int D, class R> __device__ __forceinline__ V5<R> lean_phys_flux(const V5<R>& W, const Par<R>& p) {
+  const R u = W[1 + D], m = W[0] * u;
+  const R hq = R(0.5) * m_fma(W[3], W[3], m_fma(W[2], W[2], W[1] * W[1]));
+  V5<R> F;
+  F[0] = m;
+  F[1] = m * W[1];
+  F[2] = m * W[2];
+  F[3] = m * W[3];
+  F[1 + D] += W[4];
+  F[4] = m_fma(m, hq, u * ((p.gamma * p.igm1) * W[4]));
+  return F;
+}
+
+template <class R, int RECON, int RS, int FAST> struct MhmOps {
+  using Op = LeanOps<R, RECON, RS, FAST>;
+  // untraced face states of the middle cell along D (xyz-frame in and out)
+  template <int D>
+  static __device__ __forceinline__ void recon(const V5<R>& Wm2, const V5<R>& Wm1, const V5<R>& W0, const V5<R>& Wp1,
+                                               const V5<R>& Wp2, const Par<R>& p, V5<R>& lo, V5<R>& up) {
+    if (FAST && RECON == RECON_PLM) {
+      lean_plm(Wm1, W0, Wp1, lo, up);
+    } else {
+      V5<R> l, u;
+      reconstruct<RECON, false>(to_normal<D>(Wm2), to_normal<D>(Wm1), to_normal<D>(W0), to_normal<D>(Wp1), to_normal<D>(Wp2), p, l, u);
+      lo = from_normal<D>(l);
+      up = from_normal<D>(u);
+    }
+  }
+  template <int D> static __device__ __forceinline__ V5<R> flux(const V5<R>& W, const Par<R>& p) {
+    if (FAST) return lean_phys_flux<D>(W, p);
+    return from_normal<D>(phys_flux(to_normal<D>(W), p));
+  }
+};
+
+template <class R, int RECON, int RS, int FAST, int MINB>
+__global__ void __launch_bounds__(LEAN_NT, MINB)
+mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, Par<R> p,
+                const R* __restrict__ max_speed, R cfl, long long* status) {
+  using Op = LeanOps<R, RECON, RS, FAST>;
+  using Mo = MhmOps<R, RECON, RS, FAST>;
+  constexpr int GW = 2 + RECON, RW = 1 + RECON, SWP = PS + 2 * GW, WPL = SWP * SWP, NW = 2 * RW + 1, NPL = PS + 2 * GW;
+  constexpr int NC = LEAN_COLS, NT = LEAN_NT, FT = PS + 2;
+  apply_device_dt(p, max_speed, cfl);
+
+  const int S = PS + 2 * g;
+  const int SS = S * S;
+  const size_t nS = (size_t)SS * S;
+  const int off = g - GW;  // unused outer ghost layers
+
+  extern __shared__ __align__(16) unsigned char smem[];
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
+  R* ring = reinterpret_cast<R*>(smem + 64);           // [NW] fields of WPL cells: primitive planes t-RW .. t+RW
+  R* xy = ring + NW * 5 * WPL;                         // [6] fields of NC cells: LOX UPX LOY UPY FX FY
+  R* raw = xy + 6 * 5 * NC;                            // [2][5][SS] landing zone of the bulk copies
+  auto fld = [&](int k) { return xy + k * 5 * NC; };
+
+  const int tid = threadIdx.x;
+  int ii, jj;
+  if (tid < PS * FT) { jj = 1 + tid / FT; ii = tid - (jj - 1) * FT; }
+  else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
+  const int col = jj * FT + ii;
+  const bool in_i = ii >= 1 && ii <= PS, in_j = jj >= 1 && jj <= PS, interior = in_i && in_j;
+  const int wb = (jj + GW - 1) * SWP + (ii + GW - 1);
+
+  const int my_groups = (Ng - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int total_planes = my_groups * NPL;
+  auto issue = [&](int n) {  // thread 0 only
+    if (n >= total_planes) return;
+    const int m = n / NPL, pl = n - m * NPL;
+    const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
+    const R* src = in + grp * 5 * nS + (size_t)(pl + off) * SS;
+    uint64_t* b = bar + (n & 1);
+    R* dst = raw + (size_t)(n & 1) * 5 * SS;
+    mbar_expect_tx(b, (uint32_t)(5 * SS * sizeof(R)));
+#pragma unroll
+    for (int q = 0; q < 5; ++q) bulk_g2s(dst + (size_t)q * SS, src + q * nS, (uint32_t)(SS * sizeof(R)), b);
+  };
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    mbar_init(bar + 1, 1);
+    fence_mbar_init();
+    fence_async_smem();
+  }
+  __syncthreads();
+  if (tid == 0) { issue(0); issue(1); }
+
+  Cnt c = {0, 0, 0};
+  int nseq = 0;
+  auto convert = [&](int slot) {
+    const int st = nseq & 1;
+    mbar_wait(bar + st, (uint32_t)((nseq >> 1) & 1));
+    const R* rp = raw + (size_t)st * 5 * SS;
+    R* wp = ring + slot * 5 * WPL;
+    for (int idx = tid; idx < WPL; idx += NT) {
+      const int b = idx / SWP, a = idx - b * SWP;
+      stv(wp, WPL, idx, Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c));
+    }
+  };
+  auto refill = [&]() {
+    if (tid == 0) { fence_async_smem(); issue(nseq + 2); }
+    ++nseq;
+  };
+
+  V5<R> uzc, Dz;  // advanced up_z of plane t-1; (dF_x + dF_y) - F_z of plane t-1
+#pragma unroll
+  for (int q = 0; q < 5; ++q) { uzc[q] = R(0); Dz[q] = R(0); }
+
+  for (int m = 0; m < my_groups; ++m) {
+    const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
+    const R* gin0 = in + grp * 5 * nS + ((size_t)g * S + (jj - 1 + g)) * S + (ii - 1 + g);
+    R* gout0 = out + grp * 5 * PS * PS * PS + (jj - 1) * PS + (ii - 1);
+    R* gff = face_flux ? face_flux + grp * 9 * 5 * PS * PS : nullptr;
+    for (int k = 0; k < NW; ++k) {  // prologue: planes -1-RW .. -1+RW
+      convert(k);
+      __syncthreads();
+      refill();
+    }
+    int sl = 0;  // ring slot of plane t-RW
+
+#pragma unroll 1
+    for (int t = -1; t <= PS; ++t) {
+      const bool tin = t >= 0 && t < PS;
+      int slot[NW];
+#pragma unroll
+      for (int s = 0; s < NW; ++s) slot[s] = (sl + s < NW) ? sl + s : sl + s - NW;
+      // ================= P1: face states of plane t, Hancock half step, F_z(t), update of plane t-1 =================
+      if (tin || interior) {
+        V5<R> Uold;
+        const bool upd = interior && t >= 1;
+        if (upd) {
+          const R* gin = gin0 + (t - 1) * SS;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += nS; }
+        }
+        const R* wpl = ring + slot[RW] * 5 * WPL;
+        const V5<R> W0 = ldv(wpl, WPL, wb);
+        V5<R> lox, upx, loy, upy, loz, upz, inc;
+        {
+          const V5<R> Wb = ldv(wpl, WPL, wb - 1), Wc = ldv(wpl, WPL, wb + 1);
+          V5<R> Wa = Wb, Wd = Wc;
+          if (RECON == RECON_PPM) { Wa = ldv(wpl, WPL, wb - 2); Wd = ldv(wpl, WPL, wb + 2); }
+          Mo::template recon<0>(Wa, Wb, W0, Wc, Wd, p, lox, upx);
+          const V5<R> fu = Mo::template flux<0>(upx, p), fl = Mo::template flux<0>(lox, p);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) inc[q] = fu[q] - fl[q];
+        }
+        {
+          const V5<R> Wb = ldv(wpl, WPL, wb - SWP), Wc = ldv(wpl, WPL, wb + SWP);
+          V5<R> Wa = Wb, Wd = Wc;
+          if (RECON == RECON_PPM) { Wa = ldv(wpl, WPL, wb - 2 * SWP); Wd = ldv(wpl, WPL, wb + 2 * SWP); }
+          Mo::template recon<1>(Wa, Wb, W0, Wc, Wd, p, loy, upy);
+          const V5<R> fu = Mo::template flux<1>(upy, p), fl = Mo::template flux<1>(loy, p);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) inc[q] = inc[q] + (fu[q] - fl[q]);
+        }
+        {
+          const V5<R> Wb = ldv(ring + slot[RW - 1] * 5 * WPL, WPL, wb), Wc = ldv(ring + slot[RW + 1] * 5 * WPL, WPL, wb);
+          V5<R> Wa = Wb, Wd = Wc;
+          if (RECON == RECON_PPM) { Wa = ldv(ring + slot[0] * 5 * WPL, WPL, wb); Wd = ldv(ring + slot[2 * RW] * 5 * WPL, WPL, wb); }
+          Mo::template recon<2>(Wa, Wb, W0, Wc, Wd, p, loz, upz);
+          const V5<R> fu = Mo::template flux<2>(upz, p), fl = Mo::template flux<2>(loz, p);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) inc[q] = p.hnu * (inc[q] + (fu[q] - fl[q]));
+        }
+        if (tin && in_j) {
+          stv(fld(LF_LOX), NC, col, Op::correct(lox, inc, p, c));
+          stv(fld(LF_UPX), NC, col, Op::correct(upx, inc, p, c));
+        }
+        if (tin && in_i) {
+          stv(fld(LF_LOY), NC, col, Op::correct(loy, inc, p, c));
+          stv(fld(LF_UPY), NC, col, Op::correct(upy, inc, p, c));
+        }
+        if (interior) {
+          if (t >= 0) {
+            const V5<R> Fz = Op::template riemann<2>(uzc, Op::correct(loz, inc, p, c), p, c);
+            if (gff && (t & 7) == 0) st5(gff + (size_t)((6 + (t >> 3)) * 5) * 256 + (jj - 1) * PS + (ii - 1), 256, Fz);
+            if (upd) {
+              V5<R> U;
+#pragma unroll
+              for (int q = 0; q < 5; ++q) U[q] = Uold[q] - p.nu * (Dz[q] + Fz[q]);
+              const V5<R> Wn = Op::c2p(U, p, c);
+              if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
+              st5(gout0 + (t - 1) * PS * PS, PS * PS * PS, U);
+            }
+            Dz = Fz;
+          }
+          if (t < PS) uzc = Op::correct(upz, inc, p, c);
+        }
+      }
+      __syncthreads();  // barrier A
+
+      // ================= P2: F_x(t), F_y(t), boundary-flux stores; con->prim of the next plane =================
+      if (tin) {
+        if (in_j && ii >= 1) {
+          const V5<R> f = Op::template riemann<0>(ldv(fld(LF_UPX), NC, col - 1), ldv(fld(LF_LOX), NC, col), p, c);
+          stv(fld(LF_FX), NC, col, f);
+          if (gff && ((ii - 1) & 7) == 0) st5(gff + (size_t)(((ii - 1) >> 3) * 5) * 256 + t * PS + (jj - 1), 256, f);
+        }
+        if (in_i && jj >= 1) {
+          const V5<R> f = Op::template riemann<1>(ldv(fld(LF_UPY), NC, col - FT), ldv(fld(LF_LOY), NC, col), p, c);
+          stv(fld(LF_FY), NC, col, f);
+          if (gff && ((jj - 1) & 7) == 0) st5(gff + (size_t)((3 + ((jj - 1) >> 3)) * 5) * 256 + t * PS + (ii - 1), 256, f);
+        }
+      }
+      const bool conv = t + RW + 1 <= PS - 1 + GW;  // plane t+RW+1 replaces plane t-RW (read for the last time in P1)
+      if (conv) convert(sl);
+      __syncthreads();  // barrier B
+      if (conv) refill();
+
+      // ================= P3: carried x+y flux difference of plane t minus F_z(t) =================
+      if (tin && interior) {
+        const V5<R> x1 = ldv(fld(LF_FX), NC, col + 1), x0 = ldv(fld(LF_FX), NC, col);
+        const V5<R> y1 = ldv(fld(LF_FY), NC, col + FT), y0 = ldv(fld(LF_FY), NC, col);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) Dz[q] = ((x1[q] - x0[q]) + (y1[q] - y0[q])) - Dz[q];
+      }
+      sl = (sl + 1 < NW) ? sl + 1 : 0;
+    }
+  }
+  flush_counters(c, status);
+}
+
+template <class R, int RECON, int RS, int FAST, int MINB> cudaError_t launch_mhm_lean(const SolveArgs<R>& a) {
+  auto kern = mhm_lean_kernel<R, RECON, RS, FAST, MINB>;
+  const size_t smem = mhm_smem_bytes(sizeof(R), RECON, a.g);
+  if (smem > SMEM_MAX_OPTIN) return cudaErrorInvalidConfiguration;
+  static int sms = 0;
+  if (!sms) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (sms <= 0) sms = 148;
+  }
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, LEAN_NT, smem);
+  if (e != cudaSuccess) return e;
+  if (per_sm < 1) return cudaErrorInvalidConfiguration;
+  long long grid = (long long)sms * per_sm;
+  if (grid > a.Ng) grid = a.Ng;
+  kern<<<(unsigned)grid, LEAN_NT, smem, a.stream>>>(a.in, a.out, a.face_flux, a.Ng, a.g, a.par, a.max_speed, a.cfl, a.status);
+  return cudaGetLastError();
+}
+
+}  // namespace hydro
