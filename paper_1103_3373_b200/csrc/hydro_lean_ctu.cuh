@@ -53,6 +53,7 @@ template <class R, int RECON, int RS, int FAST> struct LeanOps {
   static __device__ __forceinline__ void recon(const V5<R>& Wm2, const V5<R>& Wm1, const V5<R>& W0, const V5<R>& Wp1,
                                                const V5<R>& Wp2, const Par<R>& p, V5<R>& lo, V5<R>& up) {
     if (FAST && RECON == RECON_PLM) lean_plm_trace(Wm1, W0, Wp1, p, p.nu, p.hnu, lo, up);
+    else if (FAST) lean_ppm_trace(Wm2, Wm1, W0, Wp1, Wp2, p, p.nu, lo, up);
     else reconstruct<RECON, true>(Wm2, Wm1, W0, Wp1, Wp2, p, lo, up);
   }
   template <int D> static __device__ __forceinline__ V5<R> riemann(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {

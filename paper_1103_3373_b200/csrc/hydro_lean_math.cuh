@@ -97,6 +97,90 @@ __device__ __forceinline__ void lean_plm_trace(const V5<R>& Wm, const V5<R>& W0,
   lo[4] = m_fma(km, s[4], W0[4]) + B4;
 }
 
+// ---- c2-c3: PPM (S6: Colella-Woodward interpolation + monotonisation, no steepening / flattening), van Leer slopes on
+// primitive variables, branch-free.  Parabola of the middle cell: edge values wl, wr; D = wr - wl; W6 = 6 (w0 - (wl+wr)/2)
+template <class R>
+__device__ __forceinline__ void lean_ppm_parabola(const V5<R>& Wm2, const V5<R>& Wm1, const V5<R>& W0, const V5<R>& Wp1,
+                                                  const V5<R>& Wp2, V5<R>& WL, V5<R>& WR) {
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    const R w0 = W0[q];
+    const R dLm = Wm1[q] - Wm2[q], dL = w0 - Wm1[q], dR = Wp1[q] - w0, dRp = Wp2[q] - Wp1[q];
+    const R sm = vl_slope(dLm, dL), s0 = vl_slope(dL, dR), sp = vl_slope(dR, dRp);
+    R wl = m_fma(R(-1.0 / 6.0), s0 - sm, R(0.5) * (Wm1[q] + w0));
+    R wr = m_fma(R(-1.0 / 6.0), sp - s0, R(0.5) * (w0 + Wp1[q]));
+    const bool ext = (wr - w0) * (w0 - wl) <= R(0);
+    const R dd = wr - wl, m6 = R(6) * m_fma(R(-0.5), wl + wr, w0);
+    const R t = dd * m6, d2 = dd * dd;
+    const bool c1 = t > d2, c2 = !c1 && t < -d2;
+    const R wl1 = m_fma(R(-2), wr, R(3) * w0), wr1 = m_fma(R(-2), wl, R(3) * w0);
+    wl = ext ? w0 : (c1 ? wl1 : wl);
+    wr = ext ? w0 : (c2 ? wr1 : wr);
+    WL[q] = wl;
+    WR[q] = wr;
+  }
+}
+// untraced PPM face values (MHM, VL)
+template <class R>
+__device__ __forceinline__ void lean_ppm(const V5<R>& Wm2, const V5<R>& Wm1, const V5<R>& W0, const V5<R>& Wp1, const V5<R>& Wp2,
+                                         V5<R>& lo, V5<R>& up) {
+  lean_ppm_parabola(Wm2, Wm1, W0, Wp1, Wp2, lo, up);
+}
+// PPM + CTU characteristic tracing to dt/2 (S5: reference-state form, approaching waves only), normal frame
+template <class R>
+__device__ __forceinline__ void lean_ppm_trace(const V5<R>& Wm2, const V5<R>& Wm1, const V5<R>& W0, const V5<R>& Wp1,
+                                               const V5<R>& Wp2, const Par<R>& p, R nu, V5<R>& lo, V5<R>& up) {
+  V5<R> WL, WR, D, W6;
+  lean_ppm_parabola(Wm2, Wm1, W0, Wp1, Wp2, WL, WR);
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    D[q] = WR[q] - WL[q];
+    W6[q] = R(6) * m_fma(R(-0.5), WL[q] + WR[q], W0[q]);
+  }
+  const R gP = p.gamma * W0[4], x = gP * W0[0];
+  const R irc = m_rsqrt(x);
+  const R c = gP * irc, ic = W0[0] * irc, ic2 = ic * ic, rc = x * irc;
+  const R u = W0[1], lamM = u + c, lam0 = u - c;
+  const R nc = nu * c, n23 = nu * nu * R(1.0 / 3.0), uc = u * c, c2 = c * c;
+  // upper face (lambda > 0): A = (nu/2)(lamM - lambda), B = (nu^2/3)(lamM^2 - lambda^2); per wave V = A D + (B - A) W6
+  const bool p0 = lam0 > R(0), p1 = u > R(0), m1 = u < R(0), m4 = lamM < R(0);
+  const R A0 = p0 ? nc : R(0), BA0 = p0 ? m_fma(n23, R(4) * uc, -nc) : R(0);
+  const R A1 = p1 ? R(0.5) * nc : R(0), BA1 = p1 ? m_fma(n23, uc + uc + c2, R(-0.5) * nc) : R(0);
+  // lower face (lambda < 0): C = (nu/2)(lam0 - lambda), Dk = (nu^2/3)(lam0^2 - lambda^2); per wave V = C D + (C + Dk) W6
+  const R C1 = m1 ? R(-0.5) * nc : R(0), CD1 = m1 ? m_fma(n23, c2 - (uc + uc), R(-0.5) * nc) : R(0);
+  const R C4 = m4 ? -nc : R(0), CD4 = m4 ? m_fma(n23, R(-4) * uc, -nc) : R(0);
+  const R sgp = nu * m_max(lamM, R(0)), sgm = nu * m_min(lam0, R(0));
+  const R kp = m_fma(R(-2.0 / 3.0), sgp, R(1)), km = m_fma(R(2.0 / 3.0), sgm, R(1));
+  const R hp = R(-0.5) * sgp, hm = R(-0.5) * sgm;
+  // acoustic amplitudes times c^2: (L . V) c^2 = (V_P -+ rho c V_u) / 2
+  const R V0u = m_fma(A0, D[1], BA0 * W6[1]), V0p = m_fma(A0, D[4], BA0 * W6[4]);
+  const R V4u = m_fma(C4, D[1], CD4 * W6[1]), V4p = m_fma(C4, D[4], CD4 * W6[4]);
+  const R B0 = R(0.5) * m_fma(-rc, V0u, V0p), B4 = R(0.5) * m_fma(rc, V4u, V4p);
+  // entropy / shear waves
+  V5<R> V1, Vm;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    V1[q] = m_fma(A1, D[q], BA1 * W6[q]);
+    Vm[q] = m_fma(C1, D[q], CD1 * W6[q]);
+  }
+  V5<R> bu, bl;  // W_R - (sgp/2)(D - kp W6),  W_L - (sgm/2)(D + km W6)
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    bu[q] = m_fma(hp, m_fma(-kp, W6[q], D[q]), WR[q]);
+    bl[q] = m_fma(hm, m_fma(km, W6[q], D[q]), WL[q]);
+  }
+  up[0] = m_fma(B0, ic2, m_fma(-V1[4], ic2, V1[0])) + bu[0];
+  up[1] = m_fma(-B0, irc, bu[1]);
+  up[2] = bu[2] + V1[2];
+  up[3] = bu[3] + V1[3];
+  up[4] = bu[4] + B0;
+  lo[0] = m_fma(B4, ic2, m_fma(-Vm[4], ic2, Vm[0])) + bl[0];
+  lo[1] = m_fma(B4, irc, bl[1]);
+  lo[2] = bl[2] + Vm[2];
+  lo[3] = bl[3] + Vm[3];
+  lo[4] = bl[4] + B4;
+}
+
 // ---- c4: Roe's solver, primitive-jump form (normal frame in, normal-frame flux out) ------------
 // per-state quantities of a Riemann problem
 template <class R> struct LeanState { R ir, sq, H, m, F1, F2, F3, F4; };

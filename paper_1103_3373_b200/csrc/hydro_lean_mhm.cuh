@@ -49,6 +49,8 @@ template <class R, int RECON, int RS, int FAST> struct MhmOps {
                                                const V5<R>& Wp2, const Par<R>& p, V5<R>& lo, V5<R>& up) {
     if (FAST && RECON == RECON_PLM) {
       lean_plm(Wm1, W0, Wp1, lo, up);
+    } else if (FAST) {
+      lean_ppm(Wm2, Wm1, W0, Wp1, Wp2, lo, up);
     } else {
       V5<R> l, u;
       reconstruct<RECON, false>(to_normal<D>(Wm2), to_normal<D>(Wm1), to_normal<D>(W0), to_normal<D>(Wp1), to_normal<D>(Wp2), p, l, u);
