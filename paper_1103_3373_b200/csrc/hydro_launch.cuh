@@ -50,14 +50,22 @@ constexpr size_t mhm_smem_bytes(size_t elem, int recon, int g) {
   const size_t S = PS + 2 * g, SWP = PS + 2 * (2 + recon), NW = 2 * (1 + recon) + 1;
   return 64 + elem * (2 * 5 * S * S + NW * 5 * SWP * SWP + (size_t)30 * LEAN_COLS);
 }
+// fused VL kernel (hydro_lean_vl.cuh): plus cells within E = recon + 2 of the interior + one warp of boundary faces
+constexpr int VL_NT(int recon) { return 320 + 64 * (recon + 1) + 32; }
+// mbarriers | two primitive planes | W-half ring | LOX UPX LOY UPY FX FY | raw planes
+constexpr size_t vl_smem_bytes(size_t elem, int recon, int g) {
+  const size_t S = PS + 2 * g, SW = PS + 2 * (recon + 3), SH = PS + 2 * (recon + 2), NW = 2 * (1 + recon) + 1;
+  return 64 + elem * (2 * 5 * S * S + 2 * 5 * SW * SW + NW * 5 * SH * SH + (size_t)30 * LEAN_COLS);
+}
 constexpr bool lean_available(int precision_bytes, int scheme, int recon) {
   (void)precision_bytes; (void)recon;
-  return scheme == SCHEME_CTU || scheme == SCHEME_MHM;
+  return scheme == SCHEME_CTU || scheme == SCHEME_MHM || scheme == SCHEME_VL;
 }
 constexpr bool lean_fits(int precision_bytes, int scheme, int recon, int g) {
   return lean_available(precision_bytes, scheme, recon) &&
-         (scheme == SCHEME_MHM ? mhm_smem_bytes((size_t)precision_bytes, recon, g) : lean_smem_bytes((size_t)precision_bytes, recon, g)) <=
-             SMEM_MAX_OPTIN;
+         (scheme == SCHEME_MHM ? mhm_smem_bytes((size_t)precision_bytes, recon, g)
+          : scheme == SCHEME_VL ? vl_smem_bytes((size_t)precision_bytes, recon, g)
+                                : lean_smem_bytes((size_t)precision_bytes, recon, g)) <= SMEM_MAX_OPTIN;
 }
 
 template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_lean(const SolveArgs<R>& a);

@@ -1,9 +1,9 @@
-// hydro_lean.cuh -- dispatch of the lean fused kernels.  Variants without one return
-// cudaErrorNotSupported; the C ABI never reaches them because lean_available() gates the dispatch.
+// hydro_lean.cuh -- dispatch of the fused z-marching kernels (CTU, MHM, VL); lean_fits() gates it in the C ABI.
 #pragma once
 #include "hydro_launch.cuh"
 #include "hydro_lean_ctu.cuh"
 #include "hydro_lean_mhm.cuh"
+#include "hydro_lean_vl.cuh"
 
 namespace hydro {
 
@@ -22,8 +22,9 @@ template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_lean(const 
     if (fast) return launch_mhm_lean<R, RECON, RS, 1, MINB>(a);
     return launch_mhm_lean<R, RECON, RS, 0, MINB>(a);
   } else {
-    (void)a;
-    return cudaErrorNotSupported;
+    const bool fast = a.par.limiter == LIM_VANLEER && !a.par.char_limit && !(a.par.min_dens > R(0)) && !(a.par.min_pres > R(0));
+    if (fast) return launch_vl_lean<R, RECON, RS, 1>(a);
+    return launch_vl_lean<R, RECON, RS, 0>(a);
   }
 }
 
