@@ -291,3 +291,43 @@ def test_pipeline_matches_device_path(B, dtype):
     pipe.solve(hin, hout, hff, 0.1, 1.0, gamma, CTU, ROE, VANLEER, status=st)
     assert torch.equal(hout, dev_out.cpu()) and torch.equal(hff, dev_ff.cpu())
     pipe.close()
+
+
+# ---- config 3 at BASELINE.json's full size, in the launch configuration bench.py times ---------------
+# 8192 groups, g = 3, hydro_dt -> hydro_solve with dt formed on the device (max_speed + cfl), AUTO kernel choice,
+# face fluxes on.  Groups are independent, so sampled groups are compared element by element with the oracle; the
+# conservation balance that ties `out` to `face_flux` (P11) is checked on ALL groups.
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+def test_config3_full_size_sampled(B, oracle, nthreads, dtype):
+    import torch
+    Ng, g, gamma, dh, cfl = 8192, 3, 5.0 / 3.0, 1.0, 0.5
+    tdt = torch.float32 if dtype == np.float32 else torch.float64
+    u = wl.amr_batch(Ng, g=g, gamma=gamma, seed=0, dtype=np.dtype(dtype).name, device=torch.device("cuda"))
+    smax = torch.empty((), dtype=tdt, device="cuda")
+    status = torch.zeros(3, dtype=torch.int64, device="cuda")
+    B.hydro_dt(u, gamma, 0, max_speed=smax)
+    out, ff = B.hydro_solve(u, 0.0, dh, gamma, CTU, ROE, VANLEER, status=status, max_speed=smax, cfl=cfl)
+    torch.cuda.synchronize()
+    assert status.cpu().tolist() == [0, 0, 0]
+    # the whole-batch reduction against the oracle's (order-independent maximum)
+    rng = np.random.default_rng(7)
+    pick = np.sort(np.concatenate([[0, 1, 147, 148, 295, 296, Ng - 1], rng.choice(Ng, 25, replace=False)]))
+    Gs = u[torch.from_numpy(pick).cuda()].cpu().numpy()
+    s_gpu = dtype(smax.item())
+    s_ref = max(oracle.hydro_dt(u[k:k + 512].cpu().numpy(), gamma, 0) for k in range(0, Ng, 512))
+    assert abs(float(s_gpu) - s_ref) <= 4 * np.finfo(dtype).eps * s_ref
+    dt = float(dtype(cfl) / s_gpu)  # the kernel forms nu = cfl / max_speed in the working precision; dh = 1
+    ref_out, ref_ff, ref_st = oracle.hydro_solve(Gs, dt, dh, gamma, CTU, ROE, VANLEER, nthreads=nthreads)[:3]
+    idx = torch.from_numpy(pick).cuda()
+    check(out[idx].cpu().numpy(), ff[idx].cpu().numpy(), ref_out, ref_ff, dtype, ("config3 full size", np.dtype(dtype).name))
+    d = np.abs(out[idx].cpu().numpy().astype(np.float64) - ref_out).reshape(len(pick), -1).max(1)
+    assert d.max() <= (1e-4 if dtype == np.float32 else 1e-11) * np.abs(ref_out).max()
+    # P11 on every group: sum_interior(out - in) = -nu * (signed sum of the six outer flux planes)
+    o64, f64 = out.double(), ff.double()
+    uin = u[:, :, g:g + PS, g:g + PS, g:g + PS].double()
+    lhs = (o64 - uin).sum(dim=(2, 3, 4))
+    net = sum(f64[:, 3 * d + 2].sum(dim=(2, 3)) - f64[:, 3 * d + 0].sum(dim=(2, 3)) for d in range(3))
+    nu = float(dtype(cfl) / s_gpu) / dh
+    scale = uin.abs().sum(dim=(2, 3, 4)).max().item()
+    tol = (2e-6 if dtype == np.float32 else 1e-13) * scale
+    assert (lhs + nu * net).abs().max().item() <= tol
