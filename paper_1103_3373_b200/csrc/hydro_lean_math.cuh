@@ -183,7 +183,7 @@ __device__ __forceinline__ void lean_ppm_trace(const V5<R>& Wm2, const V5<R>& Wm
 
 // ---- c4: Roe's solver, primitive-jump form (normal frame in, normal-frame flux out) ------------
 // per-state quantities of a Riemann problem
-template <class R> struct LeanState { R ir, sq, H, m, F1, F2, F3, F4; };
+template <class R> struct LeanState { R ir, sq, H, m, F1; };  // the other flux components are m v, m w, m H
 template <class R> __device__ __forceinline__ LeanState<R> lean_state(const V5<R>& W, R g1) {
   LeanState<R> s;
   if (sizeof(R) == 4) {  // fp32: two SFU instructions are cheaper than the extra multiplies
@@ -198,9 +198,6 @@ template <class R> __device__ __forceinline__ LeanState<R> lean_state(const V5<R
   s.H = m_fma(R(0.5), q2, (g1 * W[4]) * s.ir);
   s.m = W[0] * W[1];
   s.F1 = m_fma(s.m, W[1], W[4]);
-  s.F2 = s.m * W[2];
-  s.F3 = s.m * W[3];
-  s.F4 = s.m * s.H;
   return s;
 }
 
@@ -253,9 +250,9 @@ template <class R> __device__ __forceinline__ bool lean_roe_core(const V5<R>& WL
   const R d4 = m_fma(w5, H5, m_fma(w4, wt, m_fma(w3, vt, m_fma(w2, hq, w1 * H1))));
   F[0] = R(0.5) * ((L.m + Rr.m) - d0);
   F[1] = R(0.5) * ((L.F1 + Rr.F1) - d1);
-  F[2] = R(0.5) * ((L.F2 + Rr.F2) - d2);
-  F[3] = R(0.5) * ((L.F3 + Rr.F3) - d3);
-  F[4] = R(0.5) * ((L.F4 + Rr.F4) - d4);
+  F[2] = R(0.5) * m_fma(L.m, WL[2], m_fma(Rr.m, WR[2], -d2));
+  F[3] = R(0.5) * m_fma(L.m, WL[3], m_fma(Rr.m, WR[3], -d3));
+  F[4] = R(0.5) * m_fma(L.m, L.H, m_fma(Rr.m, Rr.H, -d4));
   return ok;
 }
 // Roe failed at this face: count it and replace the flux by the fallback solver's
