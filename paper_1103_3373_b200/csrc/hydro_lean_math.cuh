@@ -28,10 +28,51 @@ __device__ __forceinline__ double m_rsqrt(double x) { return rsqrt(x); }  // <= 
 __device__ __forceinline__ float m_fma(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ double m_fma(double a, double b, double c) { return fma(a, b, c); }
 
+// Division-like operations of the lean path.  fp32: the SFU approximations of hydro_math.cuh.  fp64: an IEEE division
+// or square root is ~20 instructions with a branch to a slow path; the lean path instead refines the SFU's
+// 2^-23 seed (rcp.approx.ftz.f64 / rsqrt.approx.ftz.f64) with two Newton steps in FMAs: branch-free, <= 2 ulp,
+// far inside the fp64 parity budget.  Zero / denormal arguments give inf / NaN, which every
+// caller either discards by a select (limiter) or routes to the Roe failure test; -DHYDRO_F64_IEEE=1 restores
+// IEEE operations for A/B measurements.
+#ifndef HYDRO_F64_IEEE
+#define HYDRO_F64_IEEE 0
+#endif
+__device__ __forceinline__ float l_rcp(float x) { return m_rcp(x); }
+__device__ __forceinline__ float l_div(float a, float b) { return m_div(a, b); }
+__device__ __forceinline__ float l_sqrt(float x) { return m_sqrt(x); }
+__device__ __forceinline__ float l_rsqrt(float x) { return m_rsqrt(x); }
+#if HYDRO_F64_IEEE
+__device__ __forceinline__ double l_rcp(double x) { return 1.0 / x; }
+__device__ __forceinline__ double l_div(double a, double b) { return a / b; }
+__device__ __forceinline__ double l_sqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ double l_rsqrt(double x) { return rsqrt(x); }
+#else
+__device__ __forceinline__ double l_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  r = fma(r, fma(-x, r, 1.0), r);
+  return fma(r, fma(-x, r, 1.0), r);
+}
+__device__ __forceinline__ double l_div(double a, double b) {
+  const double r = l_rcp(b), q = a * r;
+  return fma(fma(-b, q, a), r, q);
+}
+__device__ __forceinline__ double l_rsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  y = fma(0.5 * y, fma(-x * y, y, 1.0), y);
+  return fma(0.5 * y, fma(-x * y, y, 1.0), y);
+}
+__device__ __forceinline__ double l_sqrt(double x) {
+  const double y = l_rsqrt(x), s = x * y;
+  return fma(fma(-s, s, x), 0.5 * y, s);
+}
+#endif
+
 // ---- c0: conversions --------------------------------------------------------------------------
 // rho |v|^2 is formed as m . v (3 instructions); `bad` counts non-positive rho / P (status[1])
 template <class R> __device__ __forceinline__ V5<R> lean_cons2prim(const V5<R>& U, const Par<R>& p, int& bad) {
-  const R ir = m_rcp(U[0]);
+  const R ir = l_rcp(U[0]);
   V5<R> W;
   W[0] = U[0];
   W[1] = U[1] * ir;
@@ -58,7 +99,7 @@ template <class R> __device__ __forceinline__ V5<R> lean_correct(const V5<R>& W,
 // ---- c1-c3: PLM + van Leer limiter on primitive variables + CTU tracing (normal frame) ---------
 template <class R> __device__ __forceinline__ R vl_slope(R dL, R dR) {
   const R prod = dL * dR;
-  const R s = m_div(prod + prod, dL + dR);
+  const R s = l_div(prod + prod, dL + dR);
   return prod > R(0) ? s : R(0);  // S19; the select also discards inf/NaN of the unused quotient
 }
 
@@ -70,7 +111,7 @@ __device__ __forceinline__ void lean_plm_trace(const V5<R>& Wm, const V5<R>& W0,
   for (int q = 0; q < 5; ++q) s[q] = vl_slope(W0[q] - Wm[q], Wp[q] - W0[q]);
   // eigen-system scalars from one rsqrt: irc = 1/(rho c), c = gamma P irc, 1/c = rho irc
   const R gP = p.gamma * W0[4], x = gP * W0[0];
-  const R irc = m_rsqrt(x);
+  const R irc = l_rsqrt(x);
   const R c = gP * irc, ic = W0[0] * irc, ic2 = ic * ic, rc = x * irc;
   const R u = W0[1], lamM = u + c, lam0 = u - c;
   const R nc = nu * c, hnc = R(0.5) * nc;
@@ -138,7 +179,7 @@ __device__ __forceinline__ void lean_ppm_trace(const V5<R>& Wm2, const V5<R>& Wm
     W6[q] = R(6) * m_fma(R(-0.5), WL[q] + WR[q], W0[q]);
   }
   const R gP = p.gamma * W0[4], x = gP * W0[0];
-  const R irc = m_rsqrt(x);
+  const R irc = l_rsqrt(x);
   const R c = gP * irc, ic = W0[0] * irc, ic2 = ic * ic, rc = x * irc;
   const R u = W0[1], lamM = u + c, lam0 = u - c;
   const R nc = nu * c, n23 = nu * nu * R(1.0 / 3.0), uc = u * c, c2 = c * c;
@@ -187,10 +228,10 @@ template <class R> struct LeanState { R ir, sq, H, m, F1; };  // the other flux 
 template <class R> __device__ __forceinline__ LeanState<R> lean_state(const V5<R>& W, R g1) {
   LeanState<R> s;
   if (sizeof(R) == 4) {  // fp32: two SFU instructions are cheaper than the extra multiplies
-    s.ir = m_rcp(W[0]);
-    s.sq = m_sqrt(W[0]);
+    s.ir = l_rcp(W[0]);
+    s.sq = l_sqrt(W[0]);
   } else {               // fp64: one rsqrt instead of a division and a square root
-    const R is = m_rsqrt(W[0]);
+    const R is = l_rsqrt(W[0]);
     s.ir = is * is;
     s.sq = W[0] * is;
   }
@@ -216,7 +257,7 @@ template <class R> __device__ __forceinline__ bool lean_roe_core(const V5<R>& WL
   const R g1 = p.gamma * p.igm1;
   const LeanState<R> L = lean_state(WL, g1), Rr = lean_state(WR, g1);
   // Roe averages with weights wL = sqrt(rhoL)/(sqrt(rhoL)+sqrt(rhoR)), wR = 1 - wL; rho~ = sqrt(rhoL rhoR)
-  const R wR = Rr.sq * m_rcp(L.sq + Rr.sq);
+  const R wR = Rr.sq * l_rcp(L.sq + Rr.sq);
   const R rt = L.sq * Rr.sq;
   const R du = WR[1] - WL[1], dv = WR[2] - WL[2], dw = WR[3] - WL[3];
   const R ut = m_fma(wR, du, WL[1]), vt = m_fma(wR, dv, WL[2]), wt = m_fma(wR, dw, WL[3]);
@@ -224,8 +265,8 @@ template <class R> __device__ __forceinline__ bool lean_roe_core(const V5<R>& WL
   const R hq = R(0.5) * m_fma(wt, wt, m_fma(vt, vt, ut * ut));
   const R a2 = p.gm1 * (Ht - hq);
   R a, ia2;
-  if (sizeof(R) == 4) { a = m_sqrt(a2); ia2 = m_rcp(a2); }
-  else { const R ia = m_rsqrt(a2); a = a2 * ia; ia2 = ia * ia; }
+  if (sizeof(R) == 4) { a = l_sqrt(a2); ia2 = l_rcp(a2); }
+  else { const R ia = l_rsqrt(a2); a = a2 * ia; ia2 = ia * ia; }
   // wave strengths from the primitive jumps
   const R dp = WR[4] - WL[4], dr = WR[0] - WL[0];
   const R y = (rt * a) * du, h = R(0.5) * ia2;
@@ -272,16 +313,16 @@ template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, co
 // ---- c4: HLLC, Toro's pressure-based speeds (S9), select form ----------------------------------
 template <class R> __device__ __forceinline__ V5<R> lean_hllc(const V5<R>& WL, const V5<R>& WR, const Par<R>& p) {
   const R g = p.gamma;
-  const R irL = m_rcp(WL[0]), irR = m_rcp(WR[0]);
-  const R cL = m_sqrt(g * WL[4] * irL), cR = m_sqrt(g * WR[4] * irR);
+  const R irL = l_rcp(WL[0]), irR = l_rcp(WR[0]);
+  const R cL = l_sqrt(g * WL[4] * irL), cR = l_sqrt(g * WR[4] * irR);
   const R ppv = R(0.5) * (WL[4] + WR[4]) - R(0.125) * (WR[1] - WL[1]) * (WL[0] + WR[0]) * (cL + cR);
   const R ps = m_max(R(0), ppv);
-  const R gf = (g + R(1)) * (R(0.5) * m_rcp(g));
-  const R qL = (ps <= WL[4]) ? R(1) : m_sqrt(m_fma(gf, m_div(ps, WL[4]) - R(1), R(1)));
-  const R qR = (ps <= WR[4]) ? R(1) : m_sqrt(m_fma(gf, m_div(ps, WR[4]) - R(1), R(1)));
+  const R gf = (g + R(1)) * (R(0.5) * l_rcp(g));
+  const R qL = (ps <= WL[4]) ? R(1) : l_sqrt(m_fma(gf, l_div(ps, WL[4]) - R(1), R(1)));
+  const R qR = (ps <= WR[4]) ? R(1) : l_sqrt(m_fma(gf, l_div(ps, WR[4]) - R(1), R(1)));
   const R SL = m_fma(-cL, qL, WL[1]), SR = m_fma(cR, qR, WR[1]);
   const R mL = WL[0] * (SL - WL[1]), mR = WR[0] * (SR - WR[1]);
-  const R Ss = m_div((WR[4] - WL[4]) + WL[1] * mL - WR[1] * mR, mL - mR);
+  const R Ss = l_div((WR[4] - WL[4]) + WL[1] * mL - WR[1] * mR, mL - mR);
   // F_L if S_L >= 0, F_R if S_R <= 0, else the star state on the side of the contact (S19: S* = 0 -> left)
   const bool supL = SL >= R(0), supR = SR <= R(0);
   const bool left = supL || (!supR && Ss >= R(0));
@@ -295,13 +336,13 @@ template <class R> __device__ __forceinline__ V5<R> lean_hllc(const V5<R>& WL, c
   V5<R> U, F;
   U[0] = rK; U[1] = mom; U[2] = rK * vK; U[3] = rK * wK; U[4] = E;
   F[0] = mom; F[1] = m_fma(mom, uK, pK); F[2] = mom * vK; F[3] = mom * wK; F[4] = (E + pK) * uK;
-  const R f = m_div(mK, SK - Ss);
+  const R f = l_div(mK, SK - Ss);
   V5<R> Us;
   Us[0] = f;
   Us[1] = f * Ss;
   Us[2] = f * vK;
   Us[3] = f * wK;
-  Us[4] = f * (m_div(E, rK) + (Ss - uK) * (Ss + m_div(pK, mK)));
+  Us[4] = f * (l_div(E, rK) + (Ss - uK) * (Ss + l_div(pK, mK)));
 #pragma unroll
   for (int q = 0; q < 5; ++q) F[q] = star ? m_fma(SK, Us[q] - U[q], F[q]) : F[q];
   return F;
