@@ -60,6 +60,7 @@ template <class R, int RECON, int RS, int FAST> struct LeanOps {
     const V5<R> l = to_normal<D>(WL), r = to_normal<D>(WR);
     if (FAST && RS == RS_ROE) return from_normal<D>(lean_roe(l, r, p, c));
     if (FAST && RS == RS_HLLC) return from_normal<D>(lean_hllc(l, r, p));
+    if (FAST && RS == RS_EXACT) return from_normal<D>(lean_exact(l, r, p, c));
     return from_normal<D>(riemann_n<RS>(l, r, p, c));
   }
 };

@@ -310,6 +310,108 @@ template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, co
   return F;
 }
 
+// ---- c4: exact solver (Toro ch. 4; S11), same iteration and sampling as hydro_math.cuh `exact` with the per-side
+// constants hoisted out of the Newton loop and ONE pow per rarefaction evaluation: with z = (p/P_K)^((g-1)/(2g)),
+// the derivative's (p/P_K)^(-(g+1)/(2g)) is z P_K / p, the star sound speed is c_K z, the star density behind the
+// tail is rho_K (p/P_K) / z^2, and inside the fan phi^(2g/(g-1)) = phi^2 phi^(2/(g-1)).
+template <class R> struct ExactSide { R rho, u, P, c, iP, A, B, k, irc; };
+template <class R> __device__ __forceinline__ ExactSide<R> exact_side(const V5<R>& W, const Par<R>& p) {
+  ExactSide<R> s;
+  const R g = p.gamma, ig1 = l_rcp(g + R(1));
+  s.rho = W[0]; s.u = W[1]; s.P = W[4];
+  const R ir = l_rcp(W[0]);
+  s.c = l_sqrt(g * W[4] * ir);
+  s.iP = l_rcp(W[4]);
+  s.A = (ig1 + ig1) * ir;             // 2 / ((g+1) rho)
+  s.B = p.gm1 * ig1 * W[4];           // (g-1)/(g+1) P
+  s.k = (s.c + s.c) * p.igm1;         // 2 c / (g-1)
+  s.irc = ir * l_rcp(s.c);            // 1 / (rho c)
+  return s;
+}
+// f_K(p), f_K'(p) and, on the rarefaction branch, z = (p/P_K)^e1 (else 0)
+template <class R> __device__ __forceinline__ void exact_fn(R ps, R ips, const ExactSide<R>& s, R e1, R& f, R& df, R& z) {
+  if (ps > s.P) {
+    const R t = l_rcp(ps + s.B), q = l_sqrt(s.A * t), d = ps - s.P;
+    f = d * q;
+    df = q * m_fma(R(-0.5) * d, t, R(1));
+    z = R(0);
+  } else {
+    z = m_pow(ps * s.iP, e1);
+    f = s.k * (z - R(1));
+    df = (z * s.P * ips) * s.irc;
+  }
+}
+template <class R> __device__ __noinline__ void lean_exact_impl(const V5<R>* pWL, const V5<R>* pWR, const Par<R>* pp, int* cnt, V5<R>* pF) {
+  const V5<R>& WL = *pWL; const V5<R>& WR = *pWR; const Par<R>& p = *pp;
+  const R g = p.gamma;
+  const ExactSide<R> L = exact_side(WL, p), Rs = exact_side(WR, p);
+  const R du = Rs.u - L.u;
+  if ((L.k + Rs.k) <= du) {  // vacuum generation -> HLLE flux (S11)
+    *cnt += 1;
+    *pF = hlle(WL, WR, p);
+    return;
+  }
+  const R e1 = p.gm1 * (R(0.5) * l_rcp(g));
+  const R epsp = R(1e-6) * m_min(L.P, Rs.P);
+  const R ppv = R(0.5) * (L.P + Rs.P) - R(0.125) * du * (L.rho + Rs.rho) * (L.c + Rs.c);
+  R ps = m_max(epsp, ppv), fL, dL, zL, fR, dR, zR;
+  bool conv = false;
+  for (int it = 0; it < 40; ++it) {
+    const R ips = l_rcp(ps);
+    exact_fn(ps, ips, L, e1, fL, dL, zL);
+    exact_fn(ps, ips, Rs, e1, fR, dR, zR);
+    R pn = ps - l_div((fL + fR) + du, dL + dR);
+    if (!(pn > R(0))) pn = epsp;
+    const R chg = l_div(R(2) * m_abs(pn - ps), pn + ps);
+    ps = pn;
+    if (chg < ExactTol<R>::v()) { conv = true; break; }
+  }
+  if (!conv) *cnt += 1;
+  {
+    const R ips = l_rcp(ps);
+    exact_fn(ps, ips, L, e1, fL, dL, zL);
+    exact_fn(ps, ips, Rs, e1, fR, dR, zR);
+  }
+  const R us = R(0.5) * (L.u + Rs.u) + R(0.5) * (fR - fL);
+  // sample at x/t = 0 on the side of the contact given by sign(u*) (S19: u* = 0 -> left); right side mirrored
+  const bool left = us >= R(0);
+  const R sg = left ? R(1) : R(-1);
+  const R rK = left ? L.rho : Rs.rho, PK = left ? L.P : Rs.P, cK = left ? L.c : Rs.c, vK = left ? L.u : Rs.u;
+  const R iPK = left ? L.iP : Rs.iP, zK = left ? zL : zR;
+  const R ig1 = l_rcp(g + R(1)), mu = p.gm1 * ig1, pr = ps * iPK;
+  V5<R> W;
+  W[2] = left ? WL[2] : WR[2];
+  W[3] = left ? WL[3] : WR[3];
+  if (ps > PK) {  // shock
+    const R ig2 = R(0.5) * l_rcp(g);
+    const R S = vK - sg * cK * l_sqrt(m_fma((g + R(1)) * ig2, pr, p.gm1 * ig2));
+    const bool undisturbed = left ? (S >= R(0)) : (S <= R(0));
+    if (undisturbed) { W[0] = rK; W[1] = vK; W[4] = PK; }
+    else { W[0] = l_div(rK * (pr + mu), m_fma(mu, pr, R(1))); W[1] = us; W[4] = ps; }
+  } else {  // rarefaction
+    const R head = vK - sg * cK, tail = us - sg * (cK * zK);
+    const bool before_head = left ? (head >= R(0)) : (head <= R(0));
+    const bool behind_tail = left ? (tail <= R(0)) : (tail >= R(0));
+    if (before_head) { W[0] = rK; W[1] = vK; W[4] = PK; }
+    else if (behind_tail) { W[0] = l_div(rK * pr, zK * zK); W[1] = us; W[4] = ps; }
+    else {
+      const R phi = (ig1 + ig1) + l_div(sg * mu * vK, cK);
+      const R w = m_pow(phi, R(2) * p.igm1);
+      W[0] = rK * w;
+      W[1] = (ig1 + ig1) * (sg * cK + R(0.5) * p.gm1 * vK);
+      W[4] = PK * (phi * phi) * w;
+    }
+  }
+  *pF = phys_flux(W, p);
+}
+template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
+  V5<R> F, l = WL, r = WR;
+  int ex = 0;
+  lean_exact_impl(&l, &r, &p, &ex, &F);
+  c.exact += ex;
+  return F;
+}
+
 // ---- c4: HLLC, Toro's pressure-based speeds (S9), select form ----------------------------------
 template <class R> __device__ __forceinline__ V5<R> lean_hllc(const V5<R>& WL, const V5<R>& WR, const Par<R>& p) {
   const R g = p.gamma;
