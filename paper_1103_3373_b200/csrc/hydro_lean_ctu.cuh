@@ -61,6 +61,7 @@ template <class R, int RECON, int RS, int FAST> struct LeanOps {
     if (FAST && RS == RS_ROE) return from_normal<D>(lean_roe(l, r, p, c));
     if (FAST && RS == RS_HLLC) return from_normal<D>(lean_hllc(l, r, p));
     if (FAST && RS == RS_EXACT) return from_normal<D>(lean_exact(l, r, p, c));
+    if (FAST && RS == RS_HLLE) return from_normal<D>(lean_hlle(l, r, p));
     return from_normal<D>(riemann_n<RS>(l, r, p, c));
   }
 };

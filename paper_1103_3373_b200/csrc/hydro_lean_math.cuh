@@ -310,6 +310,28 @@ template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, co
   return F;
 }
 
+// ---- c4: HLLE (Einfeldt 1991; S9: Roe-average and local signal speeds), normal frame
+template <class R> __device__ __forceinline__ V5<R> lean_hlle(const V5<R>& WL, const V5<R>& WR, const Par<R>& p) {
+  const R g1 = p.gamma * p.igm1;
+  const LeanState<R> L = lean_state(WL, g1), Rr = lean_state(WR, g1);
+  const R wR = Rr.sq * l_rcp(L.sq + Rr.sq);
+  const R ut = m_fma(wR, WR[1] - WL[1], WL[1]), vt = m_fma(wR, WR[2] - WL[2], WL[2]), wt = m_fma(wR, WR[3] - WL[3], WL[3]);
+  const R Ht = m_fma(wR, Rr.H - L.H, L.H);
+  const R a = l_sqrt(p.gm1 * m_fma(R(-0.5), m_fma(wt, wt, m_fma(vt, vt, ut * ut)), Ht));
+  const R cL = l_sqrt(p.gamma * WL[4] * L.ir), cR = l_sqrt(p.gamma * WR[4] * Rr.ir);
+  const R bm = m_min(m_min(ut - a, WL[1] - cL), R(0)), bp = m_max(m_max(ut + a, WR[1] + cR), R(0));
+  const R iw = l_rcp(bp - bm), bb = bp * bm;
+  // U = (rho, m, rho v, rho w, rho H - P),  F = (m, m u + P, m v, m w, m H)
+  V5<R> F;
+  F[0] = (m_fma(bp, L.m, -bm * Rr.m) + bb * (WR[0] - WL[0])) * iw;
+  F[1] = (m_fma(bp, L.F1, -bm * Rr.F1) + bb * (Rr.m - L.m)) * iw;
+  F[2] = (m_fma(bp, L.m * WL[2], -bm * (Rr.m * WR[2])) + bb * m_fma(WR[0], WR[2], -WL[0] * WL[2])) * iw;
+  F[3] = (m_fma(bp, L.m * WL[3], -bm * (Rr.m * WR[3])) + bb * m_fma(WR[0], WR[3], -WL[0] * WL[3])) * iw;
+  const R EL = m_fma(WL[0], L.H, -WL[4]), ER = m_fma(WR[0], Rr.H, -WR[4]);
+  F[4] = (m_fma(bp, L.m * L.H, -bm * (Rr.m * Rr.H)) + bb * (ER - EL)) * iw;
+  return F;
+}
+
 // ---- c4: exact solver (Toro ch. 4; S11), same iteration and sampling as hydro_math.cuh `exact` with the per-side
 // constants hoisted out of the Newton loop and ONE pow per rarefaction evaluation: with z = (p/P_K)^((g-1)/(2g)),
 // the derivative's (p/P_K)^(-(g+1)/(2g)) is z P_K / p, the star sound speed is c_K z, the star density behind the
