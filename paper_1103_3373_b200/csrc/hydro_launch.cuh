@@ -40,10 +40,13 @@ constexpr int FUSED_COLS = (PS + 2) * (PS + 2);     // 18 x 18 columns: interior
 // two co-resident CTAs per SM where the tiles allow ------------------------------------------------------------
 constexpr int LEAN_NT = 320;                        // 10 warps: 288 columns of the rows j = 0..15, 32 of the rows j = -1, 16
 constexpr int LEAN_COLS = FUSED_COLS;
-// mbarriers | raw planes [2][5][S*S] | W ring | private z states [2][2][5][NT] | LOX UPX LOY UPY FX FY [6][5][324]
+// PPM tiles are trimmed (one raw landing plane; the oldest z-pencil plane carried in registers) so that two fp32 CTAs fit
+constexpr int LEAN_NRAW(int recon) { return recon == RECON_PPM ? 1 : 2; }
+constexpr int LEAN_RING_CARRY(int recon) { return recon == RECON_PPM ? 1 : 0; }
+// mbarriers | W ring | private z states [2][2][5][NT] | LOX UPX LOY UPY FX FY [6][5][324] | raw planes [NRAW][5][S*S]
 constexpr size_t lean_smem_bytes(size_t elem, int recon, int g) {
-  const size_t S = PS + 2 * g, SWP = PS + 2 * (2 + recon), NW = 2 * (1 + recon) + 1;
-  return 64 + elem * (2 * 5 * S * S + NW * 5 * SWP * SWP + (size_t)20 * LEAN_NT + (size_t)30 * LEAN_COLS);
+  const size_t S = PS + 2 * g, SWP = PS + 2 * (2 + recon), NWS = 2 * (1 + recon) + 1 - LEAN_RING_CARRY(recon);
+  return 64 + elem * (LEAN_NRAW(recon) * 5 * S * S + NWS * 5 * SWP * SWP + (size_t)20 * LEAN_NT + (size_t)30 * LEAN_COLS);
 }
 // fused MHM kernel (hydro_lean_mhm.cuh): mbarriers | raw planes | W ring | LOX UPX LOY UPY FX FY
 constexpr size_t mhm_smem_bytes(size_t elem, int recon, int g) {

@@ -7,8 +7,8 @@
 
 namespace hydro {
 
-// co-resident CTAs per SM the register budget is set for: two where the tiles of two groups fit (fp32, PLM)
-template <class R, int RECON> struct LeanTune { static constexpr int MINB = (sizeof(R) == 4 && RECON == RECON_PLM) ? 2 : 1; };
+// co-resident CTAs per SM the register budget is set for: two where the tiles of two groups fit (fp32)
+template <class R, int RECON> struct LeanTune { static constexpr int MINB = sizeof(R) == 4 ? 2 : 1; };
 
 template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_lean(const SolveArgs<R>& a) {
   if constexpr (SCHEME == SCHEME_CTU) {

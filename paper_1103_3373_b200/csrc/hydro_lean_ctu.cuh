@@ -72,6 +72,9 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
                 const R* __restrict__ max_speed, R cfl, long long* status) {
   using Op = LeanOps<R, RECON, RS, FAST>;
   constexpr int GW = 2 + RECON, RW = 1 + RECON, SWP = PS + 2 * GW, WPL = SWP * SWP, NW = 2 * RW + 1, NPL = PS + 2 * GW;
+  // PPM tiles are trimmed so that two fp32 CTAs (or one fp64 CTA) fit: one raw landing plane instead of two, and the
+  // oldest plane of the z pencil (needed only at the thread's own column) carried in registers instead of the ring
+  constexpr int NRAW = RECON == RECON_PPM ? 1 : 2, RC = RECON == RECON_PPM ? 1 : 0, NWS = NW - RC;  // == LEAN_NRAW, LEAN_RING_CARRY
   constexpr int NC = LEAN_COLS, NT = LEAN_NT, FT = PS + 2;
   apply_device_dt(p, max_speed, cfl);
 
@@ -83,8 +86,8 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   // shared memory: everything at compile-time offsets; the raw planes, whose size depends on g, come last
   extern __shared__ __align__(16) unsigned char smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
-  R* ring = reinterpret_cast<R*>(smem + 64);           // [NW] fields of WPL cells: primitive planes
-  R* zs = ring + NW * 5 * WPL;                         // [2][2] fields of NT cells: private traced z states (lo, up) of planes t, t+1
+  R* ring = reinterpret_cast<R*>(smem + 64);           // [NWS] fields of WPL cells: primitive planes
+  R* zs = ring + NWS * 5 * WPL;                        // [2][2] fields of NT cells: private traced z states (lo, up) of planes t, t+1
   R* xy = zs + 4 * 5 * NT;                             // [6] fields of NC cells: LOX UPX LOY UPY FX FY
   R* raw = xy + 6 * 5 * NC;                            // [2][5][SS] landing zone of the bulk copies (SoA as in HBM)
   auto fld = [&](int k) { return xy + k * 5 * NC; };
@@ -118,8 +121,8 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     const int m = n / NPL, pl = n - m * NPL;
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
     const R* src = in + grp * 5 * nS + (size_t)(pl + off) * SS;
-    uint64_t* b = bar + (n & 1);
-    R* dst = raw + (size_t)(n & 1) * 5 * SS;
+    uint64_t* b = bar + (n % NRAW);
+    R* dst = raw + (size_t)(n % NRAW) * 5 * SS;
     mbar_expect_tx(b, (uint32_t)(5 * SS * sizeof(R)));
 #pragma unroll
     for (int q = 0; q < 5; ++q) bulk_g2s(dst + (size_t)q * SS, src + q * nS, (uint32_t)(SS * sizeof(R)), b);
@@ -131,14 +134,14 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     fence_async_smem();
   }
   __syncthreads();
-  if (tid == 0) { issue(0); issue(1); }
+  if (tid == 0) { issue(0); if (NRAW > 1) issue(1); }
 
   Cnt c = {0, 0, 0};
   int nseq = 0;  // planes converted so far
   // con->prim of the next raw plane into ring slot `slot` (all threads)
   auto convert = [&](int slot) {
-    const int st = nseq & 1;
-    mbar_wait(bar + st, (uint32_t)((nseq >> 1) & 1));
+    const int st = nseq % NRAW;
+    mbar_wait(bar + st, (uint32_t)((nseq / NRAW) & 1));
     const R* rp = raw + (size_t)st * 5 * SS;
     R* wp = ring + slot * 5 * WPL;
     for (int idx = tid; idx < WPL; idx += NT) {
@@ -148,7 +151,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   };
   // after the barrier that follows a conversion: refill the raw stage it consumed
   auto refill = [&]() {
-    if (tid == 0) { fence_async_smem(); issue(nseq + 2); }
+    if (tid == 0) { fence_async_smem(); issue(nseq + NRAW); }
     ++nseq;
   };
   // traced states of a corner column of primitive plane `wpl` along x (cdir 0) or y (cdir 1)
@@ -183,12 +186,20 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     const R* gin0 = in + grp * 5 * nS + ((size_t)g * S + (jj - 1 + g)) * S + (ii - 1 + g);
     R* gout0 = out + grp * 5 * PS * PS * PS + (jj - 1) * PS + (ii - 1);
     // ---- prologue: the first NW primitive planes (-GW .. -GW+NW-1)
-    for (int k = 0; k < NW; ++k) {
+    V5<R> Wold;  // RC: W(t+1-RW) at the thread's own column
+    if (RC) {
+      convert(0);
+      __syncthreads();
+      refill();
+      Wold = ldv(ring, WPL, wb);
+      __syncthreads();
+    }
+    for (int k = 0; k < NWS; ++k) {
       convert(k);
       __syncthreads();
       refill();
     }
-    int sl = 0;  // ring slot of plane t+1-RW (the oldest plane held)
+    int sl = 0;  // ring slot of the oldest plane held in shared memory: plane t+1-RW+RC
 
 #pragma unroll 1
     for (int t = -2; t <= PS; ++t) {
@@ -197,7 +208,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
       // ring slots of the planes this step touches
       int slot[NW];
 #pragma unroll
-      for (int s = 0; s < NW; ++s) slot[s] = (sl + s < NW) ? sl + s : sl + s - NW;
+      for (int s = RC; s < NW; ++s) slot[s] = (sl + s - RC < NWS) ? sl + s - RC : sl + s - RC - NWS;
       // ================= B: z states of plane t+1, F*_z(t+1) =================
       V5<R> dFz;
 #pragma unroll
@@ -205,7 +216,11 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
       if (t < PS) {
         V5<R> Wz[NW];
 #pragma unroll
-        for (int s = 0; s < NW; ++s) Wz[s] = to_normal<2>(ldv(ring + slot[s] * 5 * WPL, WPL, wb));
+        for (int s = RC; s < NW; ++s) {
+          const V5<R> w = ldv(ring + slot[s] * 5 * WPL, WPL, wb);
+          if (RC && s == RC) { Wz[0] = to_normal<2>(Wold); Wold = w; }
+          Wz[s] = to_normal<2>(w);
+        }
         V5<R> l, u;
         Op::recon(Wz[0], Wz[RW - 1], Wz[RW], Wz[RW + 1], Wz[2 * RW], p, l, u);
         const V5<R> lz = from_normal<2>(l), uz = from_normal<2>(u);
@@ -252,7 +267,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
           stv(fld(LF_FY), NC, fyc, Op::template riemann<1>(ldv(fld(LF_UPY), NC, fyc - FT), ldv(fld(LF_LOY), NC, fyc), p, c));
       }
       const bool conv = t + 2 + RW <= PS - 1 + GW;  // plane t+2+RW replaces plane t+1-RW (read for the last time in B / C)
-      if (conv) convert(sl);
+      if (conv) convert(sl);  // the oldest shared-memory plane: last read in B / C of this step
       __syncthreads();  // barrier 2
       if (conv) refill();
 
@@ -342,7 +357,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
 #pragma unroll
         for (int q = 0; q < 5; ++q) Dz[q] = ((x1[q] - x0[q]) + (y1[q] - y0[q])) - Dz[q];
       }
-      sl = (sl + 1 < NW) ? sl + 1 : 0;
+      sl = (sl + 1 < NWS) ? sl + 1 : 0;
     }
   }
   flush_counters(c, status);
