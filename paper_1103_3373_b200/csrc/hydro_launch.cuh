@@ -55,10 +55,10 @@ constexpr size_t mhm_smem_bytes(size_t elem, int recon, int g) {
 }
 // fused VL kernel (hydro_lean_vl.cuh): plus cells within E = recon + 2 of the interior + one warp of boundary faces
 constexpr int VL_NT(int recon) { return 320 + 64 * (recon + 1) + 32; }
-// mbarriers | two primitive planes | W-half ring | LOX UPX LOY UPY FX FY | raw planes
+// mbarriers | one primitive plane | W-half ring | LOX UPX LOY UPY FX FY | one raw plane
 constexpr size_t vl_smem_bytes(size_t elem, int recon, int g) {
   const size_t S = PS + 2 * g, SW = PS + 2 * (recon + 3), SH = PS + 2 * (recon + 2), NW = 2 * (1 + recon) + 1;
-  return 64 + elem * (2 * 5 * S * S + 2 * 5 * SW * SW + NW * 5 * SH * SH + (size_t)30 * LEAN_COLS);
+  return 64 + elem * (5 * S * S + 5 * SW * SW + NW * 5 * SH * SH + (size_t)30 * LEAN_COLS);
 }
 constexpr bool lean_available(int precision_bytes, int scheme, int recon) {
   (void)precision_bytes; (void)recon;

@@ -43,10 +43,10 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
 
   extern __shared__ __align__(16) unsigned char smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
-  R* wpl = reinterpret_cast<R*>(smem + 64);            // [2] fields of WPL cells: primitive plane a in buffer (a + E) & 1
-  R* hring = wpl + 2 * 5 * WPL;                        // [NW] fields of HPL cells: W-half planes b-RW .. b+RW
+  R* wpl = reinterpret_cast<R*>(smem + 64);            // one field of WPL cells: primitive plane a (W(a-1) lives in registers)
+  R* hring = wpl + 5 * WPL;                       // [NW] fields of HPL cells: W-half planes b-RW .. b+RW
   R* xy = hring + NW * 5 * HPL;                        // [6] fields of NC cells: LOX UPX LOY UPY FX FY
-  R* raw = xy + 6 * 5 * NC;                            // [2][5][SS]
+  R* raw = xy + 6 * 5 * NC;                            // [5][SS] one landing plane: a step is long against a plane load
   R* f1x = xy;                                         // first-pass fluxes alias LOX.. (FPL cells each)
   R* f1y = xy + 5 * FPL;
   auto fld = [&](int k) { return xy + k * 5 * NC; };
@@ -78,8 +78,8 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     const int m = n / NPL, pl = n - m * NPL;
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
     const R* src = in + grp * 5 * nS + (size_t)(pl + off) * SS;
-    uint64_t* b = bar + (n & 1);
-    R* dst = raw + (size_t)(n & 1) * 5 * SS;
+    uint64_t* b = bar;
+    R* dst = raw;
     mbar_expect_tx(b, (uint32_t)(5 * SS * sizeof(R)));
 #pragma unroll
     for (int q = 0; q < 5; ++q) bulk_g2s(dst + (size_t)q * SS, src + q * nS, (uint32_t)(SS * sizeof(R)), b);
@@ -91,22 +91,21 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     fence_async_smem();
   }
   __syncthreads();
-  if (tid == 0) { issue(0); issue(1); }
+  if (tid == 0) issue(0);
 
   Cnt c = {0, 0, 0};
   int nseq = 0;
-  auto convert = [&](int buf) {
-    const int st = nseq & 1;
-    mbar_wait(bar + st, (uint32_t)((nseq >> 1) & 1));
-    const R* rp = raw + (size_t)st * 5 * SS;
-    R* wp = wpl + buf * 5 * WPL;
+  auto convert = [&]() {
+    mbar_wait(bar, (uint32_t)(nseq & 1));
+    const R* rp = raw;
+    R* wp = wpl;
     for (int idx = tid; idx < WPL; idx += NT) {
       const int b = idx / SW, a = idx - b * SW;
       stv(wp, WPL, idx, Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c));
     }
   };
   auto refill = [&]() {
-    if (tid == 0) { fence_async_smem(); issue(nseq + 2); }
+    if (tid == 0) { fence_async_smem(); issue(nseq + 1); }
     ++nseq;
   };
 
@@ -120,12 +119,12 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     R* gout0 = out + grp * 5 * PS * PS * PS + cj * PS + ci;
     R* gff = face_flux ? face_flux + grp * 9 * 5 * PS * PS : nullptr;
     // ---- prologue: plane -GW (only its own-column values are needed, as W(a-1) of the first step), then plane -E
-    convert(1);
+    convert();
     __syncthreads();
     refill();
-    if (c_int) Wprev = ldv(wpl + 5 * WPL, WPL, wb);
+    if (c_int) Wprev = ldv(wpl, WPL, wb);
     __syncthreads();
-    convert(0);
+    convert();
     __syncthreads();
     refill();
 
@@ -133,7 +132,7 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     for (int a = -E; a <= PS + E; ++a) {
       const bool a_in = a >= 0 && a < PS;          // plane a holds arm cells
       const bool a_xy = a < PS + E;                // plane a needs its in-plane first-pass fluxes
-      const R* wa = wpl + ((a + E) & 1) * 5 * WPL;
+      const R* wa = wpl;
       // arm cells (outside the interior columns) live in planes 0..15 only, but need W(-1) and F1_z at faces 0 and 16
       const bool act1 = cell && (c_int || (a >= -1 && a <= PS));
       const bool zf = cell && (c_int || (a >= 0 && a <= PS));
@@ -254,7 +253,7 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
         }
       }
       const bool conv = a + 1 <= PS - 1 + GW;
-      if (conv) convert((a + 1 + E) & 1);
+      if (conv) convert();  // plane a+1 replaces plane a, read for the last time in S1
       __syncthreads();  // barrier 4
       if (conv) refill();
 
