@@ -331,3 +331,34 @@ def test_config3_full_size_sampled(B, oracle, nthreads, dtype):
     scale = uin.abs().sum(dim=(2, 3, 4)).max().item()
     tol = (2e-6 if dtype == np.float32 else 1e-13) * scale
     assert (lhs + nu * net).abs().max().item() <= tol
+
+
+# ---- the other schemes / reconstructions / solvers on a batch that fills the persistent grid many times over -------
+# (the kernels of configs 4 and 5: MHM, VL, PPM, HLLC, exact), sampled groups against the oracle, flux balance on all.
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+@pytest.mark.parametrize("scheme,recon,riemann", ((MHM, PLM, HLLC), (MHM, PPM, ROE), (VL, PLM, ROE), (VL, PPM, HLLC),
+                                                  (CTU, PPM, EXACT), (CTU, PPM, ROE)))
+def test_large_batch_sampled_variants(B, oracle, nthreads, dtype, scheme, recon, riemann):
+    import torch
+    Ng, gamma, dh = 2048, 5.0 / 3.0, 1.0
+    g = oracle.min_ghost(scheme, recon)
+    tdt = torch.float32 if dtype == np.float32 else torch.float64
+    assert B.hydro_fused_fits(tdt, scheme, recon, g)
+    u = wl.amr_batch(Ng, g=g, gamma=gamma, seed=5, dtype=np.dtype(dtype).name, device=torch.device("cuda"))
+    status = torch.zeros(3, dtype=torch.int64, device="cuda")
+    dt = 0.3 * dh / float(B.hydro_dt(u, gamma, 0).item())  # CFL 0.3: stable for MHM and VL too (S15)
+    out, ff = B.hydro_solve(u, dt, dh, gamma, scheme, riemann, VANLEER, recon=recon, status=status, impl=FUSED)
+    torch.cuda.synchronize()
+    st = status.cpu().tolist()
+    assert st[1] == 0 and st[2] == 0
+    pick = np.sort(np.concatenate([[0, 147, 148, 296, Ng - 1], np.random.default_rng(11).choice(Ng, 11, replace=False)]))
+    idx = torch.from_numpy(pick).cuda()
+    ref_out, ref_ff, _ = oracle.hydro_solve(u[idx].cpu().numpy(), dt, dh, gamma, scheme, riemann, VANLEER, recon=recon,
+                                            nthreads=nthreads)[:3]
+    check(out[idx].cpu().numpy(), ff[idx].cpu().numpy(), ref_out, ref_ff, dtype, (scheme, recon, riemann, np.dtype(dtype).name))
+    uin = u[:, :, g:g + PS, g:g + PS, g:g + PS].double()
+    lhs = (out.double() - uin).sum(dim=(2, 3, 4))
+    f64 = ff.double()
+    net = sum(f64[:, 3 * d + 2].sum(dim=(2, 3)) - f64[:, 3 * d + 0].sum(dim=(2, 3)) for d in range(3))
+    scale = uin.abs().sum(dim=(2, 3, 4)).max().item()
+    assert (lhs + (dt / dh) * net).abs().max().item() <= (2e-6 if dtype == np.float32 else 1e-13) * scale
