@@ -21,6 +21,7 @@ PS = 16
 
 EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64", "hydro_pipeline_create",
            "hydro_pipeline_destroy", "hydro_pipeline_solve_f32", "hydro_pipeline_solve_f64", "hydro_min_ghost",
+           "hydro_gather_f32", "hydro_gather_f64", "hydro_scatter_f32", "hydro_scatter_f64",
            "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror")
 
 
@@ -57,6 +58,9 @@ def lib():
         L.hydro_pipeline_create.argtypes = [C.POINTER(vp), i, i, i, i]
         L.hydro_pipeline_destroy.argtypes = [vp]
         L.hydro_pipeline_destroy.restype = None
+        for name in ("f32", "f64"):
+            getattr(L, "hydro_gather_" + name).argtypes = [vp, vp, i, i, i, i, i, vp]
+            getattr(L, "hydro_scatter_" + name).argtypes = [vp, vp, i, i, i, vp]
         L.hydro_min_ghost.argtypes = [i, i]
         L.hydro_has_fused.argtypes = [i, i, i, i]
         L.hydro_fused_fits.argtypes = [i, i, i, i]
@@ -186,6 +190,65 @@ def hydro_dt(u, gamma, norm=0, *, max_speed=None, stream=None):
     if rc != 0:
         raise HydroError(rc, "hydro_dt_" + sfx)
     return max_speed
+
+
+BC_PERIODIC, BC_OUTFLOW = 0, 1
+
+
+def hydro_gather(grid, nghost, bc=BC_PERIODIC, *, groups=None, stream=None):
+    """hydro_gather_f32/f64: padded patch groups [Ng,5,S,S,S] of a CUDA grid [5,Nz,Ny,Nx] (multiples of 16)."""
+    if not grid.is_cuda or not grid.is_contiguous() or grid.dim() != 4 or grid.shape[0] != 5:
+        raise ValueError("hydro_gather: grid must be a contiguous CUDA tensor [5,Nz,Ny,Nx]")
+    sfx, _ = _suffix(grid)
+    nz, ny, nx = grid.shape[1:]
+    S = PS + 2 * nghost
+    Ng = (nx // PS) * (ny // PS) * (nz // PS)
+    if groups is None:
+        groups = torch.empty((Ng, 5, S, S, S), dtype=grid.dtype, device=grid.device)
+    st = (stream or torch.cuda.current_stream(grid.device)).cuda_stream
+    with torch.cuda.device(grid.device):
+        rc = getattr(lib(), "hydro_gather_" + sfx)(grid.data_ptr(), groups.data_ptr(), nx, ny, nz, nghost, bc, st)
+    if rc != 0:
+        raise HydroError(rc, "hydro_gather_" + sfx)
+    return groups
+
+
+def hydro_scatter(out, shape, *, grid=None, stream=None):
+    """hydro_scatter_f32/f64: interiors out[Ng,5,16,16,16] back into a grid [5,Nz,Ny,Nx] with shape = (Nz,Ny,Nx)."""
+    if not out.is_cuda or not out.is_contiguous() or out.dim() != 5 or tuple(out.shape[1:]) != (5, PS, PS, PS):
+        raise ValueError("hydro_scatter: out must be a contiguous CUDA tensor [Ng,5,16,16,16]")
+    sfx, _ = _suffix(out)
+    nz, ny, nx = shape
+    if out.shape[0] != (nx // PS) * (ny // PS) * (nz // PS):
+        raise ValueError("hydro_scatter: group count does not match the grid shape")
+    if grid is None:
+        grid = torch.empty((5, nz, ny, nx), dtype=out.dtype, device=out.device)
+    st = (stream or torch.cuda.current_stream(out.device)).cuda_stream
+    with torch.cuda.device(out.device):
+        rc = getattr(lib(), "hydro_scatter_" + sfx)(out.data_ptr(), grid.data_ptr(), nx, ny, nz, st)
+    if rc != 0:
+        raise HydroError(rc, "hydro_scatter_" + sfx)
+    return grid
+
+
+def hydro_advance(grid, steps, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, cfl=0.5, bc=BC_PERIODIC, recon=PLM,
+                  nghost=0, status=None, **optkw):
+    """`steps` updates of a uniform CUDA grid [5,Nz,Ny,Nx] without leaving the device: per step
+    hydro_gather -> hydro_dt -> hydro_solve (dt = cfl*dh/max_speed formed on the device) -> hydro_scatter.
+    Returns (grid, t) with t a device scalar (fp64) holding the elapsed time.  No host synchronisation."""
+    g = nghost or hydro_min_ghost(scheme, recon)
+    shape = tuple(grid.shape[1:])
+    groups = out = None
+    smax = torch.empty((), dtype=grid.dtype, device=grid.device)
+    t = torch.zeros((), dtype=torch.float64, device=grid.device)
+    for _ in range(steps):
+        groups = hydro_gather(grid, g, bc, groups=groups)
+        hydro_dt(groups, gamma, 0, max_speed=smax)
+        out, _ = hydro_solve(groups, 0.0, dh, gamma, scheme, riemann, limiter, out=out, face_flux=False, status=status,
+                             recon=recon, max_speed=smax, cfl=cfl, **optkw)
+        grid = hydro_scatter(out, shape, grid=grid)
+        t += (cfl * dh) / smax.double()
+    return grid, t
 
 
 class HydroPipeline:

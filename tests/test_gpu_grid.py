@@ -1,0 +1,104 @@
+"""SURVEY.md 8(f)-1 on the GPU: device-side gather / scatter for uniform grids (bit-exact against the numpy
+definition in workloads.py, which the CUDA path does not use) and the on-device multi-step driver."""
+import numpy as np
+import pytest
+
+from paper_1103_3373_b200 import workloads as wl
+from tests.harness import CudaBackend, OracleBackend, run_grid
+
+pytestmark = pytest.mark.gpu
+CTU, ROE, HLLC, VANLEER = 2, 3, 2, 1
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1103_3373_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+@pytest.mark.parametrize("bc", ("periodic", "outflow"))
+@pytest.mark.parametrize("g", (2, 3, 4))
+def test_gather_scatter_bit_exact(B, dtype, bc, g):
+    import torch
+    rng = np.random.default_rng(g)
+    U = rng.standard_normal((5, 32, 48, 16)).astype(dtype)   # Nz, Ny, Nx all different
+    ref = wl.grid_to_groups(U, g, bc)
+    Ud = torch.from_numpy(U).cuda()
+    G = B.hydro_gather(Ud, g, B.BC_PERIODIC if bc == "periodic" else B.BC_OUTFLOW)
+    assert np.array_equal(G.cpu().numpy(), ref)
+    out = torch.from_numpy(np.ascontiguousarray(ref[:, :, g:g + 16, g:g + 16, g:g + 16])).cuda()
+    back = B.hydro_scatter(out, U.shape[1:])
+    assert np.array_equal(back.cpu().numpy(), U)
+    assert np.array_equal(back.cpu().numpy(), wl.groups_to_grid(out.cpu().numpy(), U.shape[1:]))
+
+
+def test_gather_argument_errors(B):
+    import torch
+    bad = torch.zeros((5, 16, 16, 24), device="cuda")
+    with pytest.raises(B.HydroError):
+        B.hydro_gather(bad, 2)
+    ok = torch.zeros((5, 16, 16, 16), device="cuda")
+    with pytest.raises(B.HydroError):
+        B.hydro_gather(ok, 2, 7)
+    empty = torch.zeros((5, 0, 16, 16), device="cuda")
+    assert B.hydro_gather(empty, 2).shape[0] == 0
+
+
+# the on-device driver against the host-gather loop of tests/harness.py (same kernels; dt/dh is formed on the device
+# as cfl / max_speed instead of on the host as (cfl * dh / max_speed) / dh, so agreement is to rounding, not bitwise)
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+def test_advance_matches_host_gather_loop(B, dtype):
+    import torch
+    gamma, N, steps = 5.0 / 3.0, 32, 6
+    U0 = wl.blast_grid(N, dtype=dtype)
+    Uh, th, _, _ = run_grid(CudaBackend(0), U0.copy(), steps, 1.0, gamma, CTU, HLLC, VANLEER, cfl=0.5)
+    Ud, td = B.hydro_advance(torch.from_numpy(U0).cuda(), steps, 1.0, gamma, CTU, HLLC, VANLEER, cfl=0.5)
+    d = np.abs(Ud.cpu().numpy().astype(np.float64) - Uh)
+    tol = steps * (1e-5 if dtype == np.float32 else 1e-13)
+    for v in ((0,), (1, 2, 3), (4,)):
+        assert d[list(v)].sum() <= tol * np.abs(Uh[list(v)]).sum()
+    assert abs(td.item() - th) <= 1e-6 * th
+
+
+# config 1 on the device driver against the oracle (outflow ghosts, 20 steps, fp64)
+def test_config1_sod_on_device(B):
+    import torch
+    from oracle import oracle as O
+    gamma, N = 1.4, 32
+    U0 = wl.sod_grid(N, axis=0, gamma=gamma)
+    Ur, tr, _, _ = run_grid(OracleBackend(O, 4), U0.copy(), 20, 1.0 / N, gamma, CTU, ROE, VANLEER, cfl=0.5, bc="outflow")
+    Ud, td = B.hydro_advance(torch.from_numpy(U0).cuda(), 20, 1.0 / N, gamma, CTU, ROE, VANLEER, cfl=0.5, bc=B.BC_OUTFLOW)
+    d = np.abs(Ud.cpu().numpy() - Ur)
+    for v, sc in ((0, np.abs(Ur[0]).max()), (1, np.abs(Ur[1:4]).max()), (4, np.abs(Ur[4]).max())):
+        assert d[v].max() <= 20 * 1e-12 * sc
+    assert abs(td.item() - tr) <= 1e-12 * tr
+
+
+# config 2 at its FULL size (128^3 fp32, 50 steps, periodic) on the device: the properties that hold at any size
+def test_config2_blast_full_size_properties(B):
+    import torch
+    gamma, N, steps = 5.0 / 3.0, 128, 50
+    U0 = wl.blast_grid(N, dtype=np.float32)
+    status = torch.zeros(3, dtype=torch.int64, device="cuda")
+    Ud, _ = B.hydro_advance(torch.from_numpy(U0).cuda(), steps, 1.0, gamma, CTU, HLLC, VANLEER, cfl=0.5, status=status)
+    U = Ud.cpu().numpy().astype(np.float64)
+    assert status.cpu().tolist()[1] == 0 and np.isfinite(U).all() and U[0].min() > 0
+    # conserved totals (P11): mass and energy drift, net momentum
+    for v in (0, 4):
+        s0 = U0[v].sum(dtype=np.float64)
+        assert abs(U[v].sum() - s0) <= 1e-6 * s0
+    assert np.abs(U[1:4].sum(axis=(1, 2, 3))).max() <= 1e-6 * np.abs(U[1:4]).sum()
+    # axis-permutation and mirror symmetry (P14): rounding level in fp32, a direction bug gives O(1)
+    rho = U[0]
+    scale = np.abs(rho - 1.0).max()
+    assert scale > 1e-2  # the blast has moved
+    for perm in ((1, 0, 2), (2, 1, 0), (0, 2, 1), (1, 2, 0)):
+        assert np.abs(rho - rho.transpose(perm)).max() <= 1e-4 * rho.max()
+    # mirror about the grid node N/2 (the blast centre): cell i <-> N - 1 - i; the normal momentum changes sign
+    assert np.abs(rho - rho[::-1, :, :]).max() <= 1e-4 * rho.max()
+    assert np.abs(U[1] + U[1][:, :, ::-1]).max() <= 1e-4 * np.abs(U[1:4]).max()
