@@ -16,32 +16,50 @@ namespace hydro {
 
 constexpr int GRID_NT = 256;
 
-// one CTA per (group, variable, z plane of the padded group); threads sweep the S x S plane, x fastest
+// one CTA per (group, variable), GATHER_PL z planes of the padded group per pass: warp w fetches the rows j = w, w+8, ...
+// of all those planes (lane = x, so a lane's source column is computed once; all loads of a pass are in flight
+// together), the planes are staged in shared memory and leave as 16-byte pieces: GATHER_PL destination planes are
+// GATHER_PL * S*S contiguous elements starting on a 16-byte boundary.
 template <class R>
 __global__ void __launch_bounds__(GRID_NT) gather_kernel(const R* __restrict__ grid, R* __restrict__ groups, int Gx, int Gy, int Gz,
                                                           int g, int bc) {
-  const int S = PS + 2 * g, Nx = Gx * PS, Ny = Gy * PS, Nz = Gz * PS;
-  long long b = blockIdx.x;
-  const int k = (int)(b % S); b /= S;
-  const int v = (int)(b % 5); b /= 5;
-  const int n = (int)b;
+  constexpr int VEC = 16 / sizeof(R), NWARP = GRID_NT / 32, MAXR = (32 + NWARP - 1) / NWARP;  // rows per warp and plane
+  constexpr int GATHER_PL = 4;  // planes per pass (8 measured slower: ragged last pass, fewer resident CTAs)
+  __shared__ __align__(16) R tile[GATHER_PL * 32 * 32];
+  const int S = PS + 2 * g, SS = S * S, Nx = Gx * PS, Ny = Gy * PS, Nz = Gz * PS;
+  const int v = blockIdx.x % 5, n = blockIdx.x / 5;
   const int gx = n % Gx, gy = (n / Gx) % Gy, gz = n / (Gx * Gy);
-  int z = gz * PS - g + k;
-  if (bc == 0) z = z < 0 ? z + Nz : (z >= Nz ? z - Nz : z);
-  else z = z < 0 ? 0 : (z >= Nz ? Nz - 1 : z);
-  const R* src = grid + ((size_t)v * Nz + z) * Ny * Nx;
-  R* dst = groups + (((size_t)n * 5 + v) * S + k) * S * S;
-  for (int idx = threadIdx.x; idx < S * S; idx += GRID_NT) {
-    const int j = idx / S, i = idx - j * S;
-    int y = gy * PS - g + j, x = gx * PS - g + i;
-    if (bc == 0) {
-      y = y < 0 ? y + Ny : (y >= Ny ? y - Ny : y);
-      x = x < 0 ? x + Nx : (x >= Nx ? x - Nx : x);
-    } else {
-      y = y < 0 ? 0 : (y >= Ny ? Ny - 1 : y);
-      x = x < 0 ? 0 : (x >= Nx ? Nx - 1 : x);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  auto fold = [bc](int c, int N) {  // periodic wrap or zero-gradient clamp (ghost width <= 8 < 16 <= N)
+    return bc == 0 ? (c < 0 ? c + N : (c >= N ? c - N : c)) : (c < 0 ? 0 : (c >= N ? N - 1 : c));
+  };
+  const R* src = grid + (size_t)v * Nz * Ny * Nx + fold(gx * PS - g + lane, Nx);
+  size_t yo[MAXR];  // source row offsets of this warp's rows
+#pragma unroll
+  for (int r = 0; r < MAXR; ++r) yo[r] = (size_t)fold(gy * PS - g + min(warp + r * NWARP, S - 1), Ny) * Nx;
+  uint4* dst = reinterpret_cast<uint4*>(groups + ((size_t)n * 5 + v) * S * SS);
+  for (int k0 = 0; k0 < S; k0 += GATHER_PL) {
+    const int np = min(GATHER_PL, S - k0);
+    R val[GATHER_PL][MAXR];
+#pragma unroll
+    for (int q = 0; q < GATHER_PL; ++q) {
+      const R* sp = src + (size_t)fold(gz * PS - g + min(k0 + q, S - 1), Nz) * Ny * Nx;
+#pragma unroll
+      for (int r = 0; r < MAXR; ++r) val[q][r] = (lane < S) ? __ldg(sp + yo[r]) : R(0);
     }
-    dst[idx] = __ldg(src + (size_t)y * Nx + x);
+    __syncthreads();  // the previous pass has left the tile
+    if (lane < S) {
+#pragma unroll
+      for (int q = 0; q < GATHER_PL; ++q)
+#pragma unroll
+        for (int r = 0; r < MAXR; ++r) {
+          const int j = warp + r * NWARP;
+          if (j < S && q < np) tile[q * SS + j * S + lane] = val[q][r];
+        }
+    }
+    __syncthreads();
+    const uint4* t4 = reinterpret_cast<const uint4*>(tile);
+    for (int q = threadIdx.x; q < np * SS / VEC; q += GRID_NT) dst[(size_t)k0 * (SS / VEC) + q] = t4[q];
   }
 }
 
@@ -74,7 +92,7 @@ static int gather_impl(const R* grid, R* groups, int nx, int ny, int nz, int ngh
   if (Ng == 0) return HYDRO_OK;
   if (!grid || !groups) return HYDRO_E_NULL;
   if (((uintptr_t)grid & 15) || ((uintptr_t)groups & 15)) return HYDRO_E_ALIGN;
-  const long long blocks = Ng * 5 * (PS + 2 * nghost);
+  const long long blocks = Ng * 5;
   if (blocks > 0x7fffffffLL) return HYDRO_E_COUNT;
   gather_kernel<R><<<(unsigned)blocks, GRID_NT, 0, st>>>(grid, groups, nx / PS, ny / PS, nz / PS, nghost, bc);
   return (int)cudaGetLastError();
