@@ -92,6 +92,11 @@ typedef struct hydro_opts {      /* NULL => all defaults */
                            ignored and dt/dh = cfl / *max_speed is formed on the device, so that
                            hydro_dt -> hydro_solve stays asynchronous (no host read of the reduction)   */
   double cfl;           /* CFL number used with max_speed (> 0)                                       */
+  void* next_max_speed; /* device scalar (float / double as the call) or NULL.  If set, it receives the hydro_dt reduction
+                           (norm `next_norm`) of the UPDATED state `out`, formed inside the update (fused kernels) or by a
+                           hydro_dt launch on `out` (staged kernel): the next step's max_speed without another pass
+                           over the data.  Must not alias max_speed                                     */
+  int next_norm;        /* 0 / 1 as in hydro_dt                                                         */
 } hydro_opts;
 
 /* One unsplit update of Ng patch groups.  in/out/face_flux: device pointers,

@@ -29,7 +29,8 @@ class HydroOpts(C.Structure):
     _fields_ = [("recon", C.c_int), ("nghost", C.c_int), ("char_limit", C.c_int), ("minmod_coeff", C.c_float),
                 ("roe_fallback", C.c_int), ("min_dens", C.c_double), ("min_pres", C.c_double),
                 ("status", C.c_void_p), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
-                ("impl", C.c_int), ("max_speed", C.c_void_p), ("cfl", C.c_double)]
+                ("impl", C.c_int), ("max_speed", C.c_void_p), ("cfl", C.c_double),
+                ("next_max_speed", C.c_void_p), ("next_norm", C.c_int)]
 
 
 class HydroError(RuntimeError):
@@ -121,12 +122,14 @@ def _suffix(t):
 
 
 def make_opts(*, recon=PLM, nghost=0, char_limit=0, minmod_coeff=0.0, roe_fallback=0, min_dens=0.0, min_pres=0.0,
-              status=None, workspace=None, impl=IMPL_AUTO, max_speed=None, cfl=0.0):
+              status=None, workspace=None, impl=IMPL_AUTO, max_speed=None, cfl=0.0, next_max_speed=None, next_norm=0):
     o = HydroOpts()
     o.recon, o.nghost, o.char_limit, o.minmod_coeff, o.roe_fallback = recon, nghost, char_limit, minmod_coeff, roe_fallback
     o.min_dens, o.min_pres, o.impl = min_dens, min_pres, impl
     o.max_speed = max_speed.data_ptr() if max_speed is not None else None
     o.cfl = cfl
+    o.next_max_speed = next_max_speed.data_ptr() if next_max_speed is not None else None
+    o.next_norm = next_norm
     o.status = status.data_ptr() if status is not None else None
     o.workspace = workspace.data_ptr() if workspace is not None else None
     o.workspace_bytes = workspace.numel() * workspace.element_size() if workspace is not None else 0
@@ -234,20 +237,24 @@ def hydro_scatter(out, shape, *, grid=None, stream=None):
 def hydro_advance(grid, steps, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, cfl=0.5, bc=BC_PERIODIC, recon=PLM,
                   nghost=0, status=None, **optkw):
     """`steps` updates of a uniform CUDA grid [5,Nz,Ny,Nx] without leaving the device: per step
-    hydro_gather -> hydro_dt -> hydro_solve (dt = cfl*dh/max_speed formed on the device) -> hydro_scatter.
+    hydro_gather -> hydro_solve (dt = cfl*dh/max_speed formed on the device; the update also reduces the wave speed
+    of the new state for the next step, so hydro_dt runs once, before the first step) -> hydro_scatter.
     Returns (grid, t) with t a device scalar (fp64) holding the elapsed time.  No host synchronisation."""
     g = nghost or hydro_min_ghost(scheme, recon)
     shape = tuple(grid.shape[1:])
     groups = out = None
     smax = torch.empty((), dtype=grid.dtype, device=grid.device)
+    snext = torch.empty((), dtype=grid.dtype, device=grid.device)
     t = torch.zeros((), dtype=torch.float64, device=grid.device)
-    for _ in range(steps):
+    for k in range(steps):
         groups = hydro_gather(grid, g, bc, groups=groups)
-        hydro_dt(groups, gamma, 0, max_speed=smax)
+        if k == 0:  # later steps get their wave-speed maximum from the previous update (next_max_speed)
+            hydro_dt(groups, gamma, 0, max_speed=smax)
         out, _ = hydro_solve(groups, 0.0, dh, gamma, scheme, riemann, limiter, out=out, face_flux=False, status=status,
-                             recon=recon, max_speed=smax, cfl=cfl, **optkw)
+                             recon=recon, max_speed=smax, cfl=cfl, next_max_speed=snext, **optkw)
         grid = hydro_scatter(out, shape, grid=grid)
         t += (cfl * dh) / smax.double()
+        smax, snext = snext, smax
     return grid, t
 
 

@@ -47,18 +47,6 @@ template <class R> static LaunchFn<R> lean_fn(int scheme, int recon, int rs) {
 // ---- hydro_dt (DESIGN.md c6) -------------------------------------------------------
 // Non-negative IEEE values order like their bit patterns, and the canonical NaN pattern is larger
 // than +inf, so one integer atomicMax per CTA yields "max, or NaN if any cell was bad".
-template <class R> struct Bits;
-template <> struct Bits<float> {
-  using U = unsigned int;
-  static __device__ __forceinline__ U of(float x) { return __float_as_uint(x); }
-  static __device__ __forceinline__ U nan() { return 0x7fc00000u; }
-};
-template <> struct Bits<double> {
-  using U = unsigned long long;
-  static __device__ __forceinline__ U of(double x) { return (U)__double_as_longlong(x); }
-  static __device__ __forceinline__ U nan() { return 0x7ff8000000000000ull; }
-};
-
 constexpr int DT_NT = 256;
 constexpr int DT_ROWS_PER_THREAD = 4;  // independent 16-cell rows in flight per half-warp
 
@@ -176,6 +164,8 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   if (!(gamma > R(1)) || !(dh > R(0)) || !(dt >= R(0)) || !(theta >= 1.0 && theta <= 2.0)) return HYDRO_E_VALUE;
   if (o && (!(o->min_dens >= 0.0) || !(o->min_pres >= 0.0))) return HYDRO_E_VALUE;
   if (o && o->max_speed && (!(o->cfl > 0.0) || ((uintptr_t)o->max_speed & (sizeof(R) - 1)))) return HYDRO_E_VALUE;
+  if (o && o->next_max_speed && (((uintptr_t)o->next_max_speed & (sizeof(R) - 1)) || o->next_max_speed == o->max_speed)) return HYDRO_E_ALIGN;
+  if (o && (o->next_norm < 0 || o->next_norm > 1)) return HYDRO_E_ENUM;
   par.gamma = gamma;
   par.gm1 = gamma - R(1);
   par.igm1 = R(1) / par.gm1;
@@ -187,6 +177,8 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   par.limiter = limiter;
   par.char_limit = o ? o->char_limit : 0;
   par.roe_fallback = fb;
+  par.next_speed = (o && device_ptrs) ? static_cast<R*>(o->next_max_speed) : nullptr;
+  par.next_norm = o ? o->next_norm : 0;
   const bool has = lean_fits((int)sizeof(R), scheme, recon, g);  // kernel exists and its tiles fit in shared memory
   if (impl == HYDRO_IMPL_FUSED && !has) return HYDRO_E_NOFUSED;
   pl.recon = recon;
@@ -214,10 +206,18 @@ static int solve_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, i
   a.workspace = o ? o->workspace : nullptr;
   a.workspace_bytes = o ? o->workspace_bytes : 0;
   a.stream = st;
+  if (a.par.next_speed) {
+    const cudaError_t e = cudaMemsetAsync(a.par.next_speed, 0, sizeof(R), st);
+    if (e != cudaSuccess) return (int)e;
+  }
   if (pl.impl == HYDRO_IMPL_STAGED) {
     if (!a.workspace || ((uintptr_t)a.workspace & 15) || a.workspace_bytes < staged_slot_bytes(scheme, pl.recon, sizeof(R)))
       return HYDRO_E_WORKSPACE;
-    return (int)staged_fn<R>(scheme, pl.recon, riemann)(a);
+    R* next = a.par.next_speed;
+    a.par.next_speed = nullptr;  // the staged kernel has no fused reduction: hydro_dt on `out` after it
+    const int rc2 = (int)staged_fn<R>(scheme, pl.recon, riemann)(a);
+    if (rc2 != 0 || !next) return rc2;
+    return dt_impl<R>(out, Ng, 0, gamma, a.par.next_norm, next, st, true);
   }
   return (int)lean_fn<R>(scheme, pl.recon, riemann)(a);
 }
@@ -246,6 +246,7 @@ static int pipeline_solve(hydro_pipeline* p, const R* in, R* out, R* ff, int Ng,
   oo.nghost = p->g;
   oo.status = status_host ? p->d_status : nullptr;
   oo.max_speed = nullptr;
+  oo.next_max_speed = nullptr;
   Par<R> par;
   Plan pl;
   int rc = make_plan<R>(in, out, ff, Ng, dt, dh, gamma, scheme, riemann, limiter, &oo, false, par, pl);

@@ -137,6 +137,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   if (tid == 0) { issue(0); if (NRAW > 1) issue(1); }
 
   Cnt c = {0, 0, 0};
+  typename Bits<R>::U best = 0;  // running maximum of the updated cells' wave speed (next_max_speed)
   int nseq = 0;  // planes converted so far
   // con->prim of the next raw plane into ring slot `slot` (all threads)
   auto convert = [&](int slot) {
@@ -322,6 +323,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
 #pragma unroll
               for (int q = 0; q < 5; ++q) U[q] = Uold[q] - p.nu * (Dz[q] + Fz[q]);
               const V5<R> Wn = Op::c2p(U, p, c);
+              if (p.next_speed) track_speed(Wn, p, best);
               if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
               st5(gout0 + (t - 1) * PS * PS, PS * PS * PS, U);
             }
@@ -361,6 +363,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     }
   }
   flush_counters(c, status);
+  flush_speed(best, p.next_speed);
 }
 
 // persistent grid: SMs x resident CTAs per SM (occupancy API), capped at Ng

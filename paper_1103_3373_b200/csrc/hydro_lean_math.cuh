@@ -96,6 +96,27 @@ template <class R> __device__ __forceinline__ V5<R> lean_correct(const V5<R>& W,
   return lean_cons2prim(U, p, bad);
 }
 
+// ---- c6 fused into the update: wave speed of the UPDATED cell for the next step's dt (hydro_opts::next_max_speed)
+template <class R> __device__ __forceinline__ void track_speed(const V5<R>& W, const Par<R>& p, typename Bits<R>::U& best) {
+  using U = typename Bits<R>::U;
+  const R c = l_sqrt(p.gamma * W[4] * l_rcp(W[0]));
+  const R ax = m_abs(W[1]), ay = m_abs(W[2]), az = m_abs(W[3]);
+  const R s = p.next_norm == 0 ? m_max(m_max(ax, ay), az) + c : ((ax + ay) + az) + R(3) * c;
+  const bool bad = !(W[0] > R(0)) || !(W[4] > R(0)) || !(s == s);
+  const U bits = bad ? Bits<R>::nan() : Bits<R>::of(s);
+  best = bits > best ? bits : best;
+}
+template <class R> __device__ __forceinline__ void flush_speed(typename Bits<R>::U best, R* dst) {
+  using U = typename Bits<R>::U;
+  if (!dst) return;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const U other = __shfl_xor_sync(0xffffffffu, best, o);
+    best = other > best ? other : best;
+  }
+  if ((threadIdx.x & 31) == 0 && best) atomicMax(reinterpret_cast<U*>(dst), best);
+}
+
 // ---- c1-c3: PLM + van Leer limiter on primitive variables + CTU tracing (normal frame) ---------
 template <class R> __device__ __forceinline__ R vl_slope(R dL, R dR) {
   const R prod = dL * dR;

@@ -94,6 +94,7 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
   if (tid == 0) issue(0);
 
   Cnt c = {0, 0, 0};
+  typename Bits<R>::U best = 0;  // running maximum of the updated cells' wave speed (next_max_speed)
   int nseq = 0;
   auto convert = [&]() {
     mbar_wait(bar, (uint32_t)(nseq & 1));
@@ -229,6 +230,7 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
 #pragma unroll
               for (int q = 0; q < 5; ++q) U[q] = Uold[q] - p.nu * (Dz[q] + Fz[q]);
               const V5<R> Wn = Op::c2p(U, p, c);
+              if (p.next_speed) track_speed(Wn, p, best);
               if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
               st5(gout0 + (b - 1) * PS * PS, PS * PS * PS, U);
             }
@@ -267,6 +269,7 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     }
   }
   flush_counters(c, status);
+  flush_speed(best, p.next_speed);
 }
 
 template <class R, int RECON, int RS, int FAST> cudaError_t launch_vl_lean(const SolveArgs<R>& a) {

@@ -62,6 +62,21 @@ template <class R> struct V5 {
   __device__ __forceinline__ const R& operator[](int i) const { return q[i]; }
 };
 
+// IEEE bit patterns for the wave-speed maxima (hydro_dt, hydro_opts::next_max_speed): non-negative values order like
+// their bits and the canonical NaN pattern is larger than +inf, so an integer atomicMax yields "max, or NaN if bad"
+template <class R> struct Bits;
+template <> struct Bits<float> {
+  using U = unsigned int;
+  static __device__ __forceinline__ U of(float x) { return __float_as_uint(x); }
+  static __device__ __forceinline__ U nan() { return 0x7fc00000u; }
+};
+template <> struct Bits<double> {
+  using U = unsigned long long;
+  static __device__ __forceinline__ U of(double x) { return (U)__double_as_longlong(x); }
+  static __device__ __forceinline__ U nan() { return 0x7ff8000000000000ull; }
+};
+
+
 // run-time parameters of one hydro_solve call (uniform over the grid)
 template <class R> struct Par {
   R gamma, gm1;   // gamma, gamma-1
@@ -70,6 +85,8 @@ template <class R> struct Par {
   R theta;        // generalized-minmod coefficient (S7)
   R min_dens, min_pres;
   int limiter, char_limit, roe_fallback;
+  R* next_speed;  // hydro_opts::next_max_speed (device scalar, zeroed by the host before the launch) or nullptr
+  int next_norm;
 };
 
 // dt/dh from the device-resident hydro_dt result (hydro_opts::max_speed), uniform over the grid

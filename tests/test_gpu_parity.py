@@ -362,3 +362,28 @@ def test_large_batch_sampled_variants(B, oracle, nthreads, dtype, scheme, recon,
     net = sum(f64[:, 3 * d + 2].sum(dim=(2, 3)) - f64[:, 3 * d + 0].sum(dim=(2, 3)) for d in range(3))
     scale = uin.abs().sum(dim=(2, 3, 4)).max().item()
     assert (lhs + (dt / dh) * net).abs().max().item() <= (2e-6 if dtype == np.float32 else 1e-13) * scale
+
+
+# ---- hydro_opts::next_max_speed: the update's fused wave-speed reduction equals hydro_dt of `out` ----------------
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+@pytest.mark.parametrize("scheme", (MHM, VL, CTU))
+def test_next_max_speed_matches_hydro_dt(B, dtype, scheme):
+    import torch
+    gamma, dh = 5.0 / 3.0, 1.0
+    tdt = torch.float32 if dtype == np.float32 else torch.float64
+    g = B.hydro_min_ghost(scheme, PLM)
+    u = wl.amr_batch(301, g=g, gamma=gamma, seed=9, dtype=np.dtype(dtype).name, device=torch.device("cuda"))
+    dt = 0.3 * dh / float(B.hydro_dt(u, gamma, 0).item())
+    for impl in impls(B, dtype, scheme, PLM):
+        for norm in (0, 1):
+            nxt = torch.full((), -1.0, dtype=tdt, device="cuda")
+            out, _ = B.hydro_solve(u, dt, dh, gamma, scheme, ROE, VANLEER, impl=impl, face_flux=False,
+                                   next_max_speed=nxt, next_norm=norm)
+            ref = B.hydro_dt(out, gamma, norm).item()
+            assert abs(nxt.item() - ref) <= 16 * np.finfo(dtype).eps * ref, (scheme, impl, norm)
+    # a bad updated cell must surface as NaN, as in hydro_dt
+    bad = u.clone()
+    bad[7, 4] = -1.0  # negative energy everywhere in one group -> negative pressure after the update
+    nxt = torch.zeros((), dtype=tdt, device="cuda")
+    B.hydro_solve(bad, dt, dh, gamma, scheme, HLLE, VANLEER, face_flux=False, next_max_speed=nxt)
+    assert np.isnan(nxt.item())
