@@ -102,3 +102,52 @@ def test_config2_blast_full_size_properties(B):
     # mirror about the grid node N/2 (the blast centre): cell i <-> N - 1 - i; the normal momentum changes sign
     assert np.abs(rho - rho[::-1, :, :]).max() <= 1e-4 * rho.max()
     assert np.abs(U[1] + U[1][:, :, ::-1]).max() <= 1e-4 * np.abs(U[1:4]).max()
+
+
+def _totals(U):
+    return [U[v].double().sum().item() for v in range(5)], U.abs().double().sum(dim=(1, 2, 3)).cpu().numpy()
+
+
+# config 4 at its FULL size (256^3 fp32, periodic Kelvin-Helmholtz layer): every scheme x reconstruction x {Roe, HLLC},
+# 10 steps each on the device; the properties that hold at any size (the element-wise parity of these variants is in
+# test_gpu_parity.py: small KH box for 10 steps, and sampled groups of large batches)
+@pytest.mark.parametrize("scheme", (0, 1, 2))
+def test_config4_kh_full_size_properties(B, scheme):
+    import torch
+    gamma, N, steps = 1.4, 256, 10
+    U0 = torch.from_numpy(wl.kh_grid((N, N, N), gamma=gamma, seed=1, dtype=np.float32)).cuda()
+    tot0, abs0 = _totals(U0)
+    for recon in (0, 1):
+        for riemann in (ROE, HLLC):
+            status = torch.zeros(3, dtype=torch.int64, device="cuda")
+            U, t = B.hydro_advance(U0.clone(), steps, 1.0 / N, gamma, scheme, riemann, VANLEER, cfl=0.3, recon=recon,
+                                   status=status)
+            assert status.cpu().tolist()[1] == 0 and torch.isfinite(U).all().item()
+            assert U[0].min().item() > 0.9 and t.item() > 0
+            tot, _ = _totals(U)
+            for v in (0, 1, 4):  # mass, x momentum, energy; y and z momenta start at ~0
+                assert abs(tot[v] - tot0[v]) <= 2e-6 * abs0[v], (scheme, recon, riemann, v)
+            for v in (2, 3):
+                assert abs(tot[v] - tot0[v]) <= 2e-6 * abs0[1]
+            # the shear layer is still there and the perturbation has not blown up
+            assert 0.4 < U[1].abs().max().item() / U[0].max().item() < 0.7
+
+
+# config 5 at its FULL size (512^3, 32768 patch groups, Mach-1 turbulence): CTU + PPM + exact solver, 10 steps, both precisions
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+def test_config5_turbulence_full_size_properties(B, dtype):
+    import torch
+    gamma, N, steps = 5.0 / 3.0, 512, 10
+    U0 = torch.from_numpy(wl.turbulence_grid(N, gamma=gamma, kmax=32, seed=2, dtype=dtype)).cuda()
+    tot0, abs0 = _totals(U0)
+    status = torch.zeros(3, dtype=torch.int64, device="cuda")
+    U, t = B.hydro_advance(U0, steps, 1.0 / N, gamma, CTU, 0, VANLEER, cfl=0.5, recon=1, status=status)
+    st = status.cpu().tolist()
+    assert st[1] == 0 and st[2] == 0 and torch.isfinite(U).all().item() and U[0].min().item() > 0
+    tot, _ = _totals(U)
+    tol = 2e-6 if dtype == np.float32 else 1e-12
+    for v in (0, 4):
+        assert abs(tot[v] - tot0[v]) <= tol * abs0[v]
+    for v in (1, 2, 3):
+        assert abs(tot[v] - tot0[v]) <= tol * abs0[0]  # |v| ~ 1, rho = 1: the mass scale
+    assert 0 < t.item() < 10 * 0.5 / N  # max speed >= c = 1
