@@ -235,26 +235,45 @@ def hydro_scatter(out, shape, *, grid=None, stream=None):
 
 
 def hydro_advance(grid, steps, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, cfl=0.5, bc=BC_PERIODIC, recon=PLM,
-                  nghost=0, status=None, **optkw):
+                  nghost=0, status=None, graph=False, **optkw):
     """`steps` updates of a uniform CUDA grid [5,Nz,Ny,Nx] without leaving the device: per step
     hydro_gather -> hydro_solve (dt = cfl*dh/max_speed formed on the device; the update also reduces the wave speed
     of the new state for the next step, so hydro_dt runs once, before the first step) -> hydro_scatter.
-    Returns (grid, t) with t a device scalar (fp64) holding the elapsed time.  No host synchronisation."""
+    Returns (grid, t) with t a device scalar (fp64) holding the elapsed time; `grid` is updated in place.
+    No host synchronisation.  graph=True captures one step in a CUDA graph after the first step and replays it:
+    small grids are launch-bound (four launches and a memset per step)."""
     g = nghost or hydro_min_ghost(scheme, recon)
     shape = tuple(grid.shape[1:])
-    groups = out = None
+    S = PS + 2 * g
+    Ng = (shape[0] // PS) * (shape[1] // PS) * (shape[2] // PS)
+    groups = torch.empty((Ng, 5, S, S, S), dtype=grid.dtype, device=grid.device)
+    out = torch.empty((Ng, 5, PS, PS, PS), dtype=grid.dtype, device=grid.device)
     smax = torch.empty((), dtype=grid.dtype, device=grid.device)
     snext = torch.empty((), dtype=grid.dtype, device=grid.device)
     t = torch.zeros((), dtype=torch.float64, device=grid.device)
-    for k in range(steps):
-        groups = hydro_gather(grid, g, bc, groups=groups)
-        if k == 0:  # later steps get their wave-speed maximum from the previous update (next_max_speed)
-            hydro_dt(groups, gamma, 0, max_speed=smax)
-        out, _ = hydro_solve(groups, 0.0, dh, gamma, scheme, riemann, limiter, out=out, face_flux=False, status=status,
-                             recon=recon, max_speed=smax, cfl=cfl, next_max_speed=snext, **optkw)
-        grid = hydro_scatter(out, shape, grid=grid)
-        t += (cfl * dh) / smax.double()
-        smax, snext = snext, smax
+    if steps <= 0:
+        return grid, t
+
+    def step():
+        hydro_gather(grid, g, bc, groups=groups)
+        hydro_solve(groups, 0.0, dh, gamma, scheme, riemann, limiter, out=out, face_flux=False, status=status,
+                    recon=recon, max_speed=smax, cfl=cfl, next_max_speed=snext, **optkw)
+        hydro_scatter(out, shape, grid=grid)
+        t.add_((cfl * dh) / smax.double())
+        smax.copy_(snext)
+
+    hydro_dt(hydro_gather(grid, g, bc, groups=groups), gamma, 0, max_speed=smax)
+    step()
+    if graph and steps > 1:
+        cg = torch.cuda.CUDAGraph()
+        torch.cuda.synchronize(grid.device)
+        with torch.cuda.graph(cg):  # capture only records; nothing runs here
+            step()
+        for _ in range(steps - 1):
+            cg.replay()
+    else:
+        for _ in range(steps - 1):
+            step()
     return grid, t
 
 

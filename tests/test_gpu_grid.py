@@ -151,3 +151,13 @@ def test_config5_turbulence_full_size_properties(B, dtype):
     for v in (1, 2, 3):
         assert abs(tot[v] - tot0[v]) <= tol * abs0[0]  # |v| ~ 1, rho = 1: the mass scale
     assert 0 < t.item() < 10 * 0.5 / N  # max speed >= c = 1
+
+
+# CUDA-graph replay of the step (launch-bound small grids) gives the same bits as launching every step
+def test_advance_graph_replay_is_identical(B):
+    import torch
+    gamma, N, steps = 1.4, 32, 12
+    U0 = torch.from_numpy(wl.sod_grid(N, axis=1, gamma=gamma)).cuda()
+    Ua, ta = B.hydro_advance(U0.clone(), steps, 1.0 / N, gamma, CTU, ROE, VANLEER, cfl=0.5, bc=B.BC_OUTFLOW)
+    Ub, tb = B.hydro_advance(U0.clone(), steps, 1.0 / N, gamma, CTU, ROE, VANLEER, cfl=0.5, bc=B.BC_OUTFLOW, graph=True)
+    assert torch.equal(Ua, Ub) and ta.item() == tb.item()
