@@ -144,6 +144,17 @@ HYDRO_API int hydro_gather_f64(const double* grid, double* groups, int nx, int n
 HYDRO_API int hydro_scatter_f32(const float* out, float* grid, int nx, int ny, int nz, hydro_stream_t stream);
 HYDRO_API int hydro_scatter_f64(const double* out, double* grid, int nx, int ny, int nz, hydro_stream_t stream);
 
+/* One update of a UNIFORM grid in one launch (no gather / scatter pass, no group buffers): the fused kernel fetches the
+ * planes of every patch group from grid_in [5][nz][ny][nx] directly, ghost zones of width hydro_min_ghost() folded at the
+ * domain boundary (bc 0 periodic, 1 outflow), and writes the updated cells to grid_out (same shape; must not be grid_in).
+ * opts as in hydro_solve_* (nghost, workspace and impl ignored; face fluxes are not produced).  Available for the
+ * default options of the CTU scheme (van Leer limiter on primitive variables, no floors); otherwise returns
+ * HYDRO_E_NOFUSED and the caller uses hydro_gather_* -> hydro_solve_* -> hydro_scatter_*. */
+HYDRO_API int hydro_solve_grid_f32(const float* grid_in, float* grid_out, int nx, int ny, int nz, int bc, float dt, float dh,
+                         float gamma, int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream);
+HYDRO_API int hydro_solve_grid_f64(const double* grid_in, double* grid_out, int nx, int ny, int nz, int bc, double dt, double dh,
+                         double gamma, int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream);
+
 /* Sizes and capabilities. */
 HYDRO_API int hydro_min_ghost(int scheme, int recon);                 /* 2/3 (MHM, CTU with PLM/PPM), 3/4 (VL)   */
 HYDRO_API int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann); /* 1 if a fused kernel exists */

@@ -21,7 +21,7 @@ PS = 16
 
 EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64", "hydro_pipeline_create",
            "hydro_pipeline_destroy", "hydro_pipeline_solve_f32", "hydro_pipeline_solve_f64", "hydro_min_ghost",
-           "hydro_gather_f32", "hydro_gather_f64", "hydro_scatter_f32", "hydro_scatter_f64",
+           "hydro_solve_grid_f32", "hydro_solve_grid_f64", "hydro_gather_f32", "hydro_gather_f64", "hydro_scatter_f32", "hydro_scatter_f64",
            "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror")
 
 
@@ -54,6 +54,7 @@ def lib():
         for name, ft in (("f32", C.c_float), ("f64", C.c_double)):
             getattr(L, "hydro_solve_" + name).argtypes = [vp, vp, vp, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
             getattr(L, "hydro_dt_" + name).argtypes = [vp, i, i, ft, i, vp, vp]
+            getattr(L, "hydro_solve_grid_" + name).argtypes = [vp, vp, i, i, i, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
             getattr(L, "hydro_pipeline_solve_" + name).argtypes = [vp, vp, vp, vp, i, ft, ft, ft, i, i, i,
                                                                    C.POINTER(HydroOpts), vp, vp]
         L.hydro_pipeline_create.argtypes = [C.POINTER(vp), i, i, i, i]
@@ -234,6 +235,33 @@ def hydro_scatter(out, shape, *, grid=None, stream=None):
     return grid
 
 
+def hydro_solve_grid(grid, dt, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, bc=BC_PERIODIC, out=None, status=None,
+                     stream=None, **optkw):
+    """hydro_solve_grid_f32/f64: one update of a uniform CUDA grid [5,Nz,Ny,Nx] in one launch (no gather / scatter).
+    Returns the updated grid (`out`, allocated if None; must not be `grid`).  Raises HydroError(HYDRO_E_NOFUSED)
+    for variants without the grid mode (anything but CTU with the default options)."""
+    if not grid.is_cuda or not grid.is_contiguous() or grid.dim() != 4 or grid.shape[0] != 5:
+        raise ValueError("hydro_solve_grid: grid must be a contiguous CUDA tensor [5,Nz,Ny,Nx]")
+    sfx, ft = _suffix(grid)
+    nz, ny, nx = grid.shape[1:]
+    if out is None:
+        out = torch.empty_like(grid)
+    o = make_opts(status=status, **optkw)
+    st = (stream or torch.cuda.current_stream(grid.device)).cuda_stream
+    with torch.cuda.device(grid.device):
+        rc = getattr(lib(), "hydro_solve_grid_" + sfx)(grid.data_ptr(), out.data_ptr(), nx, ny, nz, bc, ft(dt), ft(dh), ft(gamma),
+                                                      scheme, riemann, limiter, C.byref(o), st)
+    if rc != 0:
+        raise HydroError(rc, "hydro_solve_grid_" + sfx)
+    return out
+
+
+def hydro_grid_mode(scheme, limiter, **optkw):
+    """True when hydro_solve_grid_* covers the variant: CTU with the default options."""
+    return (scheme == CTU and limiter == VANLEER and not optkw.get("char_limit") and not optkw.get("min_dens")
+            and not optkw.get("min_pres"))
+
+
 def hydro_advance(grid, steps, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, cfl=0.5, bc=BC_PERIODIC, recon=PLM,
                   nghost=0, status=None, graph=False, **optkw):
     """`steps` updates of a uniform CUDA grid [5,Nz,Ny,Nx] without leaving the device: per step
@@ -242,6 +270,8 @@ def hydro_advance(grid, steps, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLE
     Returns (grid, t) with t a device scalar (fp64) holding the elapsed time; `grid` is updated in place.
     No host synchronisation.  graph=True captures one step in a CUDA graph after the first step and replays it:
     small grids are launch-bound (four launches and a memset per step)."""
+    if not nghost and hydro_grid_mode(scheme, limiter, **optkw):
+        return _advance_grid_mode(grid, steps, dh, gamma, scheme, riemann, limiter, cfl, bc, recon, status, graph, optkw)
     g = nghost or hydro_min_ghost(scheme, recon)
     shape = tuple(grid.shape[1:])
     S = PS + 2 * g
@@ -274,6 +304,44 @@ def hydro_advance(grid, steps, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLE
     else:
         for _ in range(steps - 1):
             step()
+    return grid, t
+
+
+def _advance_grid_mode(grid, steps, dh, gamma, scheme, riemann, limiter, cfl, bc, recon, status, graph, optkw):
+    """hydro_advance through hydro_solve_grid_*: ONE launch per step (the kernel folds the ghost zones out of the grid,
+    forms dt from the previous step's fused wave-speed reduction and writes the new grid); two grids alternate."""
+    t = torch.zeros((), dtype=torch.float64, device=grid.device)
+    if steps <= 0:
+        return grid, t
+    other = torch.empty_like(grid)
+    sp = [torch.empty((), dtype=grid.dtype, device=grid.device) for _ in range(2)]
+    hydro_dt(hydro_gather(grid, 0, bc), gamma, 0, max_speed=sp[0])  # interiors only: the wave speed of the start state
+    bufs = [grid, other]
+
+    def step(k):
+        hydro_solve_grid(bufs[k & 1], 0.0, dh, gamma, scheme, riemann, limiter, bc=bc, out=bufs[(k + 1) & 1], status=status,
+                         recon=recon, max_speed=sp[k & 1], cfl=cfl, next_max_speed=sp[(k + 1) & 1], **optkw)
+        t.add_((cfl * dh) / sp[k & 1].double())
+
+    if graph and steps > 2:
+        step(0)
+        cg = torch.cuda.CUDAGraph()
+        torch.cuda.synchronize(grid.device)
+        with torch.cuda.graph(cg):  # two steps per replay: the buffers alternate
+            step(1)
+            step(2)
+        pairs, rest = divmod(steps - 1, 2)
+        for _ in range(pairs):
+            cg.replay()
+        if rest:
+            step(1)
+        last = 1 if steps % 2 else 0
+    else:
+        for k in range(steps):
+            step(k)
+        last = steps & 1
+    if last:  # the result sits in the scratch grid: hand it back in the caller's tensor
+        grid.copy_(other)
     return grid, t
 
 

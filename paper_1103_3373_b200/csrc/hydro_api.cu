@@ -206,6 +206,7 @@ static int solve_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, i
   a.workspace = o ? o->workspace : nullptr;
   a.workspace_bytes = o ? o->workspace_bytes : 0;
   a.stream = st;
+  a.grid = GridIO<R>{nullptr, nullptr, 0, 0, 0, 0};
   if (a.par.next_speed) {
     const cudaError_t e = cudaMemsetAsync(a.par.next_speed, 0, sizeof(R), st);
     if (e != cudaSuccess) return (int)e;
@@ -218,6 +219,46 @@ static int solve_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, i
     const int rc2 = (int)staged_fn<R>(scheme, pl.recon, riemann)(a);
     if (rc2 != 0 || !next) return rc2;
     return dt_impl<R>(out, Ng, 0, gamma, a.par.next_norm, next, st, true);
+  }
+  return (int)lean_fn<R>(scheme, pl.recon, riemann)(a);
+}
+
+// One update of a uniform grid in ONE launch: the fused CTU kernel fetches its planes from grid_in (ghost zones folded
+// at the domain boundary) and writes the updated cells into grid_out; no gather / scatter pass, no group buffers.
+template <class R>
+static int solve_grid_impl(const R* gin, R* gout, int nx, int ny, int nz, int bc, R dt, R dh, R gamma, int scheme, int riemann,
+                           int limiter, const hydro_opts* o, cudaStream_t st) {
+  if (nx < 0 || ny < 0 || nz < 0 || nx % PS || ny % PS || nz % PS) return HYDRO_E_VALUE;
+  if (bc < 0 || bc > 1) return HYDRO_E_ENUM;
+  const long long Ng = (long long)(nx / PS) * (ny / PS) * (nz / PS);
+  if (Ng > 0x7fffffffLL / 64 || nx / PS > 1023 || ny / PS > 1023 || nz / PS > 1023) return HYDRO_E_COUNT;
+  if (gin == gout && Ng > 0) return HYDRO_E_ALIGN;
+  SolveArgs<R> a;
+  Plan pl;
+  hydro_opts oo;
+  if (o) oo = *o; else std::memset(&oo, 0, sizeof(oo));
+  oo.nghost = 0;  // ghost zones come from the grid: always the minimum width
+  oo.impl = HYDRO_IMPL_FUSED;
+  const int rc = make_plan<R>(gin, gout, nullptr, (int)Ng, dt, dh, gamma, scheme, riemann, limiter, &oo, true, a.par, pl);
+  if (rc != HYDRO_OK) return rc;
+  const bool fast = limiter == LIM_VANLEER && !oo.char_limit && !(oo.min_dens > 0.0) && !(oo.min_pres > 0.0);
+  if (scheme != SCHEME_CTU || !fast) return HYDRO_E_NOFUSED;  // callers fall back to gather -> hydro_solve -> scatter
+  if (Ng == 0) return HYDRO_OK;
+  a.in = nullptr;
+  a.out = nullptr;
+  a.face_flux = nullptr;
+  a.Ng = (int)Ng;
+  a.g = pl.g;
+  a.max_speed = static_cast<const R*>(oo.max_speed);
+  a.cfl = (R)oo.cfl;
+  a.status = oo.status;
+  a.workspace = nullptr;
+  a.workspace_bytes = 0;
+  a.stream = st;
+  a.grid = GridIO<R>{gin, gout, nx / PS, ny / PS, nz / PS, bc};
+  if (a.par.next_speed) {
+    const cudaError_t e = cudaMemsetAsync(a.par.next_speed, 0, sizeof(R), st);
+    if (e != cudaSuccess) return (int)e;
   }
   return (int)lean_fn<R>(scheme, pl.recon, riemann)(a);
 }
@@ -366,6 +407,14 @@ int hydro_solve_f32(const float* in, float* out, float* face_flux, int Ng, float
 int hydro_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int scheme,
                     int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream) {
   return hydro::solve_impl<double>(in, out, face_flux, Ng, dt, dh, gamma, scheme, riemann, limiter, opts, (cudaStream_t)stream);
+}
+int hydro_solve_grid_f32(const float* grid_in, float* grid_out, int nx, int ny, int nz, int bc, float dt, float dh, float gamma,
+                         int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream) {
+  return hydro::solve_grid_impl<float>(grid_in, grid_out, nx, ny, nz, bc, dt, dh, gamma, scheme, riemann, limiter, opts, (cudaStream_t)stream);
+}
+int hydro_solve_grid_f64(const double* grid_in, double* grid_out, int nx, int ny, int nz, int bc, double dt, double dh, double gamma,
+                         int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream) {
+  return hydro::solve_grid_impl<double>(grid_in, grid_out, nx, ny, nz, bc, dt, dh, gamma, scheme, riemann, limiter, opts, (cudaStream_t)stream);
 }
 int hydro_dt_f32(const float* u, int Ng, int nghost, float gamma, int norm, float* max_speed, hydro_stream_t stream) {
   return hydro::dt_impl<float>(u, Ng, nghost, gamma, norm, max_speed, (cudaStream_t)stream);

@@ -7,6 +7,10 @@
 
 namespace hydro {
 
+// uniform-grid mode of the fused CTU kernel (hydro_solve_grid_*): planes are fetched from / written to [5][Nz][Ny][Nx]
+// grids directly, ghost zones by periodic wrap (bc 0) or zero-gradient clamp (bc 1); gin == nullptr: batch mode
+template <class R> struct GridIO { const R* gin; R* gout; int Gx, Gy, Gz, bc; };
+
 template <class R> struct SolveArgs {
   const R* in;          // [Ng][5][S^3], S = 16 + 2 g
   R* out;               // [Ng][5][16^3]
@@ -19,6 +23,7 @@ template <class R> struct SolveArgs {
   void* workspace;      // staged path only
   size_t workspace_bytes;
   cudaStream_t stream;
+  GridIO<R> grid;
 };
 
 template <class R> using LaunchFn = cudaError_t (*)(const SolveArgs<R>&);

@@ -14,6 +14,10 @@ template <class R, int SCHEME, int RECON, int RS> cudaError_t launch_lean(const 
   if constexpr (SCHEME == SCHEME_CTU) {
     // compile-time specialisation of the default options: van Leer limiter on primitive variables, no floors
     const bool fast = a.par.limiter == LIM_VANLEER && !a.par.char_limit && !(a.par.min_dens > R(0)) && !(a.par.min_pres > R(0));
+    if (a.grid.gin) {  // uniform-grid mode: only the default options are specialised
+      if (!fast) return cudaErrorNotSupported;
+      return launch_ctu_lean<R, RECON, RS, 1, LeanTune<R, RECON>::MINB, 1>(a);
+    }
     if (fast) return launch_ctu_lean<R, RECON, RS, 1, LeanTune<R, RECON>::MINB>(a);
     return launch_ctu_lean<R, RECON, RS, 0, LeanTune<R, RECON>::MINB>(a);
   } else if constexpr (SCHEME == SCHEME_MHM) {

@@ -161,3 +161,41 @@ def test_advance_graph_replay_is_identical(B):
     Ua, ta = B.hydro_advance(U0.clone(), steps, 1.0 / N, gamma, CTU, ROE, VANLEER, cfl=0.5, bc=B.BC_OUTFLOW)
     Ub, tb = B.hydro_advance(U0.clone(), steps, 1.0 / N, gamma, CTU, ROE, VANLEER, cfl=0.5, bc=B.BC_OUTFLOW, graph=True)
     assert torch.equal(Ua, Ub) and ta.item() == tb.item()
+
+
+# hydro_solve_grid_* (ghost zones folded out of the grid inside the fused kernel, one launch) against the three-launch
+# path gather -> hydro_solve -> scatter: same arithmetic on the same values, so the grids must agree bit for bit
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+@pytest.mark.parametrize("bc", (0, 1))
+@pytest.mark.parametrize("recon,riemann", ((0, ROE), (0, HLLC), (1, ROE), (1, 0)))
+def test_solve_grid_equals_gather_solve_scatter(B, dtype, bc, recon, riemann):
+    import torch
+    gamma = 1.4
+    U0 = torch.from_numpy(wl.kh_grid((32, 48, 64), gamma=gamma, seed=3, dtype=dtype)).cuda()  # Nz, Ny, Nx all different
+    g = B.hydro_min_ghost(CTU, recon)
+    groups = B.hydro_gather(U0, g, bc)
+    smax = B.hydro_dt(groups, gamma, 0)
+    dt = 0.4 * (1.0 / 64) / float(smax.item())
+    st_a = torch.zeros(3, dtype=torch.int64, device="cuda")
+    st_b = torch.zeros(3, dtype=torch.int64, device="cuda")
+    na = torch.zeros((), dtype=U0.dtype, device="cuda")
+    nb = torch.zeros((), dtype=U0.dtype, device="cuda")
+    out, _ = B.hydro_solve(groups, dt, 1.0 / 64, gamma, CTU, riemann, VANLEER, recon=recon, face_flux=False, status=st_a,
+                           next_max_speed=na)
+    ref = B.hydro_scatter(out, tuple(U0.shape[1:]))
+    got = B.hydro_solve_grid(U0, dt, 1.0 / 64, gamma, CTU, riemann, VANLEER, bc=bc, recon=recon, status=st_b, next_max_speed=nb)
+    assert torch.equal(got, ref)
+    assert st_a.tolist() == st_b.tolist() and na.item() == nb.item()
+
+
+def test_solve_grid_unsupported_variants(B):
+    import torch
+    U = torch.ones((5, 16, 16, 16), device="cuda")
+    for kw in (dict(scheme=0), dict(scheme=1), dict(limiter=0), dict(char_limit=1), dict(min_dens=1e-3)):
+        a = dict(scheme=CTU, limiter=VANLEER)
+        a.update(kw)
+        sch, lim = a.pop("scheme"), a.pop("limiter")
+        with pytest.raises(B.HydroError):
+            B.hydro_solve_grid(U, 0.01, 1.0, 1.4, sch, ROE, lim, **a)
+    with pytest.raises(B.HydroError):
+        B.hydro_solve_grid(U, 0.01, 1.0, 1.4, CTU, ROE, VANLEER, out=U)
