@@ -174,6 +174,71 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+def run_table(args):
+    """--table variants | grid: CUDA-event timings through the binding (2 warm-ups, 5 launches), inputs resident in HBM."""
+    import numpy as np
+    import torch
+    from paper_1103_3373_b200 import binding as B, workloads as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+
+    def ev(f, reps=5):
+        for _ in range(2):
+            f()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    rows = []
+    if args.table == "variants":
+        Ng = 4096
+        names, rn = {0: "MHM", 1: "VL", 2: "CTU"}, {0: "exact", 1: "HLLE", 2: "HLLC", 3: "Roe"}
+        for tdt in (torch.float32, torch.float64):
+            for scheme in (2, 0, 1):
+                for recon in (0, 1):
+                    for rs in (3, 2, 1, 0):
+                        if scheme != 2 and rs in (1, 0):
+                            continue
+                        g = B.hydro_min_ghost(scheme, recon)
+                        u = wl.amr_batch(Ng, g=g, gamma=GAMMA, seed=0, dtype=str(tdt).replace("torch.", ""), device=dev)
+                        out = torch.empty((Ng, 5, 16, 16, 16), dtype=tdt, device=dev)
+                        ff = torch.empty((Ng, 9, 5, 16, 16), dtype=tdt, device=dev)
+                        ms = ev(lambda: B.hydro_solve(u, 0.05, DH, GAMMA, scheme, rs, LIMITER, recon=recon, out=out, face_flux=ff))
+                        rows.append({"precision": "fp32" if tdt == torch.float32 else "fp64", "scheme": names[scheme],
+                                     "recon": "PPM" if recon else "PLM", "riemann": rn[rs], "ms": ms,
+                                     "cell_updates_per_s": Ng * CELLS / (ms * 1e-3),
+                                     "fused": bool(B.hydro_fused_fits(tdt, scheme, recon, g))})
+                        del u, out, ff
+        print(json.dumps({"table": "variants", "groups": Ng, "limiter": "van Leer", "rows": rows}))
+        return
+    for N, tdt in ((512, torch.float32), (256, torch.float64)):
+        es = 4 if tdt == torch.float32 else 8
+        for g in (2, 3):
+            U = torch.rand((5, N, N, N), dtype=tdt, device=dev) + 1.0
+            Ng, S = (N // 16) ** 3, 16 + 2 * g
+            G = B.hydro_gather(U, g)
+            out = torch.empty((Ng, 5, 16, 16, 16), dtype=tdt, device=dev)
+            tg = ev(lambda: B.hydro_gather(U, g, groups=G))
+            ts = ev(lambda: B.hydro_scatter(out, (N, N, N), grid=U))
+            rows.append({"kernel": "gather/scatter", "N": N, "precision": "fp32" if es == 4 else "fp64", "g": g, "gather_ms": tg,
+                         "gather_gbs": es * 5 * (N ** 3 + Ng * S ** 3) / tg / 1e6, "scatter_ms": ts,
+                         "scatter_gbs": es * 10 * N ** 3 / ts / 1e6})
+            del U, G, out
+        torch.cuda.empty_cache()
+    for N in (256, 512):
+        U = torch.from_numpy(wl.blast_grid(128, dtype=np.float32)).to(dev).repeat(1, N // 128, N // 128, N // 128).contiguous()
+        for label, kw in (("hydro_solve_grid (one launch per step)", {}), ("gather -> hydro_solve -> scatter", {"nghost": 2})):
+            ms = ev(lambda: B.hydro_advance(U, 10, 1.0, GAMMA, SCHEME, RIEMANN, LIMITER, cfl=0.4, **kw), 2) / 10
+            rows.append({"kernel": "hydro_advance, CTU+PLM+Roe fp32, " + label, "N": N, "ms_per_step": ms,
+                         "cell_updates_per_s": N ** 3 / (ms * 1e-3)})
+    print(json.dumps({"table": "grid", "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -184,9 +249,14 @@ def main():
     ap.add_argument("--ng", type=int, default=NG, help="patch groups per GPU (default: the config's 8192)")
     ap.add_argument("--kernel", default="auto", choices=("auto", "staged", "fused"))
     ap.add_argument("--no-extras", action="store_true", help="skip the e2e / cpu_baseline / f64 legs (profiling runs)")
+    ap.add_argument("--table", default=None, choices=("variants", "grid"),
+                    help="instead of the bench line: one JSON line with per-variant hydro_solve timings (4096 groups), or with the\n"
+                         "uniform-grid kernels (gather / scatter bandwidth, whole-step rates); context for DESIGN.md, profiles/")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.table:
+        return run_table(args)
 
     import torch
     import torch.distributed as dist
