@@ -9,11 +9,12 @@
 // hiding the other's barriers.  The arithmetic is the instruction-lean form of hydro_lean_math.cuh;
 // shared-memory fields use the packed "4+1" layout of hydro_ptx.cuh (2 instructions per 5-vector).
 //
-// Thread -> column of the 18 x 18 tile (interior + one-cell ring): warps 0-8 own rows j = 0..15 (18
-// columns each, i = -1..16), warp 9 owns the rows j = -1 and j = 16 (i = 0..15).  The four corner columns
-// only feed F*_x / F*_y of the ring; their work rides on lanes that would otherwise idle: their traced
-// states are formed by 8 lanes of warp 9 during phase F of the previous step, their four first-pass
-// Riemann problems by the i = -1 lanes of warp 0 (F*_x) and the j = -1 lanes of warp 9 (F*_y) in phase D.
+// Thread -> column of the 18 x 18 tile (interior + one-cell ring): warps 0-7 own the 256 interior columns (two rows of
+// 16 per warp, so no lane idles in the interior-only work), warp 8 the x ring (i = -1, 16) and warp 9 the y ring
+// (j = -1, 16), which only do the work the ring needs.  The four corner columns only feed F*_x / F*_y of the ring;
+// their work rides on lanes that would otherwise idle: their traced states are formed by 8 lanes of warp 9 during
+// phase F of the previous step, their four first-pass Riemann problems by i = -1 lanes of warp 8 (F*_x) and
+// j = -1 lanes of warp 9 (F*_y) in phase D.
 //
 // Step t = -2 .. 16 of a group (plane index; W = primitive planes in a ring, one plane converted per step):
 //   B  z: traced states of plane t+1 (own column of the ring planes) -> private slots;
@@ -100,18 +101,21 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
 
   const int tid = threadIdx.x;
   // ---- column and role of this thread
+  // warps 0-7: the 256 interior columns (two rows of 16 per warp: no lane idles in the interior-only phases);
+  // warp 8: the x ring (i = -1, 16; j = 0..15); warp 9: the y ring (j = -1, 16; i = 0..15)
   int ii, jj;
-  if (tid < PS * FT) { jj = 1 + tid / FT; ii = tid - (jj - 1) * FT; }
+  if (tid < PS * PS) { jj = 1 + (tid >> 4); ii = 1 + (tid & 15); }
+  else if (tid < PS * PS + 32) { const int l = tid - PS * PS; jj = 1 + (l >> 1); ii = (l & 1) ? FT - 1 : 0; }
   else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
   const int col = jj * FT + ii;
   const bool in_i = ii >= 1 && ii <= PS, in_j = jj >= 1 && jj <= PS, interior = in_i && in_j;
   const int wb = (jj + GW - 1) * SWP + (ii + GW - 1);  // own index in a primitive plane
   // first-pass face jobs of phase D: own lower faces, plus the corner faces on lanes that have none
   int fxc = (ii >= 1) ? col : -1, fyc = (jj >= 1) ? col : -1;
-  if (tid == 0) fxc = FT - 1;                         // F*_x(f = 16, j = -1)
-  if (tid == FT) fxc = FT * FT - 1;                   // F*_x(f = 16, j = 16)
-  if (tid == PS * FT) fyc = (FT - 1) * FT;            // F*_y(i = -1, f = 16)
-  if (tid == PS * FT + 1) fyc = FT * FT - 1;          // F*_y(i = 16, f = 16)
+  if (ii == 0 && jj == 1) fxc = FT - 1;               // F*_x(f = 16, j = -1)
+  if (ii == 0 && jj == 2) fxc = FT * FT - 1;          // F*_x(f = 16, j = 16)
+  if (jj == 0 && ii == 1) fyc = (FT - 1) * FT;        // F*_y(i = -1, f = 16)
+  if (jj == 0 && ii == 2) fyc = FT * FT - 1;          // F*_y(i = 16, f = 16)
   // corner-state job of phase F: lanes 0..7 of warp 9: corner (l & 3), direction (l >> 2)
   const int cl = tid - PS * FT;
   const bool cjob = cl >= 0 && cl < 8;

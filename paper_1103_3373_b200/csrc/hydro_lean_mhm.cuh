@@ -87,8 +87,10 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   auto fld = [&](int k) { return xy + k * 5 * NC; };
 
   const int tid = threadIdx.x;
+  // warps 0-7: interior columns (two rows of 16 per warp); warp 8: x ring (i = -1, 16); warp 9: y ring (j = -1, 16)
   int ii, jj;
-  if (tid < PS * FT) { jj = 1 + tid / FT; ii = tid - (jj - 1) * FT; }
+  if (tid < PS * PS) { jj = 1 + (tid >> 4); ii = 1 + (tid & 15); }
+  else if (tid < PS * PS + 32) { const int l = tid - PS * PS; jj = 1 + (l >> 1); ii = (l & 1) ? FT - 1 : 0; }
   else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
   const int col = jj * FT + ii;
   const bool in_i = ii >= 1 && ii <= PS, in_j = jj >= 1 && jj <= PS, interior = in_i && in_j;

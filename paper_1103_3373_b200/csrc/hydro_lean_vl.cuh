@@ -55,8 +55,9 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
   // ---- stage-1 role: plus cell (ci, cj) in interior coordinates, or a boundary-face job of the extra warp
   int ci = 0, cj = 0;
   const bool cell = tid < NP;
-  if (tid < PS * FT) { cj = tid / FT; ci = tid - cj * FT - 1; }
-  else if (tid < 320) { const int l = tid - PS * FT; cj = (l < PS) ? -1 : PS; ci = l & (PS - 1); }
+  if (tid < PS * PS) { cj = tid >> 4; ci = tid & 15; }                                           // warps 0-7: interior columns
+  else if (tid < PS * PS + 32) { const int l = tid - PS * PS; cj = l >> 1; ci = (l & 1) ? PS : -1; }  // warp 8: x ring
+  else if (tid < 320) { const int l = tid - PS * FT; cj = (l < PS) ? -1 : PS; ci = l & (PS - 1); }    // warp 9: y ring
   else if (cell) {
     const int k = tid - 320, r = 2 + k / 64, arm = (k & 63) >> 4, pos = k & 15;
     ci = arm == 0 ? -r : (arm == 1 ? PS - 1 + r : pos);
