@@ -195,6 +195,8 @@ def run_table(args):
         return e0.elapsed_time(e1) / reps
 
     rows = []
+    if args.table == "peaks":
+        return run_peaks(args, B, dev)
     if args.table == "variants":
         Ng = 4096
         names, rn = {0: "MHM", 1: "VL", 2: "CTU"}, {0: "exact", 1: "HLLE", 2: "HLLC", 3: "Roe"}
@@ -239,6 +241,55 @@ def run_table(args):
     print(json.dumps({"table": "grid", "rows": rows}))
 
 
+def run_peaks(args, B, dev):
+    """--table peaks: MEASURED ALU peaks.  Register-resident loops of hydro_alu_peak_launch on all SMs
+    (4 CTAs x 512 threads per SM, 16 independent chains per thread), each kind run back to back for ~1 s under the
+    clock sampler and timed with CUDA events; the best 0.25 s window counts as the burst figure, the whole second as
+    the sustained one.  Writes profiles/alu_peaks.json (read by the bench line for roofline.peak)."""
+    import torch
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    blocks, threads, iters = sms * 4, 512, 2048
+    scratch = torch.empty(blocks * threads * 8, dtype=torch.uint8, device=dev)
+    out = {"table": "peaks", "gpu": torch.cuda.get_device_name(dev), "sms": sms, "blocks": blocks, "threads": threads,
+           "chains_per_thread": 16, "command": "python bench.py --table peaks", "kinds": {}}
+    for kind in ("ffma", "ffma_const", "ffma2", "fmul_fadd", "ffma_fmnmx", "ffma2_fmnmx", "dfma", "mufu"):
+        ops = B.hydro_alu_peak_launch(kind, blocks, threads, iters, scratch)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        B.hydro_alu_peak_launch(kind, blocks, threads, iters, scratch)
+        e1.record()
+        torch.cuda.synchronize()
+        one = e0.elapsed_time(e1) * 1e-3
+        n = max(8, int(1.0 / max(one, 1e-6)))
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(n + 1)]
+        sampler = ClockSampler(physical_gpu_index(dev.index or 0))
+        sampler.start()
+        evs[0].record()
+        for k in range(n):
+            B.hydro_alu_peak_launch(kind, blocks, threads, iters, scratch)
+            evs[k + 1].record()
+        torch.cuda.synchronize()
+        sampler.stop_flag = True
+        sampler.join()
+        ts = [evs[k].elapsed_time(evs[k + 1]) * 1e-3 for k in range(n)]
+        w = max(1, int(0.25 / max(one, 1e-6)))
+        burst = max(ops * w / sum(ts[k:k + w]) for k in range(0, n - w + 1))
+        out["kinds"][kind] = {"ops_per_launch": ops, "launches": n, "sustained_tops": ops * n / sum(ts) / 1e12,
+                              "burst_tops": burst / 1e12, "clocks": sampler.summary()}
+    k = out["kinds"]
+    out["fp32_tflops"] = max(k["ffma"]["sustained_tops"], k["ffma2"]["sustained_tops"], k["ffma_const"]["sustained_tops"])
+    out["fp32_tflops_ffma"] = k["ffma"]["sustained_tops"]
+    out["fp64_tflops"] = k["dfma"]["sustained_tops"]
+    out["nominal"] = {"fp32_tflops": sms * 128 * 2 * 1.965e9 / 1e12, "fp64_tflops": sms * 64 * 2 * 1.965e9 / 1e12,
+                      "rule": "SMs x 128 (64) FMA lanes x 2 x 1965 MHz"}
+    for d in ("profiles", "gpurun_out"):  # gpurun_out/ is what comes back from a GPU box; profiles/ is the committed copy
+        if os.path.isdir(os.path.join(ROOT, d)):
+            with open(os.path.join(ROOT, d, "alu_peaks.json"), "w") as f:
+                json.dump(out, f, indent=1)
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -249,7 +300,7 @@ def main():
     ap.add_argument("--ng", type=int, default=NG, help="patch groups per GPU (default: the config's 8192)")
     ap.add_argument("--kernel", default="auto", choices=("auto", "staged", "fused"))
     ap.add_argument("--no-extras", action="store_true", help="skip the e2e / cpu_baseline / f64 legs (profiling runs)")
-    ap.add_argument("--table", default=None, choices=("variants", "grid"),
+    ap.add_argument("--table", default=None, choices=("variants", "grid", "peaks"),
                     help="instead of the bench line: one JSON line with per-variant hydro_solve timings (4096 groups), or with the\n"
                          "uniform-grid kernels (gather / scatter bandwidth, whole-step rates); context for DESIGN.md, profiles/")
     args = ap.parse_args()

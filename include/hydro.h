@@ -167,6 +167,17 @@ HYDRO_API size_t hydro_workspace_bytes(int Ng, int precision_bytes, int scheme, 
 HYDRO_API size_t hydro_staged_workspace_bytes(int Ng, int precision_bytes, int scheme, int recon);
 HYDRO_API const char* hydro_strerror(int code);
 
+/* Measurement helper (the FP32 / FP64 ALU peaks the roofline fractions divide by must be MEASURED on
+ * the box): launches one register-resident loop of `blocks` x `threads` threads, each running `iters` passes of
+ * 8 x 16 independent operations of one kind, on `stream`; the caller times it with CUDA events.
+ *   kind 0 FFMA (register operands)   1 FFMA2 (fma.rn.f32x2)   2 DFMA   3 FMUL / FADD alternating
+ *        4 FFMA : FMNMX 1:1           5 FFMA2 : FMNMX 1:1      6 MUFU.RSQ   7 FFMA with constant-bank operands
+ * scratch: device buffer of >= blocks*threads*8 bytes (never written in practice); *ops_per_launch (host, may be NULL)
+ * receives the floating-point operations of the timed kind per launch (FMA = 2; for kinds 4, 5 those of the FMAs only;
+ * kind 6: MUFU operations).  Errors: HYDRO_E_ENUM, HYDRO_E_VALUE (threads not a multiple of 32 in [32,512]), HYDRO_E_NULL. */
+HYDRO_API int hydro_alu_peak_launch(int kind, int blocks, int threads, int iters, void* scratch, double* ops_per_launch,
+                                    hydro_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,8 @@ PS = 16
 EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64", "hydro_pipeline_create",
            "hydro_pipeline_destroy", "hydro_pipeline_solve_f32", "hydro_pipeline_solve_f64", "hydro_min_ghost",
            "hydro_solve_grid_f32", "hydro_solve_grid_f64", "hydro_gather_f32", "hydro_gather_f64", "hydro_scatter_f32", "hydro_scatter_f64",
-           "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror")
+           "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror",
+           "hydro_alu_peak_launch")
 
 
 class HydroOpts(C.Structure):
@@ -70,6 +71,7 @@ def lib():
         L.hydro_workspace_bytes.restype = sz
         L.hydro_staged_workspace_bytes.argtypes = [i, i, i, i]
         L.hydro_staged_workspace_bytes.restype = sz
+        L.hydro_alu_peak_launch.argtypes = [i, i, i, i, vp, C.POINTER(C.c_double), vp]
         L.hydro_strerror.argtypes = [i]
         L.hydro_strerror.restype = C.c_char_p
         _lib = L
@@ -194,6 +196,21 @@ def hydro_dt(u, gamma, norm=0, *, max_speed=None, stream=None):
     if rc != 0:
         raise HydroError(rc, "hydro_dt_" + sfx)
     return max_speed
+
+
+PEAK_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "fmul_fadd": 3, "ffma_fmnmx": 4, "ffma2_fmnmx": 5, "mufu": 6, "ffma_const": 7}
+
+
+def hydro_alu_peak_launch(kind, blocks, threads, iters, scratch, *, stream=None):
+    """hydro_alu_peak_launch: one launch of a register-resident ALU loop; returns its operation count (FMA = 2)."""
+    ops = C.c_double()
+    st = (stream or torch.cuda.current_stream(scratch.device)).cuda_stream
+    with torch.cuda.device(scratch.device):
+        rc = lib().hydro_alu_peak_launch(PEAK_KINDS[kind] if isinstance(kind, str) else kind, blocks, threads, iters,
+                                         scratch.data_ptr(), C.byref(ops), st)
+    if rc != 0:
+        raise HydroError(rc, "hydro_alu_peak_launch")
+    return ops.value
 
 
 BC_PERIODIC, BC_OUTFLOW = 0, 1
