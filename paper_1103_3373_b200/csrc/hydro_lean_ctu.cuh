@@ -1,20 +1,23 @@
 // hydro_lean_ctu.cuh -- "lean" fused z-marching CTU kernel (steps (1)-(5) in one launch).
 //
-// Design point (from the ncu captures of the first two fused kernels, profiles/): the path is bound by
-// instruction issue.  The single-role kernel needed 168 registers (11 warps per SM, issue slots half
-// empty); the warp-specialised one left its corrector group waiting 40 % of the time.  This kernel keeps
-// the column-per-thread z-march but holds only 15 carried values per thread in registers; everything
-// that crosses a phase boundary lives in shared memory, so that a 320-thread CTA fits in 96 registers and
-// about 108 KB of shared memory (fp32, PLM) and TWO CTAs (two patch groups) are resident per SM, each
-// hiding the other's barriers.  The arithmetic is the instruction-lean form of hydro_lean_math.cuh;
-// shared-memory fields use the packed "4+1" layout of hydro_ptx.cuh (2 instructions per 5-vector).
+// Design point (from the ncu captures, profiles/): the path is bound by instruction ISSUE, not by HBM and not by the
+// FMA pipe itself.  A column-per-thread z-march holds only 15 carried values per thread in registers; everything that
+// crosses a phase boundary lives in shared memory, so that a 320-thread CTA fits in 96 registers and about 108 KB of
+// shared memory (fp32, PLM) and TWO CTAs (two patch groups) are resident per SM, each hiding the other's barriers.
+// Round 2 ("instruction diet", profiles/r2_*): packed FFMA2 was measured NOT to relieve the issue port on B200
+// (profiles/r2_issue_probe.md), so the kernel instead strips everything that is not the method's arithmetic:
+//   * every shared-memory access is `[R + immediate]` off per-thread 32-bit shared addresses formed once per kernel
+//     (hydro_ptx.cuh Fld<>); the primitive-plane ring rotates by renaming three address registers;
+//   * the three thread roles are separate code paths selected once per warp (warps 0-7 interior columns, warp 8 the
+//     x ring, warp 9 the y ring), so that the interior path carries no role predicates;
+//   * the Roe fallback crosses its call by value (no local memory anywhere: hydro_lean_math.cuh);
+//   * one lane waits for the bulk copies and the next CTA barrier publishes them; the least loaded warp issues them.
 //
 // Thread -> column of the 18 x 18 tile (interior + one-cell ring): warps 0-7 own the 256 interior columns (two rows of
-// 16 per warp, so no lane idles in the interior-only work), warp 8 the x ring (i = -1, 16) and warp 9 the y ring
-// (j = -1, 16), which only do the work the ring needs.  The four corner columns only feed F*_x / F*_y of the ring;
-// their work rides on lanes that would otherwise idle: their traced states are formed by 8 lanes of warp 9 during
-// phase F of the previous step, their four first-pass Riemann problems by i = -1 lanes of warp 8 (F*_x) and
-// j = -1 lanes of warp 9 (F*_y) in phase D.
+// 16 per warp), warp 8 the x ring (i = -1, 16) and warp 9 the y ring (j = -1, 16), which only do the work the ring
+// needs.  The four corner columns only feed F*_x / F*_y of the ring; their work rides on lanes that would otherwise
+// idle: their traced states are formed by 8 lanes of warp 9 during phase F of the previous step, their four first-pass
+// Riemann problems by i = -1 lanes of warp 8 (F*_x) and j = -1 lanes of warp 9 (F*_y) in phase D.
 //
 // Step t = -2 .. 16 of a group (plane index; W = primitive planes in a ring, one plane converted per step):
 //   B  z: traced states of plane t+1 (own column of the ring planes) -> private slots;
@@ -35,7 +38,14 @@
 
 namespace hydro {
 
+#ifndef LEAN_ROLE_SPLIT
+#define LEAN_ROLE_SPLIT 0
+#endif
+#ifndef LEAN_ONE_WAITER
+#define LEAN_ONE_WAITER 1  // 1: one lane polls the plane's mbarrier before barrier 1; 0: every thread polls it in phase D
+#endif
 enum : int { LF_LOX = 0, LF_UPX, LF_LOY, LF_UPY, LF_FX, LF_FY };
+enum : int { ROLE_INT = 0, ROLE_XR = 1, ROLE_YR = 2, ROLE_ANY = 3 };  // ROLE_ANY: one code stream, roles decided at run time
 
 // variant seams: FAST = van Leer limiter on primitive variables, no floors (compile time)
 template <class R, int RECON, int RS, int FAST> struct LeanOps {
@@ -67,22 +77,42 @@ template <class R, int RECON, int RS, int FAST> struct LeanOps {
   }
 };
 
-template <class R, int RECON, int RS, int FAST, int MINB, int GRID>
-__global__ void __launch_bounds__(LEAN_NT, MINB)
-ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, Par<R> p,
-                const R* __restrict__ max_speed, R cfl, long long* status, GridIO<R> gio) {
+// what a role needs from the kernel prologue: pointers, geometry, shared-memory bases
+template <class R> struct LeanCtx {
+  const R* in; R* out; R* face_flux;
+  int Ng, g;
+  long long* status;
+  GridIO<R> gio;
+  uint32_t sm_bar, sm_ring, sm_zs, sm_xy, sm_raw;  // shared-space byte addresses
+  uint64_t* bar;
+  R* raw;
+};
+
+// The whole march of one role over this CTA's groups.  All roles execute the same sequence of CTA barriers.
+template <class R, int RECON, int RS, int FAST, int GRID, int ROLE>
+__device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>& p, int ii, int jj) {
   using Op = LeanOps<R, RECON, RS, FAST>;
   constexpr int GW = 2 + RECON, RW = 1 + RECON, SWP = PS + 2 * GW, WPL = SWP * SWP, NW = 2 * RW + 1, NPL = PS + 2 * GW;
   // PPM tiles are trimmed so that two fp32 CTAs (or one fp64 CTA) fit: one raw landing plane instead of two, and the
   // oldest plane of the z pencil (needed only at the thread's own column) carried in registers instead of the ring
   constexpr int NRAW = RECON == RECON_PPM ? 1 : 2, RC = RECON == RECON_PPM ? 1 : 0, NWS = NW - RC;  // == LEAN_NRAW, LEAN_RING_CARRY
   constexpr int NC = LEAN_COLS, NT = LEAN_NT, FT = PS + 2;
-  apply_device_dt(p, max_speed, cfl);
+  constexpr uint32_t ES = sizeof(R);
+  using FW = Fld<R, WPL>;  // a primitive plane of the ring
+  using FZ = Fld<R, NT>;   // a private traced-z field (one entry per thread)
+  using FC = Fld<R, NC>;   // an exchange field LOX .. FY (one entry per column)
+  // the column lies inside the interior range along x / y; with ROLE_ANY these are run-time flags of one code stream
+  // (three specialised streams cost more in instruction-cache misses than they save: profiles/r2_ctu_diet.md)
+  const bool in_i = ROLE == ROLE_ANY ? (ii >= 1 && ii <= PS) : ROLE != ROLE_XR;
+  const bool in_j = ROLE == ROLE_ANY ? (jj >= 1 && jj <= PS) : ROLE != ROLE_YR;
+  const bool INT = in_i && in_j, XR = !in_i, YR = !in_j;
 
+  const int g = cx.g;
   const int S = PS + 2 * g;
   const int SS = S * S;
   const size_t nS = (size_t)SS * S;
   const int off = g - GW;  // unused outer ghost layers (grid mode: g == GW)
+  const GridIO<R>& gio = cx.gio;
   // grid mode: cells per axis, plane / variable strides of the grids, boundary folding
   const int Nx = gio.Gx * PS, Ny = gio.Gy * PS, Nz = gio.Gz * PS;
   const size_t N2 = (size_t)Ny * Nx, N3 = N2 * Nz;
@@ -90,60 +120,61 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     return gio.bc == 0 ? (c < 0 ? c + N : (c >= N ? c - N : c)) : (c < 0 ? 0 : (c >= N ? N - 1 : c));
   };
 
-  // shared memory: everything at compile-time offsets; the raw planes, whose size depends on g, come last
-  extern __shared__ __align__(16) unsigned char smem[];
-  uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
-  R* ring = reinterpret_cast<R*>(smem + 64);           // [NWS] fields of WPL cells: primitive planes
-  R* zs = ring + NWS * 5 * WPL;                        // [2][2] fields of NT cells: private traced z states (lo, up) of planes t, t+1
-  R* xy = zs + 4 * 5 * NT;                             // [6] fields of NC cells: LOX UPX LOY UPY FX FY
-  R* raw = xy + 6 * 5 * NC;                            // [2][5][SS] landing zone of the bulk copies (SoA as in HBM)
-  auto fld = [&](int k) { return xy + k * 5 * NC; };
-
   const int tid = threadIdx.x;
-  // ---- column and role of this thread
-  // warps 0-7: the 256 interior columns (two rows of 16 per warp: no lane idles in the interior-only phases);
-  // warp 8: the x ring (i = -1, 16; j = 0..15); warp 9: the y ring (j = -1, 16; i = 0..15)
-  int ii, jj;
-  if (tid < PS * PS) { jj = 1 + (tid >> 4); ii = 1 + (tid & 15); }
-  else if (tid < PS * PS + 32) { const int l = tid - PS * PS; jj = 1 + (l >> 1); ii = (l & 1) ? FT - 1 : 0; }
-  else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
   const int col = jj * FT + ii;
-  const bool in_i = ii >= 1 && ii <= PS, in_j = jj >= 1 && jj <= PS, interior = in_i && in_j;
   const int wb = (jj + GW - 1) * SWP + (ii + GW - 1);  // own index in a primitive plane
-  // first-pass face jobs of phase D: own lower faces, plus the corner faces on lanes that have none
-  int fxc = (ii >= 1) ? col : -1, fyc = (jj >= 1) ? col : -1;
-  if (ii == 0 && jj == 1) fxc = FT - 1;               // F*_x(f = 16, j = -1)
-  if (ii == 0 && jj == 2) fxc = FT * FT - 1;          // F*_x(f = 16, j = 16)
-  if (jj == 0 && ii == 1) fyc = (FT - 1) * FT;        // F*_y(i = -1, f = 16)
-  if (jj == 0 && ii == 2) fyc = FT * FT - 1;          // F*_y(i = 16, f = 16)
+  // ---- per-thread shared addresses (vector part; the scalar part of the same cell sits at + d?s)
+  // own cell in the ring slots, oldest plane first: a per-thread base plus CTA-uniform slot offsets that rotate once per step
+  // (the rotation state lives in uniform registers; per-thread rotating addresses cost three more live registers)
+  const uint32_t w16 = cx.sm_ring + 16u * (uint32_t)wb;
+  uint32_t wo[NWS];
+#pragma unroll
+  for (int k = 0; k < NWS; ++k) wo[k] = (uint32_t)k * FW::BYTES;
+#define wv(k) (w16 + wo[k])
+  const uint32_t dws = FW::SD - (16u - ES) * (uint32_t)wb;
+  const uint32_t z16 = cx.sm_zs + 16u * (uint32_t)tid;
+  uint32_t zo = 0;                                           // uniform: parity slot [lo, up] read this step (the other is written)
+#define zcur (z16 + zo)
+#define znxt (z16 + (2u * FZ::BYTES - zo))
+  const uint32_t dzs = FZ::SD - (16u - ES) * (uint32_t)tid;
+  const uint32_t cv = cx.sm_xy + 16u * (uint32_t)col;
+  const uint32_t cs = cv + FC::SD - (16u - ES) * (uint32_t)col;
+  constexpr uint32_t CF = FC::BYTES;  // bytes per exchange field
+  // first-pass face jobs of phase D: own lower faces, plus (ring roles) the corner faces on lanes that have none
+  int fxc = (INT || ii >= 1) ? col : -1, fyc = (INT || jj >= 1) ? col : -1;
+  if (XR) {
+    if (ii == 0 && jj == 1) fxc = FT - 1;               // F*_x(f = 16, j = -1)
+    if (ii == 0 && jj == 2) fxc = FT * FT - 1;          // F*_x(f = 16, j = 16)
+  }
+  if (YR) {
+    if (jj == 0 && ii == 1) fyc = (FT - 1) * FT;        // F*_y(i = -1, f = 16)
+    if (jj == 0 && ii == 2) fyc = FT * FT - 1;          // F*_y(i = 16, f = 16)
+  }
+  const uint32_t fxv = cx.sm_xy + 16u * (uint32_t)fxc, fxs = fxv + FC::SD - (16u - ES) * (uint32_t)fxc;
+  const uint32_t fyv = cx.sm_xy + 16u * (uint32_t)fyc, fys = fyv + FC::SD - (16u - ES) * (uint32_t)fyc;
   // corner-state job of phase F: lanes 0..7 of warp 9: corner (l & 3), direction (l >> 2)
   const int cl = tid - PS * FT;
-  const bool cjob = cl >= 0 && cl < 8;
+  const bool cjob = YR && cl >= 0 && cl < 8;
   const int cdir = (cl >> 2) & 1;
   const int cci = (cl & 1) ? FT - 1 : 0, ccj = (cl & 2) ? FT - 1 : 0;
   const int ccol = ccj * FT + cci, cwb = (ccj + GW - 1) * SWP + (cci + GW - 1);
+  // the bulk copies are issued, and waited for, by one lane of the least loaded warp (warp 9, the y ring)
+  const bool feeder = YR && tid == PS * FT;
 
   // ---- plane pipeline: sequence number n = m * NPL + (plane + GW) over this CTA's groups m
-  const int my_groups = (Ng - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int my_groups = (cx.Ng - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int total_planes = my_groups * NPL;
-  auto issue = [&](int n) {  // thread 0 only
+  auto issue = [&](int n) {  // the feeder lane only
     if (n >= total_planes) return;
     const int m = n / NPL, pl = n - m * NPL;
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
-    const R* src = in + grp * 5 * nS + (size_t)(pl + off) * SS;
-    uint64_t* b = bar + (n % NRAW);
-    R* dst = raw + (size_t)(n % NRAW) * 5 * SS;
+    const R* src = cx.in + grp * 5 * nS + (size_t)(pl + off) * SS;
+    uint64_t* b = cx.bar + (n % NRAW);
+    R* dst = cx.raw + (size_t)(n % NRAW) * 5 * SS;
     mbar_expect_tx(b, (uint32_t)(5 * SS * sizeof(R)));
 #pragma unroll
     for (int q = 0; q < 5; ++q) bulk_g2s(dst + (size_t)q * SS, src + q * nS, (uint32_t)(SS * sizeof(R)), b);
   };
-  if (tid == 0) {
-    mbar_init(bar, 1);
-    mbar_init(bar + 1, 1);
-    fence_mbar_init();
-    fence_async_smem();
-  }
-  __syncthreads();
   // grid mode: every thread copies its share of raw plane n (element-wise async copies, ghost cells folded).  Planes are
   // fed strictly in sequence, so the (group, plane) of the next feed is running state, not a division of n.
   // (A variant with padded raw rows and 16-byte copies of the aligned interior cells measured 15 % slower.)
@@ -156,7 +187,7 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
       }
       const int x0 = (f_g & 1023) * PS - GW, y0 = ((f_g >> 10) & 1023) * PS - GW, z0 = (f_g >> 20) * PS - GW;
       const R* zsrc = gio.gin + (size_t)fold(z0 + f_pl, Nz) * N2;
-      R* dst = raw + (size_t)(n % NRAW) * 5 * (SWP * SWP);
+      R* dst = cx.raw + (size_t)(n % NRAW) * 5 * (SWP * SWP);
 #pragma unroll
       for (int r = 0; r < (SWP * SWP + NT - 1) / NT; ++r) {
         const int pos = tid + r * NT;
@@ -172,35 +203,51 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     cp_async_commit();  // also when empty: keeps the wait_group arithmetic uniform
   };
   if (GRID) { feed(0); if (NRAW > 1) feed(1); }
-  else if (tid == 0) { issue(0); if (NRAW > 1) issue(1); }
+  else if (feeder) { issue(0); if (NRAW > 1) issue(1); }
 
   Cnt c = {0, 0, 0};
   typename Bits<R>::U best = 0;  // running maximum of the updated cells' wave speed (next_max_speed)
   int nseq = 0;  // planes converted so far
-  // con->prim of the next raw plane into ring slot `slot` (all threads)
-  auto convert = [&](int slot) {
-    const int st = nseq % NRAW;
-    if (!GRID) mbar_wait(bar + st, (uint32_t)((nseq / NRAW) & 1));  // grid mode: waited for before the last barrier
-    const R* rp = raw + (size_t)st * 5 * SS;
-    R* wp = ring + slot * 5 * WPL;
-    for (int idx = tid; idx < WPL; idx += NT) {
-      const int b = idx / SWP, a = idx - b * SWP;
-      stv(wp, WPL, idx, Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c));
+  // the raw plane the next conversion reads has landed: one lane polls the mbarrier (grid mode: every thread waits for its
+  // own copies); the CTA barrier that follows publishes the plane to all threads
+  auto landed = [&]() {
+    if (GRID) cp_async_wait<NRAW - 1>();
+    else if (LEAN_ONE_WAITER && feeder) mbar_wait(cx.bar + (nseq % NRAW), (uint32_t)((nseq / NRAW) & 1));
+  };
+  // prologue form: no barrier follows before the conversion, so every thread observes the mbarrier itself
+  auto landed_all = [&]() {
+    if (GRID) { cp_async_wait<NRAW - 1>(); __syncthreads(); }
+    else mbar_wait(cx.bar + (nseq % NRAW), (uint32_t)((nseq / NRAW) & 1));
+  };
+  // con->prim of the next raw plane into the ring slot whose own-cell address is wslot (all threads; cells tid, tid + NT)
+  auto convert = [&](uint32_t wslot) {
+    const R* rp = cx.raw + (size_t)(nseq % NRAW) * 5 * SS;
+    const uint32_t base = wslot - 16u * (uint32_t)wb;  // start of the slot
+#pragma unroll
+    for (int r = 0; r < (WPL + NT - 1) / NT; ++r) {
+      const int idx = tid + r * NT;
+      if ((r + 1) * NT <= WPL || idx < WPL) {
+        const int b = idx / SWP, a = idx - b * SWP;
+        const V5<R> W = Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c);
+        FW::st(base + 16u * (uint32_t)idx, base + FW::SD + ES * (uint32_t)idx, W);
+      }
     }
   };
   // after the barrier that follows a conversion: refill the raw stage it consumed
   auto refill = [&]() {
     if (GRID) feed(nseq + NRAW);
-    else if (tid == 0) { fence_async_smem(); issue(nseq + NRAW); }
+    else if (feeder) { fence_async_smem(); issue(nseq + NRAW); }
     ++nseq;
   };
-  // traced states of a corner column of primitive plane `wpl` along x (cdir 0) or y (cdir 1)
-  auto corner_states = [&](const R* wpl) {
+  // traced states of a corner column of the primitive plane in slot `wslot` along x (cdir 0) or y (cdir 1)
+  auto corner_states = [&](uint32_t wslot) {
     const int st = cdir ? SWP : 1;
+    const uint32_t base = wslot - 16u * (uint32_t)wb;
     V5<R> W[2 * RW + 1];
 #pragma unroll
     for (int s = 0; s < 2 * RW + 1; ++s) {
-      const V5<R> w = ldv(wpl, WPL, cwb + (s - RW) * st);
+      const uint32_t i = (uint32_t)(cwb + (s - RW) * st);
+      const V5<R> w = FW::ld(base + 16u * i, base + FW::SD + ES * i);
       W[s][0] = w[0]; W[s][4] = w[4];
       W[s][1] = cdir ? w[2] : w[1];
       W[s][2] = cdir ? w[3] : w[2];
@@ -212,8 +259,9 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     lo[1] = cdir ? l[3] : l[1]; up[1] = cdir ? u[3] : u[1];
     lo[2] = cdir ? l[1] : l[2]; up[2] = cdir ? u[1] : u[2];
     lo[3] = cdir ? l[2] : l[3]; up[3] = cdir ? u[2] : u[3];
-    stv(fld(LF_LOX + 2 * cdir), NC, ccol, lo);
-    stv(fld(LF_UPX + 2 * cdir), NC, ccol, up);
+    const uint32_t v = cx.sm_xy + 16u * (uint32_t)ccol + (uint32_t)(2 * cdir) * CF, s = cx.sm_xy + FC::SD + ES * (uint32_t)ccol + (uint32_t)(2 * cdir) * CF;
+    FC::st(v + LF_LOX * CF, s + LF_LOX * CF, lo);
+    FC::st(v + LF_UPX * CF, s + LF_UPX * CF, up);
   };
 
   V5<R> f1z, uzc, Dz;  // F*_z at the lower face of plane t+1; corrected up_z of plane t-1; (dF_x + dF_y) - F_z of plane t-1
@@ -222,41 +270,43 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
 
   for (int m = 0; m < my_groups; ++m) {
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
-    // own cell of plane 0 in `in` / `out` (interior columns only)
-    const R* gin0 = in + grp * 5 * nS + ((size_t)g * S + (jj - 1 + g)) * S + (ii - 1 + g);
-    R* gout0 = out + grp * 5 * PS * PS * PS + (jj - 1) * PS + (ii - 1);
-    if (GRID) {  // U^n and the result live in the grids: plane stride N2, variable stride N3
-      const int gi = (int)grp, gx = gi % gio.Gx, gy = (gi / gio.Gx) % gio.Gy, gz = gi / (gio.Gx * gio.Gy);
-      const size_t cell = ((size_t)(gz * PS) * Ny + gy * PS + (jj - 1)) * Nx + gx * PS + (ii - 1);
-      gin0 = gio.gin + cell;
-      gout0 = gio.gout + cell;
+    // own cell of plane -1 in `in` / `out` (interior columns only); both advance by one plane per step from t = 0 on
+    const R* gin = cx.in;
+    R* gout = cx.out;
+    R* gff = nullptr;
+    if (INT) {
+      gin = cx.in + grp * 5 * nS + ((size_t)(g - 1) * S + (jj - 1 + g)) * S + (ii - 1 + g);
+      gout = cx.out + grp * 5 * PS * PS * PS + (jj - 1) * PS + (ii - 1) - PS * PS;
+      if (GRID) {  // U^n and the result live in the grids: plane stride N2, variable stride N3
+        const int gi = (int)grp, gx = gi % gio.Gx, gy = (gi / gio.Gx) % gio.Gy, gz = gi / (gio.Gx * gio.Gy);
+        const size_t cell = ((size_t)(gz * PS) * Ny + gy * PS + (jj - 1)) * Nx + gx * PS + (ii - 1);
+        gin = gio.gin + cell - N2;
+        gout = gio.gout + cell - N2;
+      }
     }
+    gff = cx.face_flux ? cx.face_flux + grp * 9 * 5 * PS * PS : nullptr;
     // ---- prologue: the first NW primitive planes (-GW .. -GW+NW-1)
     V5<R> Wold;  // RC: W(t+1-RW) at the thread's own column
     if (RC) {
-      if (GRID) { cp_async_wait<NRAW - 1>(); __syncthreads(); }
-      convert(0);
+      landed_all();
+      convert(wv(0));
       __syncthreads();
       refill();
-      Wold = ldv(ring, WPL, wb);
+      Wold = FW::ld(wv(0), wv(0) + dws);
       __syncthreads();
     }
+#pragma unroll
     for (int k = 0; k < NWS; ++k) {
-      if (GRID) { cp_async_wait<NRAW - 1>(); __syncthreads(); }
-      convert(k);
+      landed_all();
+      convert(wv(k));
       __syncthreads();
       refill();
     }
-    int sl = 0;  // ring slot of the oldest plane held in shared memory: plane t+1-RW+RC
 
 #pragma unroll 1
     for (int t = -2; t <= PS; ++t) {
       const bool doxy = t >= -1;
       const bool tin = t >= 0 && t < PS;
-      // ring slots of the planes this step touches
-      int slot[NW];
-#pragma unroll
-      for (int s = RC; s < NW; ++s) slot[s] = (sl + s - RC < NWS) ? sl + s - RC : sl + s - RC - NWS;
       // ================= B: z states of plane t+1, F*_z(t+1) =================
       V5<R> dFz;
 #pragma unroll
@@ -265,18 +315,17 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
         V5<R> Wz[NW];
 #pragma unroll
         for (int s = RC; s < NW; ++s) {
-          const V5<R> w = ldv(ring + slot[s] * 5 * WPL, WPL, wb);
+          const V5<R> w = FW::ld(wv(s - RC), wv(s - RC) + dws);
           if (RC && s == RC) { Wz[0] = to_normal<2>(Wold); Wold = w; }
           Wz[s] = to_normal<2>(w);
         }
         V5<R> l, u;
         Op::recon(Wz[0], Wz[RW - 1], Wz[RW], Wz[RW + 1], Wz[2 * RW], p, l, u);
         const V5<R> lz = from_normal<2>(l), uz = from_normal<2>(u);
-        R* zn = zs + ((t + 1) & 1) * 10 * NT;
-        stv(zn, NT, tid, lz);
-        stv(zn + 5 * NT, NT, tid, uz);
+        FZ::st(znxt, znxt + dzs, lz);
+        FZ::st(znxt + FZ::BYTES, znxt + FZ::BYTES + dzs, uz);
         if (t >= -1) {
-          const V5<R> uzp = ldv(zs + (t & 1) * 10 * NT + 5 * NT, NT, tid);
+          const V5<R> uzp = FZ::ld(zcur + FZ::BYTES, zcur + FZ::BYTES + dzs);
           const V5<R> f = Op::template riemann<2>(uzp, lz, p, c);
 #pragma unroll
           for (int q = 0; q < 5; ++q) { dFz[q] = f[q] - f1z[q]; f1z[q] = f[q]; }
@@ -284,61 +333,64 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
       }
       // ================= C: x,y traced states of plane t (slot RW-1 of the held planes) =================
       if (doxy) {
-        const R* wpl = ring + slot[RW - 1] * 5 * WPL;
-        const V5<R> W0 = ldv(wpl, WPL, wb);
+        const uint32_t w0 = wv(RW - 1 - RC), s0 = w0 + dws;
+        const V5<R> W0 = FW::ld(w0, s0);
         {
-          const V5<R> Wb = ldv(wpl, WPL, wb - 1), Wc = ldv(wpl, WPL, wb + 1);
+          const V5<R> Wb = FW::ld(w0 - 16u, s0 - ES), Wc = FW::ld(w0 + 16u, s0 + ES);
           V5<R> Wa = Wb, Wd = Wc;
-          if (RECON == RECON_PPM) { Wa = ldv(wpl, WPL, wb - 2); Wd = ldv(wpl, WPL, wb + 2); }
+          if (RECON == RECON_PPM) { Wa = FW::ld(w0 - 32u, s0 - 2 * ES); Wd = FW::ld(w0 + 32u, s0 + 2 * ES); }
           V5<R> l, u;
           Op::recon(to_normal<0>(Wa), to_normal<0>(Wb), to_normal<0>(W0), to_normal<0>(Wc), to_normal<0>(Wd), p, l, u);
-          stv(fld(LF_LOX), NC, col, from_normal<0>(l));
-          stv(fld(LF_UPX), NC, col, from_normal<0>(u));
+          FC::st(cv + LF_LOX * CF, cs + LF_LOX * CF, from_normal<0>(l));
+          FC::st(cv + LF_UPX * CF, cs + LF_UPX * CF, from_normal<0>(u));
         }
         {
-          const V5<R> Wb = ldv(wpl, WPL, wb - SWP), Wc = ldv(wpl, WPL, wb + SWP);
+          const V5<R> Wb = FW::ld(w0 - 16u * SWP, s0 - ES * SWP), Wc = FW::ld(w0 + 16u * SWP, s0 + ES * SWP);
           V5<R> Wa = Wb, Wd = Wc;
-          if (RECON == RECON_PPM) { Wa = ldv(wpl, WPL, wb - 2 * SWP); Wd = ldv(wpl, WPL, wb + 2 * SWP); }
+          if (RECON == RECON_PPM) { Wa = FW::ld(w0 - 32u * SWP, s0 - 2 * ES * SWP); Wd = FW::ld(w0 + 32u * SWP, s0 + 2 * ES * SWP); }
           V5<R> l, u;
           Op::recon(to_normal<1>(Wa), to_normal<1>(Wb), to_normal<1>(W0), to_normal<1>(Wc), to_normal<1>(Wd), p, l, u);
-          stv(fld(LF_LOY), NC, col, from_normal<1>(l));
-          stv(fld(LF_UPY), NC, col, from_normal<1>(u));
+          FC::st(cv + LF_LOY * CF, cs + LF_LOY * CF, from_normal<1>(l));
+          FC::st(cv + LF_UPY * CF, cs + LF_UPY * CF, from_normal<1>(u));
         }
       }
-      if (GRID) cp_async_wait<NRAW - 1>();  // the raw plane converted in D has landed (own copies; the barrier publishes all)
+      const bool conv = t + 2 + RW <= PS - 1 + GW;  // plane t+2+RW replaces plane t+1-RW (read for the last time in B / C)
+      if (conv) landed();  // the raw plane converted in D (the barrier publishes it)
       __syncthreads();  // barrier 1
 
       // ================= D: F*_x(t), F*_y(t); con->prim of the next plane =================
       if (doxy) {
-        if (fxc >= 0)
-          stv(fld(LF_FX), NC, fxc, Op::template riemann<0>(ldv(fld(LF_UPX), NC, fxc - 1), ldv(fld(LF_LOX), NC, fxc), p, c));
-        if (fyc >= 0)
-          stv(fld(LF_FY), NC, fyc, Op::template riemann<1>(ldv(fld(LF_UPY), NC, fyc - FT), ldv(fld(LF_LOY), NC, fyc), p, c));
+        if (INT || fxc >= 0)
+          FC::st(fxv + LF_FX * CF, fxs + LF_FX * CF,
+                 Op::template riemann<0>(FC::ld(fxv + LF_UPX * CF - 16u, fxs + LF_UPX * CF - ES), FC::ld(fxv + LF_LOX * CF, fxs + LF_LOX * CF), p, c));
+        if (INT || fyc >= 0)
+          FC::st(fyv + LF_FY * CF, fys + LF_FY * CF,
+                 Op::template riemann<1>(FC::ld(fyv + LF_UPY * CF - 16u * FT, fys + LF_UPY * CF - ES * FT), FC::ld(fyv + LF_LOY * CF, fys + LF_LOY * CF), p, c));
       }
-      const bool conv = t + 2 + RW <= PS - 1 + GW;  // plane t+2+RW replaces plane t+1-RW (read for the last time in B / C)
-      if (conv) convert(sl);  // the oldest shared-memory plane: last read in B / C of this step
+      if (!LEAN_ONE_WAITER && !GRID && conv) mbar_wait(cx.bar + (nseq % NRAW), (uint32_t)((nseq / NRAW) & 1));
+      if (conv) convert(wv(0));  // the oldest shared-memory plane: last read in B / C of this step
       __syncthreads();  // barrier 2
       if (conv) refill();
 
       // ================= E: transverse correction, F_z(t), update of plane t-1 =========
       if (doxy) {
         V5<R> Uold;
-        const bool upd = interior && t >= 1;
+        const bool upd = INT && t >= 1;
         if (upd) {
-          const R* gin = GRID ? gin0 + (size_t)(t - 1) * N2 : gin0 + (t - 1) * SS;
+          const R* gp = gin;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += GRID ? N3 : nS; }
+          for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gp); gp += GRID ? N3 : nS; }
         }
         V5<R> dFx, dFy;
 #pragma unroll
         for (int q = 0; q < 5; ++q) { dFx[q] = R(0); dFy[q] = R(0); }
         if (in_i) {
-          const V5<R> a = ldv(fld(LF_FX), NC, col + 1), b = ldv(fld(LF_FX), NC, col);
+          const V5<R> a = FC::ld(cv + LF_FX * CF + 16u, cs + LF_FX * CF + ES), b = FC::ld(cv + LF_FX * CF, cs + LF_FX * CF);
 #pragma unroll
           for (int q = 0; q < 5; ++q) dFx[q] = a[q] - b[q];
         }
         if (in_j) {
-          const V5<R> a = ldv(fld(LF_FY), NC, col + FT), b = ldv(fld(LF_FY), NC, col);
+          const V5<R> a = FC::ld(cv + LF_FY * CF + 16u * FT, cs + LF_FY * CF + ES * FT), b = FC::ld(cv + LF_FY * CF, cs + LF_FY * CF);
 #pragma unroll
           for (int q = 0; q < 5; ++q) dFy[q] = a[q] - b[q];
         }
@@ -346,26 +398,25 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
           V5<R> dq;
 #pragma unroll
           for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFy[q] + dFz[q]);
-          stv(fld(LF_LOX), NC, col, Op::correct(ldv(fld(LF_LOX), NC, col), dq, p, c));
-          stv(fld(LF_UPX), NC, col, Op::correct(ldv(fld(LF_UPX), NC, col), dq, p, c));
+          FC::st(cv + LF_LOX * CF, cs + LF_LOX * CF, Op::correct(FC::ld(cv + LF_LOX * CF, cs + LF_LOX * CF), dq, p, c));
+          FC::st(cv + LF_UPX * CF, cs + LF_UPX * CF, Op::correct(FC::ld(cv + LF_UPX * CF, cs + LF_UPX * CF), dq, p, c));
         }
         if (tin && in_i) {  // y states: t1 = z, t2 = x
           V5<R> dq;
 #pragma unroll
           for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFz[q] + dFx[q]);
-          stv(fld(LF_LOY), NC, col, Op::correct(ldv(fld(LF_LOY), NC, col), dq, p, c));
-          stv(fld(LF_UPY), NC, col, Op::correct(ldv(fld(LF_UPY), NC, col), dq, p, c));
+          FC::st(cv + LF_LOY * CF, cs + LF_LOY * CF, Op::correct(FC::ld(cv + LF_LOY * CF, cs + LF_LOY * CF), dq, p, c));
+          FC::st(cv + LF_UPY * CF, cs + LF_UPY * CF, Op::correct(FC::ld(cv + LF_UPY * CF, cs + LF_UPY * CF), dq, p, c));
         }
-        if (interior) {  // z states: t1 = x, t2 = y; every plane t in [-1,16]
+        if (INT) {  // z states: t1 = x, t2 = y; every plane t in [-1,16]
           V5<R> dq;
 #pragma unroll
           for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFx[q] + dFy[q]);
-          const R* zc = zs + (t & 1) * 10 * NT;
           if (t >= 0) {
-            const V5<R> lzc = Op::correct(ldv(zc, NT, tid), dq, p, c);
+            const V5<R> lzc = Op::correct(FZ::ld(zcur, zcur + dzs), dq, p, c);
             const V5<R> Fz = Op::template riemann<2>(uzc, lzc, p, c);
-            if (face_flux && (t & 7) == 0)  // stored right after the solve
-              st5(face_flux + grp * 9 * 5 * PS * PS + (size_t)((6 + (t >> 3)) * 5) * 256 + (jj - 1) * PS + (ii - 1), 256, Fz);
+            if (gff && (t & 7) == 0)  // stored right after the solve
+              st5(gff + (size_t)((6 + (t >> 3)) * 5) * 256 + (jj - 1) * PS + (ii - 1), 256, Fz);
             if (upd) {
               V5<R> U;
 #pragma unroll
@@ -374,50 +425,108 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
               if (p.next_speed) track_speed(Wn, p, best);
               if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
               if (GRID) {
-                R* d = gout0 + (size_t)(t - 1) * N2;
+                R* d = gout;
 #pragma unroll
                 for (int q = 0; q < 5; ++q) { *d = U[q]; d += N3; }
               } else {
-                st5(gout0 + (t - 1) * PS * PS, PS * PS * PS, U);
+                st5(gout, PS * PS * PS, U);
               }
             }
             Dz = Fz;
           }
-          if (t < PS) uzc = Op::correct(ldv(zc + 5 * NT, NT, tid), dq, p, c);
+          if (t < PS) uzc = Op::correct(FZ::ld(zcur + FZ::BYTES, zcur + FZ::BYTES + dzs), dq, p, c);
         }
       }
       __syncthreads();  // barrier 3
 
       // ================= F: final fluxes of plane t + boundary-flux store ============
       if (tin) {
-        R* gff = face_flux ? face_flux + grp * 9 * 5 * PS * PS : nullptr;
-        if (in_j && ii >= 1) {
-          const V5<R> f = Op::template riemann<0>(ldv(fld(LF_UPX), NC, col - 1), ldv(fld(LF_LOX), NC, col), p, c);
-          stv(fld(LF_FX), NC, col, f);
+        if (in_j && (INT || ii >= 1)) {
+          const V5<R> f = Op::template riemann<0>(FC::ld(cv + LF_UPX * CF - 16u, cs + LF_UPX * CF - ES), FC::ld(cv + LF_LOX * CF, cs + LF_LOX * CF), p, c);
+          FC::st(cv + LF_FX * CF, cs + LF_FX * CF, f);
           if (gff && ((ii - 1) & 7) == 0) st5(gff + (size_t)(((ii - 1) >> 3) * 5) * 256 + t * PS + (jj - 1), 256, f);
         }
-        if (in_i && jj >= 1) {
-          const V5<R> f = Op::template riemann<1>(ldv(fld(LF_UPY), NC, col - FT), ldv(fld(LF_LOY), NC, col), p, c);
-          stv(fld(LF_FY), NC, col, f);
+        if (in_i && (INT || jj >= 1)) {
+          const V5<R> f = Op::template riemann<1>(FC::ld(cv + LF_UPY * CF - 16u * FT, cs + LF_UPY * CF - ES * FT), FC::ld(cv + LF_LOY * CF, cs + LF_LOY * CF), p, c);
+          FC::st(cv + LF_FY * CF, cs + LF_FY * CF, f);
           if (gff && ((jj - 1) & 7) == 0) st5(gff + (size_t)((3 + ((jj - 1) >> 3)) * 5) * 256 + t * PS + (ii - 1), 256, f);
         }
       }
       // corner columns of plane t+1 (held in ring slot RW); their entries of LOX..UPY were last read in D
-      if (cjob && t < PS) corner_states(ring + slot[RW] * 5 * WPL);
+      if (YR && cjob && t < PS) corner_states(wv(RW - RC));
       __syncthreads();  // barrier 4
 
       // ================= G: carried x+y flux difference of plane t minus F_z(t) =================
-      if (tin && interior) {
-        const V5<R> x1 = ldv(fld(LF_FX), NC, col + 1), x0 = ldv(fld(LF_FX), NC, col);
-        const V5<R> y1 = ldv(fld(LF_FY), NC, col + FT), y0 = ldv(fld(LF_FY), NC, col);
+      if (INT && tin) {
+        const V5<R> x1 = FC::ld(cv + LF_FX * CF + 16u, cs + LF_FX * CF + ES), x0 = FC::ld(cv + LF_FX * CF, cs + LF_FX * CF);
+        const V5<R> y1 = FC::ld(cv + LF_FY * CF + 16u * FT, cs + LF_FY * CF + ES * FT), y0 = FC::ld(cv + LF_FY * CF, cs + LF_FY * CF);
 #pragma unroll
         for (int q = 0; q < 5; ++q) Dz[q] = ((x1[q] - x0[q]) + (y1[q] - y0[q])) - Dz[q];
       }
-      sl = (sl + 1 < NWS) ? sl + 1 : 0;
+      // next step: the ring slots rotate (the converted plane is now the newest), the z-state slots swap, U^n / out advance
+      {
+        const uint32_t w = wo[0];
+#pragma unroll
+        for (int k = 0; k + 1 < NWS; ++k) wo[k] = wo[k + 1];
+        wo[NWS - 1] = w;
+        zo = 2u * FZ::BYTES - zo;
+      }
+      if (INT && t >= 0) { gin += GRID ? N2 : (size_t)SS; gout += GRID ? N2 : (size_t)(PS * PS); }
     }
   }
-  flush_counters(c, status);
+  flush_counters(c, cx.status);
   flush_speed(best, p.next_speed);
+#undef wv
+#undef zcur
+#undef znxt
+}
+
+template <class R, int RECON, int RS, int FAST, int MINB, int GRID>
+__global__ void __launch_bounds__(LEAN_NT, MINB)
+ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, Par<R> p,
+                const R* __restrict__ max_speed, R cfl, long long* status, GridIO<R> gio) {
+  constexpr int GW = 2 + RECON, SWP = PS + 2 * GW, WPL = SWP * SWP, NW = 2 * (1 + RECON) + 1;
+  constexpr int RC = RECON == RECON_PPM ? 1 : 0, NWS = NW - RC;
+  constexpr int NC = LEAN_COLS, NT = LEAN_NT, FT = PS + 2;
+  apply_device_dt(p, max_speed, cfl);
+
+  // shared memory: everything at compile-time offsets; the raw planes, whose size depends on g, come last
+  extern __shared__ __align__(16) unsigned char smem[];
+  LeanCtx<R> cx;
+  cx.in = in; cx.out = out; cx.face_flux = face_flux; cx.Ng = Ng; cx.g = g; cx.status = status; cx.gio = gio;
+  cx.bar = reinterpret_cast<uint64_t*>(smem);          // [2]
+  R* ring = reinterpret_cast<R*>(smem + 64);           // [NWS] fields of WPL cells: primitive planes
+  R* zs = ring + NWS * 5 * WPL;                        // [2][2] fields of NT cells: private traced z states (lo, up) of planes t, t+1
+  R* xy = zs + 4 * 5 * NT;                             // [6] fields of NC cells: LOX UPX LOY UPY FX FY
+  cx.raw = xy + 6 * 5 * NC;                            // [2][5][SS] landing zone of the bulk copies (SoA as in HBM)
+  cx.sm_bar = smem_u32(smem);
+  cx.sm_ring = smem_u32(ring);
+  cx.sm_zs = smem_u32(zs);
+  cx.sm_xy = smem_u32(xy);
+  cx.sm_raw = smem_u32(cx.raw);
+
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    mbar_init(cx.bar, 1);
+    mbar_init(cx.bar + 1, 1);
+    fence_mbar_init();
+    fence_async_smem();
+  }
+  __syncthreads();
+  // ---- column and role of this thread
+  // warps 0-7: the 256 interior columns (two rows of 16 per warp: no lane idles in the interior-only phases);
+  // warp 8: the x ring (i = -1, 16; j = 0..15); warp 9: the y ring (j = -1, 16; i = 0..15)
+  int ii, jj;
+  if (tid < PS * PS) { jj = 1 + (tid >> 4); ii = 1 + (tid & 15); }
+  else if (tid < PS * PS + 32) { const int l = tid - PS * PS; jj = 1 + (l >> 1); ii = (l & 1) ? FT - 1 : 0; }
+  else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
+  if (LEAN_ROLE_SPLIT) {
+    if (tid < PS * PS) ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_INT>(cx, p, ii, jj);
+    else if (tid < PS * PS + 32) ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_XR>(cx, p, ii, jj);
+    else ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_YR>(cx, p, ii, jj);
+  } else {
+    ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_ANY>(cx, p, ii, jj);
+  }
 }
 
 // persistent grid: SMs x resident CTAs per SM (occupancy API), capped at Ng

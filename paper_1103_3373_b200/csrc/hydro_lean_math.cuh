@@ -263,13 +263,35 @@ template <class R> __device__ __forceinline__ LeanState<R> lean_state(const V5<R
   return s;
 }
 
-// the rare path: Roe failed at this face -> HLLE / HLLC / exact flux of the same states
-template <class R> __device__ __noinline__ void roe_fallback_flux(const V5<R>* WL, const V5<R>* WR, const Par<R>* p, int* cnt_exact, V5<R>* F) {
+// the rare path: Roe failed at this face -> HLLE / HLLC / exact flux of the same states.  Everything
+// crosses the call by value (registers): a pointer argument would put the caller's states AND its flux on the stack
+// in the hot path (23.5 M local stores per launch in the round-1 kernel).
+template <class R> struct FluxRet { R f0, f1, f2, f3, f4; int ex; };
+template <class R>
+__device__ __noinline__ FluxRet<R> roe_fallback_flux(R l0, R l1, R l2, R l3, R l4, R r0, R r1, R r2, R r3, R r4, R gamma, R gm1,
+                                                     R igm1, int mode) {
+  Par<R> p;
+  p.gamma = gamma; p.gm1 = gm1; p.igm1 = igm1; p.roe_fallback = mode;
+  p.nu = p.hnu = p.theta = p.min_dens = p.min_pres = R(0);
+  p.limiter = p.char_limit = p.next_norm = 0;
+  p.next_speed = nullptr;
+  V5<R> WL, WR, F;
+  WL[0] = l0; WL[1] = l1; WL[2] = l2; WL[3] = l3; WL[4] = l4;
+  WR[0] = r0; WR[1] = r1; WR[2] = r2; WR[3] = r3; WR[4] = r4;
   Cnt c = {0, 0, 0};
-  if (p->roe_fallback == 2) *F = hllc(*WL, *WR, *p);
-  else if (p->roe_fallback == 3) *F = exact(*WL, *WR, *p, c);
-  else *F = hlle(*WL, *WR, *p);
-  *cnt_exact += c.exact;
+  if (mode == 2) F = hllc(WL, WR, p);
+  else if (mode == 3) F = exact(WL, WR, p, c);
+  else F = hlle(WL, WR, p);
+  FluxRet<R> r = {F[0], F[1], F[2], F[3], F[4], c.exact};
+  return r;
+}
+
+// fp64: thirteen doubles by value are 26 argument registers at every call site; there the two states cross by pointer (copied
+// to the stack inside the cold branch only) and just the flux comes back by value
+template <class R>
+__device__ __noinline__ FluxRet<R> roe_fallback_flux_p(const V5<R>* WL, const V5<R>* WR, R gamma, R gm1, R igm1, int mode) {
+  return roe_fallback_flux<R>((*WL)[0], (*WL)[1], (*WL)[2], (*WL)[3], (*WL)[4], (*WR)[0], (*WR)[1], (*WR)[2], (*WR)[3], (*WR)[4],
+                              gamma, gm1, igm1, mode);
 }
 
 // branch-free core: the Roe flux and whether both intermediate states passed the failure test.  Keeping the
@@ -320,10 +342,15 @@ template <class R> __device__ __forceinline__ bool lean_roe_core(const V5<R>& WL
 // Roe failed at this face: count it and replace the flux by the fallback solver's
 template <class R> __device__ __forceinline__ void lean_roe_failed(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c, V5<R>& F) {
   c.roe_fb++;
-  V5<R> l = WL, r = WR;  // copies: only this branch puts its arguments on the stack
-  int ex = 0;
-  roe_fallback_flux(&l, &r, &p, &ex, &F);
-  c.exact += ex;
+  FluxRet<R> r;
+  if (sizeof(R) == 4) {
+    r = roe_fallback_flux<R>(WL[0], WL[1], WL[2], WL[3], WL[4], WR[0], WR[1], WR[2], WR[3], WR[4], p.gamma, p.gm1, p.igm1, p.roe_fallback);
+  } else {
+    V5<R> l = WL, rr = WR;  // copies: only this branch puts its arguments on the stack
+    r = roe_fallback_flux_p<R>(&l, &rr, p.gamma, p.gm1, p.igm1, p.roe_fallback);
+  }
+  F[0] = r.f0; F[1] = r.f1; F[2] = r.f2; F[3] = r.f3; F[4] = r.f4;
+  c.exact += r.ex;
 }
 template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
   V5<R> F;

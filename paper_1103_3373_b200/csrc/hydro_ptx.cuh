@@ -87,4 +87,43 @@ __device__ __forceinline__ void stv(double* f, int N, int i, const V5<double>& x
   f[4 * N + i] = x[4];
 }
 
+
+// The same packed fields addressed by 32-bit shared-space byte addresses, so that every access of the fused kernels is
+// `LDS/STS [R + immediate]` off a per-thread address register formed once per kernel (no per-access index arithmetic):
+// v = address of the thread's 16-byte vector part, s = address of its scalar part; N = cells per field (compile time).
+// A neighbour k cells away is (v + 16 k, s + k sizeof(R)); the scalar part of cell i sits at s = v + Fld::SD - (16 - sizeof(R)) i.
+template <class R, int N> struct Fld;
+// plain C++ accesses through shared-window pointers rebuilt from the 32-bit addresses: the compiler keeps its freedom to
+// hoist and batch the loads of a phase (inline-asm accesses serialised them: 3.0 -> 3.9 ms) and still emits LDS/STS [R + imm]
+template <class T> __device__ __forceinline__ T* sm_ptr(uint32_t a) { return static_cast<T*>(__cvta_shared_to_generic((size_t)a)); }
+template <int N> struct Fld<float, N> {
+  static constexpr uint32_t SD = 16u * N;  // scalar part of cell 0 relative to its vector part
+  static constexpr uint32_t BYTES = 20u * N;
+  static __device__ __forceinline__ V5<float> ld(uint32_t v, uint32_t s) {
+    const float4 a = *sm_ptr<const float4>(v);
+    V5<float> x;
+    x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = *sm_ptr<const float>(s);
+    return x;
+  }
+  static __device__ __forceinline__ void st(uint32_t v, uint32_t s, const V5<float>& x) {
+    *sm_ptr<float4>(v) = make_float4(x[0], x[1], x[2], x[3]);
+    *sm_ptr<float>(s) = x[4];
+  }
+};
+template <int N> struct Fld<double, N> {
+  static constexpr uint32_t SD = 32u * N;
+  static constexpr uint32_t BYTES = 40u * N;
+  static __device__ __forceinline__ V5<double> ld(uint32_t v, uint32_t s) {
+    const double2 a = *sm_ptr<const double2>(v), b = *sm_ptr<const double2>(v + 16u * N);
+    V5<double> x;
+    x[0] = a.x; x[1] = a.y; x[2] = b.x; x[3] = b.y; x[4] = *sm_ptr<const double>(s);
+    return x;
+  }
+  static __device__ __forceinline__ void st(uint32_t v, uint32_t s, const V5<double>& x) {
+    *sm_ptr<double2>(v) = make_double2(x[0], x[1]);
+    *sm_ptr<double2>(v + 16u * N) = make_double2(x[2], x[3]);
+    *sm_ptr<double>(s) = x[4];
+  }
+};
+
 }  // namespace hydro
