@@ -67,6 +67,23 @@ template <class R, int RECON, int RS, int FAST> struct LeanOps {
     else if (FAST) lean_ppm_trace(Wm2, Wm1, W0, Wp1, Wp2, p, p.nu, lo, up);
     else reconstruct<RECON, true>(Wm2, Wm1, W0, Wp1, Wp2, p, lo, up);
   }
+  // trackers of non-positive states other than the per-conversion count (hydro_lean_math.cuh BadMin)
+  template <class T> static __device__ __forceinline__ V5<R> c2p(const V5<R>& U, const Par<R>& p, Cnt& c, T& trk) {
+    if (FAST) return lean_cons2prim(U, p, trk);
+    return cons2prim(U, p, c);
+  }
+  template <class T> static __device__ __forceinline__ V5<R> correct(const V5<R>& W, const V5<R>& dq, const Par<R>& p, Cnt& c, T& trk) {
+    if (FAST) return lean_correct(W, dq, p, trk);
+    return correct(W, dq, p, c);
+  }
+  // the flux times `scale` (the CTU first pass wants nu/2 F*: free inside the lean Roe solver)
+  template <int D> static __device__ __forceinline__ V5<R> riemann_scaled(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c, R scale) {
+    if (FAST && RS == RS_ROE) return from_normal<D>(lean_roe_scaled(to_normal<D>(WL), to_normal<D>(WR), p, c, scale));
+    V5<R> F = riemann<D>(WL, WR, p, c);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) F[q] = scale * F[q];
+    return F;
+  }
   template <int D> static __device__ __forceinline__ V5<R> riemann(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
     const V5<R> l = to_normal<D>(WL), r = to_normal<D>(WR);
     if (FAST && RS == RS_ROE) return from_normal<D>(lean_roe(l, r, p, c));
@@ -206,6 +223,8 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
   else if (feeder) { issue(0); if (NRAW > 1) issue(1); }
 
   Cnt c = {0, 0, 0};
+  typename BadTrk<R>::type trk;  // non-positive rho / P seen by the conversions of this step (flushed into c.bad once per step)
+  trk_reset(trk);
   typename Bits<R>::U best = 0;  // running maximum of the updated cells' wave speed (next_max_speed)
   int nseq = 0;  // planes converted so far
   // the raw plane the next conversion reads has landed: one lane polls the mbarrier (grid mode: every thread waits for its
@@ -228,7 +247,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
       const int idx = tid + r * NT;
       if ((r + 1) * NT <= WPL || idx < WPL) {
         const int b = idx / SWP, a = idx - b * SWP;
-        const V5<R> W = Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c);
+        const V5<R> W = Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c, trk);
         FW::st(base + 16u * (uint32_t)idx, base + FW::SD + ES * (uint32_t)idx, W);
       }
     }
@@ -326,7 +345,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
         FZ::st(znxt + FZ::BYTES, znxt + FZ::BYTES + dzs, uz);
         if (t >= -1) {
           const V5<R> uzp = FZ::ld(zcur + FZ::BYTES, zcur + FZ::BYTES + dzs);
-          const V5<R> f = Op::template riemann<2>(uzp, lz, p, c);
+          const V5<R> f = Op::template riemann_scaled<2>(uzp, lz, p, c, p.hnu);  // nu/2 F*_z
 #pragma unroll
           for (int q = 0; q < 5; ++q) { dFz[q] = f[q] - f1z[q]; f1z[q] = f[q]; }
         }
@@ -362,10 +381,10 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
       if (doxy) {
         if (INT || fxc >= 0)
           FC::st(fxv + LF_FX * CF, fxs + LF_FX * CF,
-                 Op::template riemann<0>(FC::ld(fxv + LF_UPX * CF - 16u, fxs + LF_UPX * CF - ES), FC::ld(fxv + LF_LOX * CF, fxs + LF_LOX * CF), p, c));
+                 Op::template riemann_scaled<0>(FC::ld(fxv + LF_UPX * CF - 16u, fxs + LF_UPX * CF - ES), FC::ld(fxv + LF_LOX * CF, fxs + LF_LOX * CF), p, c, p.hnu));
         if (INT || fyc >= 0)
           FC::st(fyv + LF_FY * CF, fys + LF_FY * CF,
-                 Op::template riemann<1>(FC::ld(fyv + LF_UPY * CF - 16u * FT, fys + LF_UPY * CF - ES * FT), FC::ld(fyv + LF_LOY * CF, fys + LF_LOY * CF), p, c));
+                 Op::template riemann_scaled<1>(FC::ld(fyv + LF_UPY * CF - 16u * FT, fys + LF_UPY * CF - ES * FT), FC::ld(fyv + LF_LOY * CF, fys + LF_LOY * CF), p, c, p.hnu));
       }
       if (!LEAN_ONE_WAITER && !GRID && conv) mbar_wait(cx.bar + (nseq % NRAW), (uint32_t)((nseq / NRAW) & 1));
       if (conv) convert(wv(0));  // the oldest shared-memory plane: last read in B / C of this step
@@ -397,23 +416,23 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
         if (tin && in_j) {  // x states: t1 = y, t2 = z
           V5<R> dq;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFy[q] + dFz[q]);
-          FC::st(cv + LF_LOX * CF, cs + LF_LOX * CF, Op::correct(FC::ld(cv + LF_LOX * CF, cs + LF_LOX * CF), dq, p, c));
-          FC::st(cv + LF_UPX * CF, cs + LF_UPX * CF, Op::correct(FC::ld(cv + LF_UPX * CF, cs + LF_UPX * CF), dq, p, c));
+          for (int q = 0; q < 5; ++q) dq[q] = dFy[q] + dFz[q];  // the first-pass fluxes carry the factor nu/2
+          FC::st(cv + LF_LOX * CF, cs + LF_LOX * CF, Op::correct(FC::ld(cv + LF_LOX * CF, cs + LF_LOX * CF), dq, p, c, trk));
+          FC::st(cv + LF_UPX * CF, cs + LF_UPX * CF, Op::correct(FC::ld(cv + LF_UPX * CF, cs + LF_UPX * CF), dq, p, c, trk));
         }
         if (tin && in_i) {  // y states: t1 = z, t2 = x
           V5<R> dq;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFz[q] + dFx[q]);
-          FC::st(cv + LF_LOY * CF, cs + LF_LOY * CF, Op::correct(FC::ld(cv + LF_LOY * CF, cs + LF_LOY * CF), dq, p, c));
-          FC::st(cv + LF_UPY * CF, cs + LF_UPY * CF, Op::correct(FC::ld(cv + LF_UPY * CF, cs + LF_UPY * CF), dq, p, c));
+          for (int q = 0; q < 5; ++q) dq[q] = dFz[q] + dFx[q];
+          FC::st(cv + LF_LOY * CF, cs + LF_LOY * CF, Op::correct(FC::ld(cv + LF_LOY * CF, cs + LF_LOY * CF), dq, p, c, trk));
+          FC::st(cv + LF_UPY * CF, cs + LF_UPY * CF, Op::correct(FC::ld(cv + LF_UPY * CF, cs + LF_UPY * CF), dq, p, c, trk));
         }
         if (INT) {  // z states: t1 = x, t2 = y; every plane t in [-1,16]
           V5<R> dq;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) dq[q] = p.hnu * (dFx[q] + dFy[q]);
+          for (int q = 0; q < 5; ++q) dq[q] = dFx[q] + dFy[q];
           if (t >= 0) {
-            const V5<R> lzc = Op::correct(FZ::ld(zcur, zcur + dzs), dq, p, c);
+            const V5<R> lzc = Op::correct(FZ::ld(zcur, zcur + dzs), dq, p, c, trk);
             const V5<R> Fz = Op::template riemann<2>(uzc, lzc, p, c);
             if (gff && (t & 7) == 0)  // stored right after the solve
               st5(gff + (size_t)((6 + (t >> 3)) * 5) * 256 + (jj - 1) * PS + (ii - 1), 256, Fz);
@@ -421,7 +440,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
               V5<R> U;
 #pragma unroll
               for (int q = 0; q < 5; ++q) U[q] = Uold[q] - p.nu * (Dz[q] + Fz[q]);
-              const V5<R> Wn = Op::c2p(U, p, c);
+              const V5<R> Wn = Op::c2p(U, p, c, trk);
               if (p.next_speed) track_speed(Wn, p, best);
               if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
               if (GRID) {
@@ -434,7 +453,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
             }
             Dz = Fz;
           }
-          if (t < PS) uzc = Op::correct(FZ::ld(zcur + FZ::BYTES, zcur + FZ::BYTES + dzs), dq, p, c);
+          if (t < PS) uzc = Op::correct(FZ::ld(zcur + FZ::BYTES, zcur + FZ::BYTES + dzs), dq, p, c, trk);
         }
       }
       __syncthreads();  // barrier 3
@@ -470,6 +489,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
         for (int k = 0; k + 1 < NWS; ++k) wo[k] = wo[k + 1];
         wo[NWS - 1] = w;
         zo = 2u * FZ::BYTES - zo;
+        c.bad += trk_flush(trk);
       }
       if (INT && t >= 0) { gin += GRID ? N2 : (size_t)SS; gout += GRID ? N2 : (size_t)(PS * PS); }
     }

@@ -70,8 +70,25 @@ __device__ __forceinline__ double l_sqrt(double x) {
 #endif
 
 // ---- c0: conversions --------------------------------------------------------------------------
-// rho |v|^2 is formed as m . v (3 instructions); `bad` counts non-positive rho / P (status[1])
-template <class R> __device__ __forceinline__ V5<R> lean_cons2prim(const V5<R>& U, const Par<R>& p, int& bad) {
+// non-positive rho / P seen by a conversion (status[1]).  `int&`: one count per conversion.  `BadMin&` (the fp32 CTU kernel,
+// which is bound by instruction issue): a NaN-propagating running minimum of every rho and P converted -- one FMNMX3.NAN
+// instead of two compares and an add -- tested and reset once per plane step, so there status[1] counts (thread, step)
+// pairs that met a bad state: non-zero exactly when the per-conversion count is.
+struct BadMin { float mn; };
+__device__ __forceinline__ void note_state(int& bad, float rho, float P) { bad += (rho > 0.f && P > 0.f) ? 0 : 1; }
+__device__ __forceinline__ void note_state(int& bad, double rho, double P) { bad += (rho > 0.0 && P > 0.0) ? 0 : 1; }
+__device__ __forceinline__ void note_state(BadMin& b, float rho, float P) {
+  asm("min.NaN.f32 %0, %0, %1, %2;" : "+f"(b.mn) : "f"(rho), "f"(P));
+}
+template <class R> struct BadTrk { using type = int; };
+template <> struct BadTrk<float> { using type = BadMin; };
+__device__ __forceinline__ void trk_reset(int& t) { t = 0; }
+__device__ __forceinline__ void trk_reset(BadMin& t) { t.mn = 1.0f; }
+__device__ __forceinline__ int trk_flush(int& t) { const int n = t; t = 0; return n; }
+__device__ __forceinline__ int trk_flush(BadMin& t) { const int n = (t.mn > 0.0f) ? 0 : 1; t.mn = 1.0f; return n; }
+
+// rho |v|^2 is formed as m . v (3 instructions)
+template <class R, class T> __device__ __forceinline__ V5<R> lean_cons2prim(const V5<R>& U, const Par<R>& p, T& bad) {
   const R ir = l_rcp(U[0]);
   V5<R> W;
   W[0] = U[0];
@@ -80,12 +97,12 @@ template <class R> __device__ __forceinline__ V5<R> lean_cons2prim(const V5<R>& 
   W[3] = U[3] * ir;
   const R mv = m_fma(U[3], W[3], m_fma(U[2], W[2], U[1] * W[1]));
   W[4] = p.gm1 * m_fma(R(-0.5), mv, U[4]);
-  bad += (U[0] > R(0) && W[4] > R(0)) ? 0 : 1;
+  note_state(bad, U[0], W[4]);
   return W;
 }
 
 // transverse correction of one face state: W <- prim(cons(W) - dq)
-template <class R> __device__ __forceinline__ V5<R> lean_correct(const V5<R>& W, const V5<R>& dq, const Par<R>& p, int& bad) {
+template <class R, class T> __device__ __forceinline__ V5<R> lean_correct(const V5<R>& W, const V5<R>& dq, const Par<R>& p, T& bad) {
   V5<R> U;
   U[0] = W[0] - dq[0];
   U[1] = m_fma(W[0], W[1], -dq[1]);
@@ -123,30 +140,37 @@ template <class R> __device__ __forceinline__ R vl_slope(R dL, R dR) {
   const R s = l_div(prod + prod, dL + dR);
   return prod > R(0) ? s : R(0);  // S19; the select also discards inf/NaN of the unused quotient
 }
+// HALF the van Leer slope, dL dR / (dL + dR): the factor 2 moves into the (compile-time or per-cell) coefficients that
+// multiply the slope, which is exact in binary arithmetic -- results are bitwise those of vl_slope, with one add less per slope
+template <class R> __device__ __forceinline__ R vl_half_slope(R dL, R dR) {
+  const R prod = dL * dR;
+  const R s = l_div(prod, dL + dR);
+  return prod > R(0) ? s : R(0);
+}
 
 template <class R>
 __device__ __forceinline__ void lean_plm_trace(const V5<R>& Wm, const V5<R>& W0, const V5<R>& Wp, const Par<R>& p, R nu, R hnu,
                                                V5<R>& lo, V5<R>& up) {
-  V5<R> s;
+  V5<R> s;  // HALF slopes (vl_half_slope); every coefficient below carries the factor 2
 #pragma unroll
-  for (int q = 0; q < 5; ++q) s[q] = vl_slope(W0[q] - Wm[q], Wp[q] - W0[q]);
+  for (int q = 0; q < 5; ++q) s[q] = vl_half_slope(W0[q] - Wm[q], Wp[q] - W0[q]);
   // eigen-system scalars from one rsqrt: irc = 1/(rho c), c = gamma P irc, 1/c = rho irc
   const R gP = p.gamma * W0[4], x = gP * W0[0];
   const R irc = l_rsqrt(x);
   const R c = gP * irc, ic = W0[0] * irc, ic2 = ic * ic, rc = x * irc;
   const R u = W0[1], lamM = u + c, lam0 = u - c;
-  const R nc = nu * c, hnc = R(0.5) * nc;
+  const R nc = nu * c;
   // S5 / S19: only waves approaching the face, lambda = 0 contributes to neither
-  const R b0 = lam0 > R(0) ? nc : R(0);     // (nu/2)(lamM - lam0)
-  const R b1 = u > R(0) ? hnc : R(0);       // (nu/2)(lamM - u)
-  const R g1 = u < R(0) ? -hnc : R(0);      // (nu/2)(lam0 - u)
+  const R b0 = lam0 > R(0) ? nc : R(0);     // (nu/2)(lamM - lam0), applied to a FULL amplitude below
+  const R b1 = u > R(0) ? nc : R(0);        // 2 (nu/2)(lamM - u)
+  const R g1 = u < R(0) ? -nc : R(0);       // 2 (nu/2)(lam0 - u)
   const R g4 = lamM < R(0) ? -nc : R(0);    // (nu/2)(lam0 - lamM)
-  const R kp = m_fma(-hnu, m_max(lamM, R(0)), R(0.5));
-  const R km = m_fma(-hnu, m_min(lam0, R(0)), R(-0.5));
-  const R Z = rc * s[1];                          // rho c du
-  const R B0 = b0 * (R(0.5) * (s[4] - Z));        // coefficient x (L_0 . s) c^2
-  const R B4 = g4 * (R(0.5) * (s[4] + Z));
-  const R e1 = m_fma(-s[4], ic2, s[0]);           // entropy-wave amplitude
+  const R kp = m_fma(-nu, m_max(lamM, R(0)), R(1));   // 2 (1/2 - (nu/2) max(lamM, 0))
+  const R km = m_fma(-nu, m_min(lam0, R(0)), R(-1));
+  const R Z = rc * s[1];                          // rho c du / 2
+  const R B0 = b0 * (s[4] - Z);                   // coefficient x (L_0 . s) c^2: half slopes give (dP - rho c du) / 2 directly
+  const R B4 = g4 * (s[4] + Z);
+  const R e1 = m_fma(-s[4], ic2, s[0]);           // half the entropy-wave amplitude
   up[0] = m_fma(B0, ic2, m_fma(b1, e1, m_fma(kp, s[0], W0[0])));
   up[1] = m_fma(-B0, irc, m_fma(kp, s[1], W0[1]));
   up[2] = m_fma(kp + b1, s[2], W0[2]);
@@ -168,9 +192,9 @@ __device__ __forceinline__ void lean_ppm_parabola(const V5<R>& Wm2, const V5<R>&
   for (int q = 0; q < 5; ++q) {
     const R w0 = W0[q];
     const R dLm = Wm1[q] - Wm2[q], dL = w0 - Wm1[q], dR = Wp1[q] - w0, dRp = Wp2[q] - Wp1[q];
-    const R sm = vl_slope(dLm, dL), s0 = vl_slope(dL, dR), sp = vl_slope(dR, dRp);
-    R wl = m_fma(R(-1.0 / 6.0), s0 - sm, R(0.5) * (Wm1[q] + w0));
-    R wr = m_fma(R(-1.0 / 6.0), sp - s0, R(0.5) * (w0 + Wp1[q]));
+    const R sm = vl_half_slope(dLm, dL), s0 = vl_half_slope(dL, dR), sp = vl_half_slope(dR, dRp);  // half slopes: -1/6 -> -1/3
+    R wl = m_fma(R(-1.0 / 3.0), s0 - sm, R(0.5) * (Wm1[q] + w0));
+    R wr = m_fma(R(-1.0 / 3.0), sp - s0, R(0.5) * (w0 + Wp1[q]));
     const bool ext = (wr - w0) * (w0 - wl) <= R(0);
     const R dd = wr - wl, m6 = R(6) * m_fma(R(-0.5), wl + wr, w0);
     const R t = dd * m6, d2 = dd * dd;
@@ -296,7 +320,8 @@ __device__ __noinline__ FluxRet<R> roe_fallback_flux_p(const V5<R>* WL, const V5
 
 // branch-free core: the Roe flux and whether both intermediate states passed the failure test.  Keeping the
 // (rare) fallback out of it lets two independent solves share one basic block and interleave.
-template <class R> __device__ __forceinline__ bool lean_roe_core(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, V5<R>& F) {
+// hs: the flux is returned times 2 hs (0.5: the flux itself; the CTU first pass asks for nu/2 times the flux at no extra cost)
+template <class R> __device__ __forceinline__ bool lean_roe_core(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, V5<R>& F, R hs = R(0.5)) {
   const R g1 = p.gamma * p.igm1;
   const LeanState<R> L = lean_state(WL, g1), Rr = lean_state(WR, g1);
   // Roe averages with weights wL = sqrt(rhoL)/(sqrt(rhoL)+sqrt(rhoR)), wR = 1 - wL; rho~ = sqrt(rhoL rhoR)
@@ -332,22 +357,27 @@ template <class R> __device__ __forceinline__ bool lean_roe_core(const V5<R>& WL
   const R d2 = m_fma(d0, vt, w3);
   const R d3 = m_fma(d0, wt, w4);
   const R d4 = m_fma(w5, H5, m_fma(w4, wt, m_fma(w3, vt, m_fma(w2, hq, w1 * H1))));
-  F[0] = R(0.5) * ((L.m + Rr.m) - d0);
-  F[1] = R(0.5) * ((L.F1 + Rr.F1) - d1);
-  F[2] = R(0.5) * m_fma(L.m, WL[2], m_fma(Rr.m, WR[2], -d2));
-  F[3] = R(0.5) * m_fma(L.m, WL[3], m_fma(Rr.m, WR[3], -d3));
-  F[4] = R(0.5) * m_fma(L.m, L.H, m_fma(Rr.m, Rr.H, -d4));
+  F[0] = hs * ((L.m + Rr.m) - d0);
+  F[1] = hs * ((L.F1 + Rr.F1) - d1);
+  F[2] = hs * m_fma(L.m, WL[2], m_fma(Rr.m, WR[2], -d2));
+  F[3] = hs * m_fma(L.m, WL[3], m_fma(Rr.m, WR[3], -d3));
+  F[4] = hs * m_fma(L.m, L.H, m_fma(Rr.m, Rr.H, -d4));
   return ok;
 }
+// out-of-line flux of solver `mode` (1 HLLE, 2 HLLC, 3 exact) for the rare paths
+template <class R> __device__ __forceinline__ void lean_fallback_call(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, int mode, Cnt& c, V5<R>& F);
 // Roe failed at this face: count it and replace the flux by the fallback solver's
 template <class R> __device__ __forceinline__ void lean_roe_failed(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c, V5<R>& F) {
   c.roe_fb++;
+  lean_fallback_call(WL, WR, p, p.roe_fallback, c, F);
+}
+template <class R> __device__ __forceinline__ void lean_fallback_call(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, int mode, Cnt& c, V5<R>& F) {
   FluxRet<R> r;
   if (sizeof(R) == 4) {
-    r = roe_fallback_flux<R>(WL[0], WL[1], WL[2], WL[3], WL[4], WR[0], WR[1], WR[2], WR[3], WR[4], p.gamma, p.gm1, p.igm1, p.roe_fallback);
+    r = roe_fallback_flux<R>(WL[0], WL[1], WL[2], WL[3], WL[4], WR[0], WR[1], WR[2], WR[3], WR[4], p.gamma, p.gm1, p.igm1, mode);
   } else {
     V5<R> l = WL, rr = WR;  // copies: only this branch puts its arguments on the stack
-    r = roe_fallback_flux_p<R>(&l, &rr, p.gamma, p.gm1, p.igm1, p.roe_fallback);
+    r = roe_fallback_flux_p<R>(&l, &rr, p.gamma, p.gm1, p.igm1, mode);
   }
   F[0] = r.f0; F[1] = r.f1; F[2] = r.f2; F[3] = r.f3; F[4] = r.f4;
   c.exact += r.ex;
@@ -355,6 +385,16 @@ template <class R> __device__ __forceinline__ void lean_roe_failed(const V5<R>& 
 template <class R> __device__ __forceinline__ V5<R> lean_roe(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
   V5<R> F;
   if (!lean_roe_core(WL, WR, p, F)) lean_roe_failed(WL, WR, p, c, F);
+  return F;
+}
+// the Roe flux times `scale` (scale folded into the solver's final multiplies)
+template <class R> __device__ __forceinline__ V5<R> lean_roe_scaled(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c, R scale) {
+  V5<R> F;
+  if (!lean_roe_core(WL, WR, p, F, R(0.5) * scale)) {
+    lean_roe_failed(WL, WR, p, c, F);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) F[q] = scale * F[q];
+  }
   return F;
 }
 
@@ -380,106 +420,119 @@ template <class R> __device__ __forceinline__ V5<R> lean_hlle(const V5<R>& WL, c
   return F;
 }
 
-// ---- c4: exact solver (Toro ch. 4; S11), same iteration and sampling as hydro_math.cuh `exact` with the per-side
-// constants hoisted out of the Newton loop and ONE pow per rarefaction evaluation: with z = (p/P_K)^((g-1)/(2g)),
-// the derivative's (p/P_K)^(-(g+1)/(2g)) is z P_K / p, the star sound speed is c_K z, the star density behind the
-// tail is rho_K (p/P_K) / z^2, and inside the fan phi^(2g/(g-1)) = phi^2 phi^(2/(g-1)).
-template <class R> struct ExactSide { R rho, u, P, c, iP, A, B, k, irc; };
-template <class R> __device__ __forceinline__ ExactSide<R> exact_side(const V5<R>& W, const Par<R>& p) {
+// ---- c4: exact solver (Toro ch. 4; S11): the same pressure function, Newton iteration, tolerance, iteration cap and
+// sampling as hydro_math.cuh `exact`, organised for the GPU ("much more time-consuming"; it is config 5):
+//   * fully inlined, everything in registers (the round-1 version was an out-of-line call with pointer arguments);
+//   * powers through one logarithm: with w = lg2(p), (p/P_K)^e = ex2(e (w - lg2 P_K)); lg2(p) is shared by both sides and
+//     lg2(P_K) leaves the loop.  fp32 uses the SFU lg2 / ex2 approximations (relative error of z ~ 3e-8, far inside the
+//     1e-6 iteration tolerance); fp64 calls log2 / exp2 once each instead of pow twice per side;
+//   * the shock branch needs one rsqrt per evaluation: sqrt(A_K / (p + B_K)) = sqrt(A_K) rsqrt(p + B_K);
+//   * no re-evaluation of f after the last iterate: the last Newton step delta < tol p gives f(p + delta) = f + f' delta with a
+//     relative error of order tol^2 (1e-12 in fp32, 1e-24 in fp64), likewise z.
+template <class R> __device__ __forceinline__ R l_lg2(R x);
+template <class R> __device__ __forceinline__ R l_ex2(R x);
+#if HYDRO_F32_IEEE
+template <> __device__ __forceinline__ float l_lg2<float>(float x) { return log2f(x); }
+template <> __device__ __forceinline__ float l_ex2<float>(float x) { return exp2f(x); }
+#else
+template <> __device__ __forceinline__ float l_lg2<float>(float x) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+template <> __device__ __forceinline__ float l_ex2<float>(float x) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+#endif
+template <> __device__ __forceinline__ double l_lg2<double>(double x) { return log2(x); }
+template <> __device__ __forceinline__ double l_ex2<double>(double x) { return exp2(x); }
+
+template <class R> struct ExactSide { R rho, u, P, c, irc, sA, B, k, w; };
+template <class R> __device__ __forceinline__ ExactSide<R> exact_side(const V5<R>& W, const Par<R>& p, R ig1, R mu) {
   ExactSide<R> s;
-  const R g = p.gamma, ig1 = l_rcp(g + R(1));
   s.rho = W[0]; s.u = W[1]; s.P = W[4];
-  const R ir = l_rcp(W[0]);
-  s.c = l_sqrt(g * W[4] * ir);
-  s.iP = l_rcp(W[4]);
-  s.A = (ig1 + ig1) * ir;             // 2 / ((g+1) rho)
-  s.B = p.gm1 * ig1 * W[4];           // (g-1)/(g+1) P
-  s.k = (s.c + s.c) * p.igm1;         // 2 c / (g-1)
-  s.irc = ir * l_rcp(s.c);            // 1 / (rho c)
+  const R gP = p.gamma * W[4];
+  s.irc = l_rsqrt(gP * W[0]);                    // 1 / (rho c)
+  s.c = gP * s.irc;
+  s.sA = l_sqrt(ig1 + ig1) * l_rsqrt(W[0]);       // sqrt(A_K), A_K = 2 / ((g+1) rho)
+  s.B = mu * W[4];                                // (g-1)/(g+1) P
+  s.k = (s.c + s.c) * p.igm1;                     // 2 c / (g-1)
+  s.w = l_lg2(W[4]);
   return s;
 }
-// f_K(p), f_K'(p) and, on the rarefaction branch, z = (p/P_K)^e1 (else 0)
-template <class R> __device__ __forceinline__ void exact_fn(R ps, R ips, const ExactSide<R>& s, R e1, R& f, R& df, R& z) {
+// f_K(p), f_K'(p) and, on the rarefaction branch, z = (p/P_K)^e1 (else 0); w = lg2(p), ips = 1/p
+template <class R> __device__ __forceinline__ void exact_fn(R ps, R w, R ips, const ExactSide<R>& s, R e1, R& f, R& df, R& z) {
   if (ps > s.P) {
-    const R t = l_rcp(ps + s.B), q = l_sqrt(s.A * t), d = ps - s.P;
+    const R rs = l_rsqrt(ps + s.B), q = s.sA * rs, d = ps - s.P;
     f = d * q;
-    df = q * m_fma(R(-0.5) * d, t, R(1));
+    df = q * m_fma(R(-0.5) * d, rs * rs, R(1));
     z = R(0);
   } else {
-    z = m_pow(ps * s.iP, e1);
+    z = l_ex2(e1 * (w - s.w));
     f = s.k * (z - R(1));
     df = (z * s.P * ips) * s.irc;
   }
 }
-template <class R> __device__ __noinline__ void lean_exact_impl(const V5<R>* pWL, const V5<R>* pWR, const Par<R>* pp, int* cnt, V5<R>* pF) {
-  const V5<R>& WL = *pWL; const V5<R>& WR = *pWR; const Par<R>& p = *pp;
+template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
   const R g = p.gamma;
-  const ExactSide<R> L = exact_side(WL, p), Rs = exact_side(WR, p);
+  const R ig1 = l_rcp(g + R(1)), mu = p.gm1 * ig1;
+  const ExactSide<R> L = exact_side(WL, p, ig1, mu), Rs = exact_side(WR, p, ig1, mu);
   const R du = Rs.u - L.u;
-  if ((L.k + Rs.k) <= du) {  // vacuum generation -> HLLE flux (S11)
-    *cnt += 1;
-    *pF = hlle(WL, WR, p);
-    return;
+  V5<R> F;
+  if ((L.k + Rs.k) <= du) {  // vacuum generation -> HLLE flux (S11); rare, out of line
+    c.exact++;
+    lean_fallback_call(WL, WR, p, 1, c, F);
+    return F;
   }
   const R e1 = p.gm1 * (R(0.5) * l_rcp(g));
   const R epsp = R(1e-6) * m_min(L.P, Rs.P);
   const R ppv = R(0.5) * (L.P + Rs.P) - R(0.125) * du * (L.rho + Rs.rho) * (L.c + Rs.c);
-  R ps = m_max(epsp, ppv), fL, dL, zL, fR, dR, zR;
+  R ps = m_max(epsp, ppv), fL, dL, zL, fR, dR, zR, dlt = R(0), ips = R(0);
   bool conv = false;
+#pragma unroll 1
   for (int it = 0; it < 40; ++it) {
-    const R ips = l_rcp(ps);
-    exact_fn(ps, ips, L, e1, fL, dL, zL);
-    exact_fn(ps, ips, Rs, e1, fR, dR, zR);
+    const R w = l_lg2(ps);
+    ips = l_rcp(ps);
+    exact_fn(ps, w, ips, L, e1, fL, dL, zL);
+    exact_fn(ps, w, ips, Rs, e1, fR, dR, zR);
     R pn = ps - l_div((fL + fR) + du, dL + dR);
     if (!(pn > R(0))) pn = epsp;
-    const R chg = l_div(R(2) * m_abs(pn - ps), pn + ps);
+    dlt = pn - ps;
+    const bool done = R(2) * m_abs(dlt) < ExactTol<R>::v() * (pn + ps);
+    if (done) { conv = true; break; }
     ps = pn;
-    if (chg < ExactTol<R>::v()) { conv = true; break; }
   }
-  if (!conv) *cnt += 1;
-  {
-    const R ips = l_rcp(ps);
-    exact_fn(ps, ips, L, e1, fL, dL, zL);
-    exact_fn(ps, ips, Rs, e1, fR, dR, zR);
-  }
+  if (!conv) { c.exact++; dlt = R(0); }  // 40 iterations without convergence: the last evaluated iterate stands
+  // first-order update of the last evaluation to the accepted iterate ps + dlt
+  fL = m_fma(dL, dlt, fL);
+  fR = m_fma(dR, dlt, fR);
+  const R zs = m_fma(e1 * ips, dlt, R(1));  // z(ps + dlt) / z(ps)
+  const R pst = ps + dlt;
   const R us = R(0.5) * (L.u + Rs.u) + R(0.5) * (fR - fL);
   // sample at x/t = 0 on the side of the contact given by sign(u*) (S19: u* = 0 -> left); right side mirrored
   const bool left = us >= R(0);
   const R sg = left ? R(1) : R(-1);
   const R rK = left ? L.rho : Rs.rho, PK = left ? L.P : Rs.P, cK = left ? L.c : Rs.c, vK = left ? L.u : Rs.u;
-  const R iPK = left ? L.iP : Rs.iP, zK = left ? zL : zR;
-  const R ig1 = l_rcp(g + R(1)), mu = p.gm1 * ig1, pr = ps * iPK;
+  const R ircK = left ? L.irc : Rs.irc, zK = (left ? zL : zR) * zs;
+  const R pr = pst * l_rcp(PK);
   V5<R> W;
   W[2] = left ? WL[2] : WR[2];
   W[3] = left ? WL[3] : WR[3];
-  if (ps > PK) {  // shock
+  if (pst > PK) {  // shock
     const R ig2 = R(0.5) * l_rcp(g);
     const R S = vK - sg * cK * l_sqrt(m_fma((g + R(1)) * ig2, pr, p.gm1 * ig2));
     const bool undisturbed = left ? (S >= R(0)) : (S <= R(0));
     if (undisturbed) { W[0] = rK; W[1] = vK; W[4] = PK; }
-    else { W[0] = l_div(rK * (pr + mu), m_fma(mu, pr, R(1))); W[1] = us; W[4] = ps; }
+    else { W[0] = l_div(rK * (pr + mu), m_fma(mu, pr, R(1))); W[1] = us; W[4] = pst; }
   } else {  // rarefaction
     const R head = vK - sg * cK, tail = us - sg * (cK * zK);
     const bool before_head = left ? (head >= R(0)) : (head <= R(0));
     const bool behind_tail = left ? (tail <= R(0)) : (tail >= R(0));
     if (before_head) { W[0] = rK; W[1] = vK; W[4] = PK; }
-    else if (behind_tail) { W[0] = l_div(rK * pr, zK * zK); W[1] = us; W[4] = ps; }
+    else if (behind_tail) { W[0] = l_div(rK * pr, zK * zK); W[1] = us; W[4] = pst; }
     else {
-      const R phi = (ig1 + ig1) + l_div(sg * mu * vK, cK);
-      const R w = m_pow(phi, R(2) * p.igm1);
-      W[0] = rK * w;
+      const R phi = (ig1 + ig1) + (sg * mu * vK) * (rK * ircK);  // 1 / c_K = rho_K / (rho_K c_K)
+      const R wf = l_ex2((R(2) * p.igm1) * l_lg2(phi));
+      W[0] = rK * wf;
       W[1] = (ig1 + ig1) * (sg * cK + R(0.5) * p.gm1 * vK);
-      W[4] = PK * (phi * phi) * w;
+      W[4] = PK * (phi * phi) * wf;
     }
   }
-  *pF = phys_flux(W, p);
-}
-template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
-  V5<R> F, l = WL, r = WR;
-  int ex = 0;
-  lean_exact_impl(&l, &r, &p, &ex, &F);
-  c.exact += ex;
-  return F;
+  return phys_flux(W, p);
 }
 
 // ---- c4: HLLC, Toro's pressure-based speeds (S9), select form ----------------------------------

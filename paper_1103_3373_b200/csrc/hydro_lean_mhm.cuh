@@ -22,7 +22,7 @@ namespace hydro {
 template <class R> __device__ __forceinline__ void lean_plm(const V5<R>& Wm, const V5<R>& W0, const V5<R>& Wp, V5<R>& lo, V5<R>& up) {
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
-    const R h = R(0.5) * vl_slope(W0[q] - Wm[q], Wp[q] - W0[q]);
+    const R h = vl_half_slope(W0[q] - Wm[q], Wp[q] - W0[q]);
     lo[q] = W0[q] - h;
     up[q] = W0[q] + h;
   }
