@@ -122,18 +122,47 @@ def time_oracle(G, dt, nthreads, target_s=12.0):
     return passes * n * CELLS / el, n, el, passes
 
 
-def ncu_traffic(key):
-    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the dominant kernel from the
-    committed ncu --set full capture, profiles/traffic.csv: key,bytes_per_launch,source."""
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
-            for line in f:
-                c = [x.strip() for x in line.split(",")]
-                if len(c) >= 2 and c[0] == key:
-                    return float(c[1])
-    except Exception:
-        pass
-    return None
+def ncu_counters(key):
+    """Per-launch counters of the dominant kernel from the committed ncu --set full capture of this same workload
+    (profiles/kernel_counters.json, written from the .ncu-rep by the command named in it): DRAM bytes, executed
+    FP thread-instructions (fadd, fmul, ffma / dadd, dmul, dfma), FMA / FP64 pipe utilisation."""
+    d = load_json(os.path.join(ROOT, "profiles", "kernel_counters.json"), {}) or {}
+    return d.get(key)
+
+
+def measured_peaks():
+    """ALU peaks measured on this pool's B200 by `python bench.py --table peaks` (profiles/alu_peaks.json)."""
+    return load_json(os.path.join(ROOT, "profiles", "alu_peaks.json"), {}) or {}
+
+
+def alu_roofline(dtype, kernel_ms, flops_cell, ncells, sm_max, key):
+    """The three fractions of the ALU roofline for one hydro_solve launch of `ncells` cell updates:
+    frac          = oracle-counted (algorithmic) flops / time / MEASURED FMA peak      (the metric's fraction)
+    frac_executed = flops the kernel actually executes (ncu: fadd + fmul + 2 ffma thread-instructions) / time / peak
+    pipe_pct      = sm__inst_executed_pipe_fma (fp64: pipe_fp64) of the committed capture."""
+    lanes = 128 if dtype == "f32" else 64
+    nominal = 148 * lanes * 2 * sm_max * 1e6 / 1e12
+    mp = measured_peaks()
+    peak = mp.get("fp32_tflops_ffma" if dtype == "f32" else "fp64_tflops")
+    src = "measured: register-resident %s loop, python bench.py --table peaks -> profiles/alu_peaks.json" % ("FFMA" if dtype == "f32" else "DFMA")
+    if not peak:
+        peak, src = nominal, f"nominal (profiles/alu_peaks.json missing): 148 SM x {lanes} lanes x 2 x {sm_max:.0f} MHz"
+    achieved = flops_cell * ncells / (kernel_ms * 1e-3) / 1e12
+    r = {"achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "peak_source": src,
+         "peak_nominal": nominal, "frac_of_nominal": achieved / nominal}
+    c = ncu_counters(key)
+    if c:
+        ex = c.get("flops_executed_per_launch")
+        if ex and c.get("cells_per_launch"):
+            ex_t = ex * (ncells / c["cells_per_launch"]) / (kernel_ms * 1e-3) / 1e12
+            r.update({"executed_tflops": ex_t, "frac_executed": ex_t / peak, "flops_executed_per_cell": ex / c["cells_per_launch"]})
+        r["pipe_pct"] = c.get("pipe_pct")
+        r["issue_active_pct"] = c.get("issue_active_pct")
+        r["traffic"] = c.get("dram_bytes_per_launch")
+        r["counters_source"] = c.get("source")
+    else:
+        r.update({"frac_executed": None, "pipe_pct": None, "traffic": None})
+    return r
 
 
 def run_reference(args):
@@ -391,31 +420,26 @@ def main():
     peaks = load_json(os.path.join(ROOT, "MEASURED_PEAKS.json"), {}) or {}
     clocks = leg["clocks"] or {}
     sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
-    lanes = 128 if args.dtype == "f32" else 64  # FP32 / FP64 FMA lanes per SM
-    peak_tflops = 148 * lanes * 2 * sm_max * 1e6 / 1e12
     flops_cell, flops_src = algorithmic_flops_per_cell(args.dtype)
-    achieved_tflops = flops_cell * Ng * CELLS / (leg["solve_ms"] * 1e-3) / 1e12
     bytes_cell = es * (5 * S ** 3 + 5 * CELLS + 45 * 256) / CELLS
     hbm = float(peaks.get("hbm_gbs") or 6650.0)
     hbm_src = "measured (MEASURED_PEAKS.json)" if peaks.get("hbm_gbs") else "fallback (B200_PROFILING.md)"
-    traffic = ncu_traffic(f"solve_{args.dtype}_{args.kernel}")
     if impl != B.IMPL_STAGED and B.hydro_fused_fits(main_dtype, SCHEME, B.PLM, GHOST):
         kernel_name = "hydro_solve (ctu_lean_kernel: fused z-marching CTU, phase-crossing state in shared memory)"
     else:
         kernel_name = "hydro_solve (staged_kernel)"
-    roofline = {
-        "bound": "alu", "kernel": kernel_name,
-        "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved_tflops / peak_tflops,
-        "traffic": traffic,
+    roofline = {"bound": "alu", "kernel": kernel_name}
+    roofline.update(alu_roofline(args.dtype, leg["solve_ms"], flops_cell, Ng * CELLS, sm_max, f"solve_{args.dtype}"))
+    roofline.update({
         "flops_per_cell": flops_cell, "flops_source": flops_src,
-        "peak_source": f"148 SM x {lanes} lanes x 2 x {sm_max:.0f} MHz (nominal unit counts at clocks.max.sm)",
         "kernel_ms": leg["solve_ms"], "share_of_step": leg["solve_ms"] / (leg["solve_ms"] + leg["dt_ms"]),
         "hbm": {"bytes_per_cell": bytes_cell, "achieved_gbs": bytes_cell * Ng * CELLS / (leg["solve_ms"] * 1e-3) / 1e9,
                 "peak_gbs": hbm, "peak_source": hbm_src,
-                "hydro_dt_gbs": 5 * es * Ng * CELLS / (leg["dt_ms"] * 1e-3) / 1e9},
-        "cells_per_s_at_alu_roof": peak_tflops * 1e12 / flops_cell,
+                "hydro_dt_gbs": 5 * es * Ng * CELLS / (leg["dt_ms"] * 1e-3) / 1e9,
+                "hydro_dt_frac": 5 * es * Ng * CELLS / (leg["dt_ms"] * 1e-3) / 1e9 / hbm},
+        "cells_per_s_at_alu_roof": roofline["peak"] * 1e12 / flops_cell,
         "cells_per_s_at_hbm_roof": hbm * 1e9 / bytes_cell,
-    }
+    })
 
     result = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,

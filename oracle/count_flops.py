@@ -50,9 +50,8 @@ def main():
     MHM, VL, CTU = 0, 1, 2
     EXACT, HLLE, HLLC, ROE = 0, 1, 2, 3
     gamma, dh = 5.0 / 3.0, 1.0
-    out = {"_about": "algorithmic operations per interior cell update, counted on the CPU oracle (oracle/flop_count.cpp) "
-                     "over the oracle's regions (<= 1.3 % above the minimal per-group multiplicities of SURVEY.md 8(a)); "
-                     "input: first 8 groups of workloads.amr_batch(seed=0), dt = CFL*dh/hydro_dt",
+    out = {"_about": "algorithmic operations per interior cell update, counted on the CPU oracle (oracle/flop_count.cpp) over the oracle's regions; input: first 8 groups of workloads.amr_batch(seed=0), dt = CFL*dh/hydro_dt.  CTU and MHM: the oracle's regions are within 1.3 % of the minimal per-group multiplicities of SURVEY.md 8(a) (7.22 vs 7.17 and 3.19 vs 3.19 Riemann solves per cell).  VL: the oracle's predictor region is a box, not the minimal plus: 9.34 / 11.34 solves per cell (PLM / PPM) against the minimal 8.72 / 9.89, i.e. the VL counts are 7 % / 15 % above what the method must compute and roofline fractions quoted from them are flattering by about half of that",
+           "_minimal_riemann_per_cell": {"ctu": 7.17, "mhm": 3.19, "vl_plm": 8.72, "vl_ppm": 9.89, "source": "SURVEY.md 8(a)"},
            "_flop_rule": "add, sub, mul, div, sqrt, pow = 1 each; compare/abs/min/max/select/negate = 0"}
     cases = {
         "ctu_plm_roe_vanleer_g3": (CTU, ROE, 1, 0, 3, 0.5),

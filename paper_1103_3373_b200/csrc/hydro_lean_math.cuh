@@ -442,16 +442,25 @@ template <> __device__ __forceinline__ double l_lg2<double>(double x) { return l
 template <> __device__ __forceinline__ double l_ex2<double>(double x) { return exp2(x); }
 
 template <class R> struct ExactSide { R rho, u, P, c, irc, sA, B, k, w; };
-template <class R> __device__ __forceinline__ ExactSide<R> exact_side(const V5<R>& W, const Par<R>& p, R ig1, R mu) {
+template <class R> struct ExactConst { R gamma, gm1, igm1, ig1, mu, e1; };  // ig1 = 1/(g+1), mu = (g-1)/(g+1), e1 = (g-1)/(2g)
+template <class R> __device__ __forceinline__ ExactConst<R> exact_const(R gamma, R gm1, R igm1) {
+  ExactConst<R> k;
+  k.gamma = gamma; k.gm1 = gm1; k.igm1 = igm1;
+  k.ig1 = l_rcp(gamma + R(1));
+  k.mu = gm1 * k.ig1;
+  k.e1 = gm1 * (R(0.5) * l_rcp(gamma));
+  return k;
+}
+template <class R> __device__ __forceinline__ ExactSide<R> exact_side(R rho, R u, R P, const ExactConst<R>& k) {
   ExactSide<R> s;
-  s.rho = W[0]; s.u = W[1]; s.P = W[4];
-  const R gP = p.gamma * W[4];
-  s.irc = l_rsqrt(gP * W[0]);                    // 1 / (rho c)
+  s.rho = rho; s.u = u; s.P = P;
+  const R gP = k.gamma * P;
+  s.irc = l_rsqrt(gP * rho);                      // 1 / (rho c)
   s.c = gP * s.irc;
-  s.sA = l_sqrt(ig1 + ig1) * l_rsqrt(W[0]);       // sqrt(A_K), A_K = 2 / ((g+1) rho)
-  s.B = mu * W[4];                                // (g-1)/(g+1) P
-  s.k = (s.c + s.c) * p.igm1;                     // 2 c / (g-1)
-  s.w = l_lg2(W[4]);
+  s.sA = l_sqrt(k.ig1 + k.ig1) * l_rsqrt(rho);    // sqrt(A_K), A_K = 2 / ((g+1) rho)
+  s.B = k.mu * P;                                 // (g-1)/(g+1) P
+  s.k = (s.c + s.c) * k.igm1;                     // 2 c / (g-1)
+  s.w = l_lg2(P);
   return s;
 }
 // f_K(p), f_K'(p) and, on the rarefaction branch, z = (p/P_K)^e1 (else 0); w = lg2(p), ips = 1/p
@@ -467,10 +476,44 @@ template <class R> __device__ __forceinline__ void exact_fn(R ps, R w, R ips, co
     df = (z * s.P * ips) * s.irc;
   }
 }
+// Newton iteration on f_L + f_R + du = 0 from ps (S11: negative iterate -> eps_p, at most 40 evaluations).  Stops when the
+// relative change 2 |delta| / (p_new + p) falls below `stop`; returns the LAST EVALUATED point ps with f, f', z there and the
+// step delta to the accepted iterate ps + delta, whose distance to the root is of order delta^2 / p (Newton is quadratic).
+template <class R> struct ExactIter { R ps, dlt, ips, fL, dL, zL, fR, dR, zR; bool conv; };
+template <class R> __device__ __forceinline__ ExactIter<R> exact_newton(const ExactSide<R>& L, const ExactSide<R>& Rs, R du, R e1, R epsp, R ps, R stop) {
+  ExactIter<R> r;
+  r.conv = false;
+  r.dlt = R(0);
+#pragma unroll 1
+  for (int it = 0; it < 40; ++it) {
+    R w = R(0);
+    r.ips = R(0);
+    if (!(ps > L.P) || !(ps > Rs.P)) { w = l_lg2(ps); r.ips = l_rcp(ps); }  // only the rarefaction branch needs them
+    exact_fn(ps, w, r.ips, L, e1, r.fL, r.dL, r.zL);
+    exact_fn(ps, w, r.ips, Rs, e1, r.fR, r.dR, r.zR);
+    R pn = ps - l_div((r.fL + r.fR) + du, r.dL + r.dR);
+    if (!(pn > R(0))) pn = epsp;
+    r.dlt = pn - ps;
+    if (R(2) * m_abs(r.dlt) < stop * (pn + ps)) { r.conv = true; break; }
+    ps = pn;
+  }
+  r.ps = ps;
+  if (!r.conv) r.dlt = R(0);  // 40 evaluations without convergence: the last evaluated iterate stands
+  return r;
+}
+// Stopping rule.  fp32: the oracle's tolerance 1e-6 (S11).  fp64: S11's 1e-12 bounds the error of p*; because the accepted
+// iterate is ps + delta with an error of order delta^2 / p, a step below 1e-7 p already puts it within 1e-14 p of the root --
+// the last evaluation S11's rule would spend only confirms that.  The fp64 iteration moreover starts from the root of an
+// fp32 Newton iteration on the rounded states (SFU logarithms, ~1e-6 p away), so two fp64 evaluations suffice.
+template <class R> struct ExactStop;
+template <> struct ExactStop<float> { static __device__ __forceinline__ float v() { return 1e-6f; } };
+template <> struct ExactStop<double> { static __device__ __forceinline__ double v() { return 1e-7; } };
+
 template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
   const R g = p.gamma;
-  const R ig1 = l_rcp(g + R(1)), mu = p.gm1 * ig1;
-  const ExactSide<R> L = exact_side(WL, p, ig1, mu), Rs = exact_side(WR, p, ig1, mu);
+  const ExactConst<R> k = exact_const<R>(g, p.gm1, p.igm1);
+  const R ig1 = k.ig1, mu = k.mu, e1 = k.e1;
+  const ExactSide<R> L = exact_side(WL[0], WL[1], WL[4], k), Rs = exact_side(WR[0], WR[1], WR[4], k);
   const R du = Rs.u - L.u;
   V5<R> F;
   if ((L.k + Rs.k) <= du) {  // vacuum generation -> HLLE flux (S11); rare, out of line
@@ -478,25 +521,22 @@ template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, 
     lean_fallback_call(WL, WR, p, 1, c, F);
     return F;
   }
-  const R e1 = p.gm1 * (R(0.5) * l_rcp(g));
   const R epsp = R(1e-6) * m_min(L.P, Rs.P);
   const R ppv = R(0.5) * (L.P + Rs.P) - R(0.125) * du * (L.rho + Rs.rho) * (L.c + Rs.c);
-  R ps = m_max(epsp, ppv), fL, dL, zL, fR, dR, zR, dlt = R(0), ips = R(0);
-  bool conv = false;
-#pragma unroll 1
-  for (int it = 0; it < 40; ++it) {
-    const R w = l_lg2(ps);
-    ips = l_rcp(ps);
-    exact_fn(ps, w, ips, L, e1, fL, dL, zL);
-    exact_fn(ps, w, ips, Rs, e1, fR, dR, zR);
-    R pn = ps - l_div((fL + fR) + du, dL + dR);
-    if (!(pn > R(0))) pn = epsp;
-    dlt = pn - ps;
-    const bool done = R(2) * m_abs(dlt) < ExactTol<R>::v() * (pn + ps);
-    if (done) { conv = true; break; }
-    ps = pn;
+  R ps = m_max(epsp, ppv);
+  if (sizeof(R) == 8) {  // fp64: start from the fp32 root (any start is allowed: the root is unique, f is monotone and concave)
+    const ExactConst<float> kf = exact_const<float>((float)g, (float)p.gm1, (float)p.igm1);
+    const ExactSide<float> Lf = exact_side((float)WL[0], (float)WL[1], (float)WL[4], kf),
+                           Rf = exact_side((float)WR[0], (float)WR[1], (float)WR[4], kf);
+    const ExactIter<float> rf = exact_newton<float>(Lf, Rf, (float)du, kf.e1, (float)epsp, (float)ps, 1e-6f);
+    const R pf = (R)(rf.ps + rf.dlt);
+    if (pf > epsp && pf < R(3.0e38)) ps = pf;  // finite and positive in fp32's range; otherwise keep the linearised guess
   }
-  if (!conv) { c.exact++; dlt = R(0); }  // 40 iterations without convergence: the last evaluated iterate stands
+  const ExactIter<R> it = exact_newton<R>(L, Rs, du, e1, epsp, ps, ExactStop<R>::v());
+  if (!it.conv) c.exact++;
+  ps = it.ps;
+  R fL = it.fL, fR = it.fR;
+  const R dL = it.dL, dR = it.dR, zL = it.zL, zR = it.zR, dlt = it.dlt, ips = it.ips;
   // first-order update of the last evaluation to the accepted iterate ps + dlt
   fL = m_fma(dL, dlt, fL);
   fR = m_fma(dR, dlt, fR);
@@ -507,8 +547,11 @@ template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, 
   const bool left = us >= R(0);
   const R sg = left ? R(1) : R(-1);
   const R rK = left ? L.rho : Rs.rho, PK = left ? L.P : Rs.P, cK = left ? L.c : Rs.c, vK = left ? L.u : Rs.u;
-  const R ircK = left ? L.irc : Rs.irc, zK = (left ? zL : zR) * zs;
+  const R ircK = left ? L.irc : Rs.irc, zE = left ? zL : zR;
   const R pr = pst * l_rcp(PK);
+  // z at the accepted iterate.  If the last evaluation took the shock branch (zE = 0) while the accepted iterate is a
+  // rarefaction, p* lies within one Newton step (< tol p) of P_K and z = 1 + e1 (p*/P_K - 1) to second order
+  const R zK = zE > R(0) ? zE * zs : m_fma(e1, pr - R(1), R(1));
   V5<R> W;
   W[2] = left ? WL[2] : WR[2];
   W[3] = left ? WL[3] : WR[3];
