@@ -270,6 +270,61 @@ def run_table(args):
     print(json.dumps({"table": "grid", "rows": rows}))
 
 
+def run_counters(args):
+    """--table counters --rep-f32 A.ncu-rep --rep-f64 B.ncu-rep: distil the committed `ncu --set full` captures of the dominant
+    kernel (one launch of hydro_solve on the bench workload) into profiles/kernel_counters.json, which the bench line reads
+    for frac_executed / pipe_pct / traffic.  Runs here (no GPU): `ncu -i <rep> --page raw --csv`."""
+    import csv
+    import subprocess
+    out = {"_command": "python bench.py --table counters --rep-f32 %s --rep-f64 %s" % (args.rep_f32, args.rep_f64),
+           "_capture": "ncu --set full --clock-control none --import-source on -k regex:ctu_lean_kernel -s 3 -c 1 -o <rep> "
+                       "python bench.py --steps 3 --warmup 3 --no-extras [--dtype f64]"}
+    for key, rep in (("solve_f32", args.rep_f32), ("solve_f64", args.rep_f64)):
+        if not rep:
+            continue
+        txt = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+        rows = list(csv.reader(txt.splitlines()))
+        hdr, vals = rows[0], rows[2]
+        m = {h: v for h, v in zip(hdr, vals)}
+
+        def f(name):
+            return float(m[name].replace(",", ""))
+        # executed FP thread-instructions by opcode from the source page (predicated-on threads of every SASS instruction)
+        src = subprocess.run(["ncu", "-i", rep, "--page", "source", "--csv"], capture_output=True, text=True, check=True).stdout
+        srows = list(csv.reader(src.splitlines()))
+        sh = srows[1]
+        i_src, i_thr = sh.index("Source"), sh.index("Predicated-On Thread Instructions Executed")
+        ops = ("FADD", "FMUL", "FFMA") if key == "solve_f32" else ("DADD", "DMUL", "DFMA")
+        fl = [0.0, 0.0, 0.0]
+        for r in srows[2:]:
+            if len(r) <= i_thr or not r[i_thr]:
+                continue
+            tok = r[i_src].split()
+            op = (tok[1] if tok and tok[0].startswith("@") and len(tok) > 1 else (tok[0] if tok else "")).split(".")[0]
+            if op in ops:
+                fl[ops.index(op)] += float(r[i_thr])
+        pipe = f("sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active" if key == "solve_f32"
+                 else "sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active")
+        unit = {h: u for h, u in zip(hdr, rows[1])}
+
+        def gb(name):  # ncu prints dram bytes in a scaled unit
+            scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[unit[name]]
+            return f(name) * scale
+        out[key] = {
+            "kernel": m.get("Kernel Name", "")[:80], "cells_per_launch": NG * CELLS,
+            "thread_inst_add_mul_fma": fl, "flops_executed_per_launch": fl[0] + fl[1] + 2 * fl[2],
+            "pipe_pct": pipe, "issue_active_pct": f("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+            "warp_inst_per_launch": f("smsp__inst_executed.sum"),
+            "registers": f("launch__registers_per_thread"),
+            "local_ld": f("smsp__sass_inst_executed_op_local_ld.sum"), "local_st": f("smsp__sass_inst_executed_op_local_st.sum"),
+            "dram_bytes_per_launch": gb("dram__bytes_read.sum") + gb("dram__bytes_write.sum"),
+            "ncu_duration_ms": f("gpu__time_duration.sum") * {"ms": 1.0, "us": 1e-3, "s": 1e3}.get(unit["gpu__time_duration.sum"], 1.0),
+            "source": os.path.basename(rep)}
+    with open(os.path.join(ROOT, "profiles", "kernel_counters.json"), "w") as fo:
+        json.dump(out, fo, indent=1)
+    print(json.dumps(out))
+
+
 def run_peaks(args, B, dev):
     """--table peaks: MEASURED ALU peaks.  Register-resident loops of hydro_alu_peak_launch on all SMs
     (4 CTAs x 512 threads per SM, 16 independent chains per thread), each kind run back to back for ~1 s under the
@@ -329,12 +384,16 @@ def main():
     ap.add_argument("--ng", type=int, default=NG, help="patch groups per GPU (default: the config's 8192)")
     ap.add_argument("--kernel", default="auto", choices=("auto", "staged", "fused"))
     ap.add_argument("--no-extras", action="store_true", help="skip the e2e / cpu_baseline / f64 legs (profiling runs)")
-    ap.add_argument("--table", default=None, choices=("variants", "grid", "peaks"),
+    ap.add_argument("--table", default=None, choices=("variants", "grid", "peaks", "counters"),
                     help="instead of the bench line: one JSON line with per-variant hydro_solve timings (4096 groups), or with the\n"
                          "uniform-grid kernels (gather / scatter bandwidth, whole-step rates); context for DESIGN.md, profiles/")
+    ap.add_argument("--rep-f32", default=None, help="--table counters: ncu report of the fp32 dominant kernel")
+    ap.add_argument("--rep-f64", default=None, help="--table counters: ncu report of the fp64 dominant kernel")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.table == "counters":
+        return run_counters(args)
     if args.table:
         return run_table(args)
 
@@ -451,48 +510,64 @@ def main():
         "roofline": roofline, "clocks": clocks, "gpu_launches": 2 * steps, "status": leg["status"],
     }
 
-    if rank == 0 and world == 1 and not args.no_extras:
-        # ---- e2e: HOST buffers through the C ABI pipeline (PAPER.md:107, 123), copies inside the timed region
-        u = leg["u"]
-        hin = torch.empty(u.shape, dtype=u.dtype, pin_memory=True)
-        hin.copy_(u)
-        del leg["u"], u
-        hout = torch.empty((Ng, 5, 16, 16, 16), dtype=main_dtype, pin_memory=True)
-        hff = torch.empty((Ng, 9, 5, 16, 16), dtype=main_dtype, pin_memory=True)
-        hs = torch.zeros((), dtype=main_dtype)
-        pipe = B.HydroPipeline(main_dtype, GHOST, groups_per_chunk=512, nstreams=4, device=dev)
-        dt0 = CFL * DH / leg["smax"]
+    def e2e_leg(tdtype, smax_val, nrep):
+        """The same metric through hydro_pipeline_solve with HOST buffers: pinned in / out, H2D and D2H
+        copies inside the timed region."""
+        name = str(tdtype).replace("torch.", "")
+        esz = 4 if tdtype == torch.float32 else 8
+        hin = torch.empty((Ng, 5, S, S, S), dtype=tdtype, pin_memory=True)
+        hin.copy_(wl.amr_batch(Ng, g=GHOST, gamma=GAMMA, seed=1000 * rank, dtype=name, device=dev))
+        hout = torch.empty((Ng, 5, 16, 16, 16), dtype=tdtype, pin_memory=True)
+        hff = torch.empty((Ng, 9, 5, 16, 16), dtype=tdtype, pin_memory=True)
+        hs = torch.zeros((), dtype=tdtype)
+        pipe = B.HydroPipeline(tdtype, GHOST, groups_per_chunk=512, nstreams=4, device=dev)
+        dt0 = CFL * DH / smax_val
         pipe.solve(hin, hout, hff, dt0, DH, GAMMA, SCHEME, RIEMANN, LIMITER, max_speed=hs, impl=impl)
-        ne = max(2, min(5, steps))
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for _ in range(ne):
+        for _ in range(nrep):
             pipe.solve(hin, hout, hff, dt0, DH, GAMMA, SCHEME, RIEMANN, LIMITER, max_speed=hs, impl=impl)
         torch.cuda.synchronize()
-        e2e_s = (time.perf_counter() - t0) / ne
+        e2e_s = (time.perf_counter() - t0) / nrep
         pipe.close()
-        result["e2e"] = {"value": Ng * CELLS / e2e_s, "unit": UNIT, "h2d_bytes_per_step": hin.numel() * es,
-                         "d2h_bytes_per_step": (hout.numel() + hff.numel()) * es + es, "ms_per_step": 1e3 * e2e_s,
-                         "api": "hydro_pipeline_solve (pinned host in/out, 4 streams x 512-group chunks; hydro_dt of the updated state fused per chunk)"}
-        # ---- cpu_baseline: the oracle as it stands, bounded sample, all host cores
+        r = {"value": Ng * CELLS / e2e_s, "unit": UNIT, "h2d_bytes_per_step": hin.numel() * esz,
+             "d2h_bytes_per_step": (hout.numel() + hff.numel()) * esz + esz, "ms_per_step": 1e3 * e2e_s,
+             "pcie_gbs": (hin.numel() + hout.numel() + hff.numel()) * esz / e2e_s / 1e9,
+             "api": "hydro_pipeline_solve (pinned host in/out, 4 streams x 512-group chunks; hydro_dt of the updated state fused per chunk)"}
+        return r, hin, dt0
+
+    if rank == 0 and world == 1 and not args.no_extras:
+        del leg["u"]
+        torch.cuda.empty_cache()
+        # ---- e2e: HOST buffers through the C ABI pipeline, copies inside the timed region
+        result["e2e"], hin, dt0 = e2e_leg(main_dtype, leg["smax"], max(2, min(5, steps)))
+        # ---- cpu_baseline: the oracle as it stands, bounded sample: all host cores (OpenMP over groups, PAPER.md:137)
+        # and ONE thread (the paper quotes its speed-ups against one core and against four, PAPER.md:147)
         from oracle import oracle as O
         nthreads = min(O.max_threads(), len(os.sched_getaffinity(0)))
         G = hin.numpy()
-        cpu_v, cpu_n, cpu_s, cpu_p = time_oracle(G, float(G.dtype.type(dt0)), nthreads)
+        cpu_v, cpu_n, cpu_s, cpu_p = time_oracle(G, float(G.dtype.type(dt0)), nthreads, target_s=10.0)
+        one_v, one_n, one_s, one_p = time_oracle(G, float(G.dtype.type(dt0)), 1, target_s=8.0)
         result["cpu_baseline"] = {"value": cpu_v, "unit": UNIT, "cores": nthreads, "kind": "oracle",
-                                  "sample": f"first {cpu_n} of {Ng} patch groups of the same batch, {cpu_p} passes of hydro_dt + one {args.dtype} CTU+PLM+Roe step, {cpu_s:.1f} s, OpenMP over groups"}
-        del hin, hout, hff
+                                  "sample": f"first {cpu_n} of {Ng} patch groups of the same batch, {cpu_p} passes of hydro_dt + one {args.dtype} CTU+PLM+Roe step, {cpu_s:.1f} s, OpenMP over groups",
+                                  "one_thread": {"value": one_v, "unit": UNIT, "cores": 1,
+                                                 "sample": f"first {one_n} groups, {one_p} passes, {one_s:.1f} s, single thread"}}
+        del hin, G
         torch.cuda.empty_cache()
-        # ---- the other precision, device-resident leg only
+        # ---- the other precision: device-resident leg with the same roofline fractions, and its own e2e
         other = torch.float64 if args.dtype == "f32" else torch.float32
         oname = "f64" if args.dtype == "f32" else "f32"
-        leg2 = device_leg(other, max(3, steps // 2), 3, False)
-        v2 = Ng * CELLS * max(3, steps // 2) / (leg2["total_ms"] * 1e-3)
-        lanes2 = 64 if oname == "f64" else 128
-        peak2 = 148 * lanes2 * 2 * sm_max * 1e6 / 1e12
-        ach2 = flops_cell * Ng * CELLS / (leg2["solve_ms"] * 1e-3) / 1e12
-        result[oname] = {"value": v2, "unit": UNIT, "ms_per_step": leg2["total_ms"] / max(3, steps // 2),
-                         "roofline": {"bound": "alu", "achieved": ach2, "peak": peak2, "unit": "TFLOP/s", "frac": ach2 / peak2}}
+        n2 = max(3, steps // 2)
+        leg2 = device_leg(other, n2, 3, False)
+        del leg2["u"]
+        torch.cuda.empty_cache()
+        v2 = Ng * CELLS * n2 / (leg2["total_ms"] * 1e-3)
+        r2 = {"bound": "alu"}
+        r2.update(alu_roofline(oname, leg2["solve_ms"], flops_cell, Ng * CELLS, sm_max, f"solve_{oname}"))
+        r2["kernel_ms"] = leg2["solve_ms"]
+        e2, hin2, _ = e2e_leg(other, leg2["smax"], 2)
+        del hin2
+        result[oname] = {"value": v2, "unit": UNIT, "ms_per_step": leg2["total_ms"] / n2, "roofline": r2, "e2e": e2}
     elif "u" in leg:
         del leg["u"]
     if "e2e" not in result:

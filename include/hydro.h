@@ -155,6 +155,37 @@ HYDRO_API int hydro_solve_grid_f32(const float* grid_in, float* grid_out, int nx
 HYDRO_API int hydro_solve_grid_f64(const double* grid_in, double* grid_out, int nx, int ny, int nz, int bc, double dt, double dh,
                          double gamma, int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream);
 
+/* Consumer of face_flux: coarse-fine flux fix-up and fine -> coarse restriction after the fluid update of two adjacent AMR
+ * levels (section 2 step 5: the stored fluxes are "only necessary in AMR"; section 4.3: the
+ * "coarse-grid correction", a CPU task in the paper).  The paper gives no formula; reading S25 of DESIGN.md:
+ *   - a refined coarse patch (8^3 coarse cells) is covered by exactly ONE fine patch group (16^3 fine cells), so the outer
+ *     boundary planes of the fine group (face_flux planes p = 3 d + s, s = 0 or 2) coincide with the faces of the coarse patch,
+ *     each coarse face being covered by 2 x 2 fine faces;
+ *   - hydro_restrict_*: for every entry of map[n][5] = (fine_group, coarse_group, pi, pj, pk) the 8^3 coarse cells of
+ *     coarse_out[coarse_group] starting at (pi, pj, pk) (each 0 or 8) become the means of their eight fine cells of
+ *     fine_out[fine_group], summed ((x pairs) + (x pairs)) over y, then over z, times 1/8: bit-exact with the oracle;
+ *   - hydro_fluxfix_*: for every entry of faces[n][7] = (fine_group, dir, fine_side, coarse_group, ci, cj, ck): the 8 x 8 layer of
+ *     UNREFINED coarse cells of coarse_out[coarse_group] adjacent to the face -- (ci, cj, ck) is the first cell of the layer:
+ *     along dir the layer index, in-plane a multiple of 8 -- is corrected by
+ *         U += sigma (dt_c / dh_c) (F_c - ((f00 + f10) + (f01 + f11)) / 4),
+ *     F_c = coarse_flux[coarse_group][3 dir + s] at the cell's face toward the fine group (s = (layer + 1) / 8 if the fine group
+ *     lies above the layer, fine_side = 0: its LOWER boundary plane is the face; s = layer / 8 if below, fine_side = 1),
+ *     f.. = the 2 x 2 fine fluxes of fine_flux[fine_group][3 dir + 2 fine_side], sigma = +1 (fine_side 0) or -1.  Contributions
+ *     of several faces to one cell are added atomically (their order is not fixed: rounding-level only).
+ *   - hydro_flux_accum_*: acc += w * face_flux over n elements (the dt-weighted time average of sub-cycled fine fluxes).
+ * coarse_out / fine_out are the `out` arrays of hydro_solve_* of the two levels, coarse_flux / fine_flux their `face_flux`
+ * arrays (raw flux densities); faces / map: device int arrays.  All pointers device, caller-owned, 16-byte aligned (int lists:
+ * 4); asynchronous on `stream`.  Errors: HYDRO_E_COUNT (n < 0), HYDRO_E_NULL, HYDRO_E_ALIGN, HYDRO_E_VALUE (dh_c <= 0, dt_c < 0).
+ * Index values are NOT range-checked (device data). */
+HYDRO_API int hydro_fluxfix_f32(float* coarse_out, const float* coarse_flux, const float* fine_flux, const int* faces, int nfaces,
+                                float dt_c, float dh_c, hydro_stream_t stream);
+HYDRO_API int hydro_fluxfix_f64(double* coarse_out, const double* coarse_flux, const double* fine_flux, const int* faces, int nfaces,
+                                double dt_c, double dh_c, hydro_stream_t stream);
+HYDRO_API int hydro_restrict_f32(const float* fine_out, float* coarse_out, const int* map, int n, hydro_stream_t stream);
+HYDRO_API int hydro_restrict_f64(const double* fine_out, double* coarse_out, const int* map, int n, hydro_stream_t stream);
+HYDRO_API int hydro_flux_accum_f32(float* acc, const float* face_flux, long long n, float w, hydro_stream_t stream);
+HYDRO_API int hydro_flux_accum_f64(double* acc, const double* face_flux, long long n, double w, hydro_stream_t stream);
+
 /* Sizes and capabilities. */
 HYDRO_API int hydro_min_ghost(int scheme, int recon);                 /* 2/3 (MHM, CTU with PLM/PPM), 3/4 (VL)   */
 HYDRO_API int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann); /* 1 if a fused kernel exists */

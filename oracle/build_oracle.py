@@ -9,14 +9,15 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "hydro_oracle.cpp")
+SRCS = [SRC, os.path.join(HERE, "amr_oracle.cpp")]  # the fluid update; the flux fix-up / restriction that consume its fluxes
 LIB = os.path.join(HERE, "liboracle.so")
 
 
 def build(force: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in SRCS):
         return LIB
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
-           "-Wall", "-Wextra", "-o", LIB + ".tmp", SRC]
+           "-Wall", "-Wextra", "-o", LIB + ".tmp"] + SRCS
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB

@@ -160,5 +160,43 @@ def eig_expand(W, gamma, a):
     return d
 
 
+# ---- consumer of face_flux (oracle/amr_oracle.cpp): coarse-fine flux fix-up and restriction, SURVEY.md 8(f)-3 ----
+def _amr_fn(name, dtype):
+    L = lib()
+    fn = getattr(L, f"oracle_{name}_{'f64' if dtype == np.float64 else 'f32'}")
+    fn.restype = None
+    return fn, (C.c_double if dtype == np.float64 else C.c_float)
+
+
+def fluxfix(coarse_out, coarse_flux, fine_flux, faces, dt_c, dh_c):
+    """In place on coarse_out[Nc,5,16,16,16]: U += sigma (dt_c/dh_c) (F_c - mean of the 4 fine fluxes) for every
+    coarse-fine face listed in faces[n,7] = (fine_group, dir, fine_side, coarse_group, ci, cj, ck) (int32)."""
+    faces = np.ascontiguousarray(faces, np.int32).reshape(-1, 7)
+    assert coarse_out.flags.c_contiguous and coarse_flux.flags.c_contiguous and fine_flux.flags.c_contiguous
+    fn, ct = _amr_fn("fluxfix", coarse_out.dtype.type)
+    fn.argtypes = [C.POINTER(ct), C.POINTER(ct), C.POINTER(ct), C.POINTER(C.c_int), C.c_int, ct, ct]
+    fn(_ptr(coarse_out, ct), _ptr(coarse_flux, ct), _ptr(fine_flux, ct), _ptr(faces, C.c_int), len(faces), dt_c, dh_c)
+    return coarse_out
+
+
+def restrict(fine_out, coarse_out, rmap):
+    """In place on coarse_out: every fine group of rmap[n,5] = (fine_group, coarse_group, pi, pj, pk) replaces the 8^3
+    coarse cells starting at (pi, pj, pk) by the means of its 2x2x2 fine cells."""
+    rmap = np.ascontiguousarray(rmap, np.int32).reshape(-1, 5)
+    assert coarse_out.flags.c_contiguous and fine_out.flags.c_contiguous
+    fn, ct = _amr_fn("restrict", coarse_out.dtype.type)
+    fn.argtypes = [C.POINTER(ct), C.POINTER(ct), C.POINTER(C.c_int), C.c_int]
+    fn(_ptr(fine_out, ct), _ptr(coarse_out, ct), _ptr(rmap, C.c_int), len(rmap))
+    return coarse_out
+
+
+def flux_accum(acc, ff, w):
+    """acc += w * ff (dt-weighted time average of the fine fluxes over sub-steps)."""
+    fn, ct = _amr_fn("flux_accum", acc.dtype.type)
+    fn.argtypes = [C.POINTER(ct), C.POINTER(ct), C.c_longlong, ct]
+    fn(_ptr(acc, ct), _ptr(np.ascontiguousarray(ff), ct), acc.size, w)
+    return acc
+
+
 def max_threads():
     return int(lib().oracle_max_threads())

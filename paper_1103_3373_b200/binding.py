@@ -23,7 +23,8 @@ EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64",
            "hydro_pipeline_destroy", "hydro_pipeline_solve_f32", "hydro_pipeline_solve_f64", "hydro_min_ghost",
            "hydro_solve_grid_f32", "hydro_solve_grid_f64", "hydro_gather_f32", "hydro_gather_f64", "hydro_scatter_f32", "hydro_scatter_f64",
            "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror",
-           "hydro_alu_peak_launch")
+           "hydro_alu_peak_launch", "hydro_fluxfix_f32", "hydro_fluxfix_f64", "hydro_restrict_f32", "hydro_restrict_f64",
+           "hydro_flux_accum_f32", "hydro_flux_accum_f64")
 
 
 class HydroOpts(C.Structure):
@@ -56,6 +57,9 @@ def lib():
             getattr(L, "hydro_solve_" + name).argtypes = [vp, vp, vp, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
             getattr(L, "hydro_dt_" + name).argtypes = [vp, i, i, ft, i, vp, vp]
             getattr(L, "hydro_solve_grid_" + name).argtypes = [vp, vp, i, i, i, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
+            getattr(L, "hydro_fluxfix_" + name).argtypes = [vp, vp, vp, vp, i, ft, ft, vp]
+            getattr(L, "hydro_restrict_" + name).argtypes = [vp, vp, vp, i, vp]
+            getattr(L, "hydro_flux_accum_" + name).argtypes = [vp, vp, C.c_longlong, ft, vp]
             getattr(L, "hydro_pipeline_solve_" + name).argtypes = [vp, vp, vp, vp, i, ft, ft, ft, i, i, i,
                                                                    C.POINTER(HydroOpts), vp, vp]
         L.hydro_pipeline_create.argtypes = [C.POINTER(vp), i, i, i, i]
@@ -211,6 +215,46 @@ def hydro_alu_peak_launch(kind, blocks, threads, iters, scratch, *, stream=None)
     if rc != 0:
         raise HydroError(rc, "hydro_alu_peak_launch")
     return ops.value
+
+
+def _stream(t, stream):
+    return (stream or torch.cuda.current_stream(t.device)).cuda_stream
+
+
+def hydro_fluxfix(coarse_out, coarse_flux, fine_flux, faces, dt_c, dh_c, *, stream=None):
+    """hydro_fluxfix_f32/f64: in place on coarse_out[Nc,5,16,16,16]; faces: CUDA int32 [n,7]."""
+    sfx, ft = _suffix(coarse_out)
+    if faces.dtype != torch.int32 or not faces.is_cuda or not faces.is_contiguous():
+        raise ValueError("hydro_fluxfix: faces must be a contiguous CUDA int32 tensor [n,7]")
+    with torch.cuda.device(coarse_out.device):
+        rc = getattr(lib(), "hydro_fluxfix_" + sfx)(coarse_out.data_ptr(), coarse_flux.data_ptr(), fine_flux.data_ptr(),
+                                                    faces.data_ptr(), faces.shape[0], ft(dt_c), ft(dh_c), _stream(coarse_out, stream))
+    if rc != 0:
+        raise HydroError(rc, "hydro_fluxfix_" + sfx)
+    return coarse_out
+
+
+def hydro_restrict(fine_out, coarse_out, rmap, *, stream=None):
+    """hydro_restrict_f32/f64: in place on coarse_out; rmap: CUDA int32 [n,5]."""
+    sfx, _ = _suffix(coarse_out)
+    if rmap.dtype != torch.int32 or not rmap.is_cuda or not rmap.is_contiguous():
+        raise ValueError("hydro_restrict: map must be a contiguous CUDA int32 tensor [n,5]")
+    with torch.cuda.device(coarse_out.device):
+        rc = getattr(lib(), "hydro_restrict_" + sfx)(fine_out.data_ptr(), coarse_out.data_ptr(), rmap.data_ptr(), rmap.shape[0],
+                                                     _stream(coarse_out, stream))
+    if rc != 0:
+        raise HydroError(rc, "hydro_restrict_" + sfx)
+    return coarse_out
+
+
+def hydro_flux_accum(acc, face_flux, w, *, stream=None):
+    """hydro_flux_accum_f32/f64: acc += w * face_flux (same shape, contiguous)."""
+    sfx, ft = _suffix(acc)
+    with torch.cuda.device(acc.device):
+        rc = getattr(lib(), "hydro_flux_accum_" + sfx)(acc.data_ptr(), face_flux.data_ptr(), acc.numel(), ft(w), _stream(acc, stream))
+    if rc != 0:
+        raise HydroError(rc, "hydro_flux_accum_" + sfx)
+    return acc
 
 
 BC_PERIODIC, BC_OUTFLOW = 0, 1

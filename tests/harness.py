@@ -65,3 +65,44 @@ class CudaBackend:
                                      impl=self.impl, **kw)
         torch.cuda.synchronize()
         return out.cpu().numpy(), (ff.cpu().numpy() if ff is not None else None), status.cpu().numpy()
+
+
+# ---- two-level (coarse + one refined patch) step: plumbing for the flux fix-up / restriction tests ----
+def two_level_lists(origin, N):
+    """Index lists for ONE refined coarse patch whose first coarse cell is origin = (ox, oy, oz) (multiples of 8) in a periodic
+    N^3 coarse grid: faces[6,7] = (fine_group, dir, fine_side, coarse_group, ci, cj, ck) and rmap[1,5] (see include/hydro.h)."""
+    G = N // 16
+    gidx = lambda c: ((c[2] // 16) * G + (c[1] // 16)) * G + (c[0] // 16)
+    faces = []
+    for d in range(3):
+        for side in (0, 1):
+            c0 = list(origin)
+            c0[d] = (origin[d] - 1) % N if side == 0 else (origin[d] + 8) % N
+            faces.append([0, d, side, gidx(c0), c0[0] % 16, c0[1] % 16, c0[2] % 16])
+    rmap = [[0, gidx(origin), origin[0] % 16, origin[1] % 16, origin[2] % 16]]
+    return np.array(faces, np.int32), np.array(rmap, np.int32)
+
+
+def two_level_step(backend, amr, Uc, Uf, origin, dt, dh_c, gamma, scheme, riemann, limiter, *, recon=0, fix=True, **kw):
+    """One step of a periodic coarse grid Uc[5,N,N,N] with one refined patch Uf[5,16,16,16] covering the coarse cells
+    origin .. origin+8 (same dt on both levels; fine ghost zones by piecewise-constant injection of the coarse data).
+    `backend` supplies hydro_solve, `amr` supplies restrict(fine_out, coarse_out, rmap) and fluxfix(coarse_out, coarse_flux,
+    fine_flux, faces, dt, dh_c) -- the oracle module or a CUDA adapter.  Returns (Uc_new, Uf_new)."""
+    from oracle import oracle as O  # min_ghost only (a table lookup)
+    g = O.min_ghost(scheme, recon)
+    N = Uc.shape[1]
+    ox, oy, oz = origin
+    Gc = wl.grid_to_groups(Uc, g, "periodic")
+    up = np.repeat(np.repeat(np.repeat(Uc, 2, 1), 2, 2), 2, 3)
+    up[:, 2 * oz:2 * oz + 16, 2 * oy:2 * oy + 16, 2 * ox:2 * ox + 16] = Uf
+    upp = np.pad(up, ((0, 0), (g, g), (g, g), (g, g)), mode="wrap")
+    S = 16 + 2 * g
+    Gf = np.ascontiguousarray(upp[None, :, 2 * oz:2 * oz + S, 2 * oy:2 * oy + S, 2 * ox:2 * ox + S])
+    out_c, ff_c, _ = backend.solve(Gc, dt, dh_c, gamma, scheme, riemann, limiter, recon=recon, **kw)
+    out_f, ff_f, _ = backend.solve(Gf, dt, 0.5 * dh_c, gamma, scheme, riemann, limiter, recon=recon, **kw)
+    faces, rmap = two_level_lists(origin, N)
+    out_c = np.ascontiguousarray(out_c)
+    amr.restrict(np.ascontiguousarray(out_f), out_c, rmap)
+    if fix:
+        amr.fluxfix(out_c, np.ascontiguousarray(ff_c), np.ascontiguousarray(ff_f), faces, dt, dh_c)
+    return wl.groups_to_grid(out_c, Uc.shape[1:]), out_f[0]
