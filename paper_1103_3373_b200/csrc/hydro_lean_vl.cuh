@@ -175,7 +175,16 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
         const int ap = a - 1;  // plane whose half step is complete now
         const bool ap_in = ap >= 0 && ap < PS;
         if (ap >= -E && (ap_in || c_int)) {
-          V5<R> U = prim2cons(Wprev, p);
+          // U^n of plane a-1 (the half step starts from U^n): rebuilt from the primitives held in registers, which
+          // is U^n to rounding -- unless a floor changed them: then the raw conserved state is re-read (L2-resident)
+          V5<R> U;
+          if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) {
+            const R* gp = gin0 + (ptrdiff_t)ap * SS;
+#pragma unroll
+            for (int q = 0; q < 5; ++q) { U[q] = __ldg(gp); gp += nS; }
+          } else {
+            U = prim2cons(Wprev, p);
+          }
 #pragma unroll
           for (int q = 0; q < 5; ++q) U[q] = U[q] - p.hnu * (s1prev[q] + (f1z[q] - f1zprev[q]));
           stv(hring + ((ap + E) % NW) * 5 * HPL, HPL, hb, Op::c2p(U, p, c));

@@ -270,7 +270,7 @@ def test_config5_turbulence_small(B, oracle, nthreads, dtype):
         Ug, _, stg, _ = run_grid(CudaBackend(impl), U0.copy(), steps, 1.0 / N, gamma, CTU, EXACT, VANLEER, recon=PPM,
                                  cfl=0.5)
         if dtype == np.float64:
-            assert err_max(Ug[None], Ur[None]) <= steps * TOL64, impl
+            assert err_max(Ug[None], Ur[None]) <= TOL64, impl  # the bar itself after 5 steps, as config 1 after 20
         else:
             assert err_l1(Ug[None], Ur[None]) <= steps * TOL32, impl
         assert stg[2] == 0 and str_[2] == 0
@@ -311,7 +311,7 @@ def test_config3_full_size_sampled(B, oracle, nthreads, dtype):
     assert status.cpu().tolist() == [0, 0, 0]
     # the whole-batch reduction against the oracle's (order-independent maximum)
     rng = np.random.default_rng(7)
-    pick = np.sort(np.concatenate([[0, 1, 147, 148, 295, 296, Ng - 1], rng.choice(Ng, 25, replace=False)]))
+    pick = np.sort(np.unique(np.concatenate([[0, 1, 147, 148, 295, 296, Ng - 1], rng.choice(Ng, 60, replace=False)])))[:64]  # 64 groups
     Gs = u[torch.from_numpy(pick).cuda()].cpu().numpy()
     s_gpu = dtype(smax.item())
     s_ref = max(oracle.hydro_dt(u[k:k + 512].cpu().numpy(), gamma, 0) for k in range(0, Ng, 512))
