@@ -59,7 +59,7 @@ enum { HYDRO_GMINMOD = 0, HYDRO_VANLEER = 1, HYDRO_VANALBADA = 2, HYDRO_HYBRID =
 enum { HYDRO_PLM = 0, HYDRO_PPM = 1 };                                     /* recon */
 /* kernel organisation (both compute the same update): staged = one phase per stage with global scratch (any
  * variant, any ghost width); fused = z-marching, every intermediate on chip, phase-crossing state in shared
- * memory (CTU; two CTAs per SM where the tiles allow).  AUTO picks fused when it exists and its tiles fit. */
+ * memory (CTU, MHM and VL; two CTAs per SM where the tiles allow).  AUTO picks fused when it exists and its tiles fit. */
 enum { HYDRO_IMPL_AUTO = 0, HYDRO_IMPL_STAGED = 1, HYDRO_IMPL_FUSED = 2 };
 
 enum {
@@ -83,8 +83,9 @@ typedef struct hydro_opts {      /* NULL => all defaults */
   double min_dens;      /* density floor, 0 => none (default)                                        */
   double min_pres;      /* pressure floor, 0 => none (default)                                       */
   long long* status;    /* device long long[3] or NULL; accumulated atomically:
-                           [0] Roe failures, [1] non-positive rho or P seen by a conversion,
-                           [2] exact-solver vacuum / non-convergence                                 */
+                           [0] Roe failures, [1] non-positive rho or P seen by a conversion (the fp32 fused CTU kernel
+                           with default options counts (thread, plane) pairs that met one, not single conversions:
+                           non-zero exactly when the others are), [2] exact-solver vacuum / non-convergence   */
   void* workspace;      /* device scratch for the staged path (hydro_workspace_bytes); else NULL     */
   size_t workspace_bytes;
   int impl;             /* HYDRO_IMPL_AUTO: a fused z-marching kernel when one exists and fits, else staged */
@@ -154,6 +155,23 @@ HYDRO_API int hydro_solve_grid_f32(const float* grid_in, float* grid_out, int nx
                          float gamma, int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream);
 HYDRO_API int hydro_solve_grid_f64(const double* grid_in, double* grid_out, int nx, int ny, int nz, int bc, double dt, double dh,
                          double gamma, int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream);
+
+/* `steps` updates of a UNIFORM grid without leaving the device (the paper's preparation / solver / closing
+ * cycle, with the evolution time-step of PAPER.md:137 formed on the device): hydro_dt of the start state once,
+ * then per step dt = opts->cfl * dh / max_speed, the update, and the wave speed of the new state for the next step (fused into
+ * the update, hydro_opts::next_max_speed).  Variants hydro_solve_grid_* covers run ONE launch per step between `grid` and a
+ * second grid in `work` (unless opts->nghost is set, which asks for the group path); the others run hydro_gather -> hydro_solve -> hydro_scatter with the group buffers (and the staged
+ * scratch, if that path is taken) in `work`.  grid: device [5][nz][ny][nx], updated in place.  opts: required; cfl > 0;
+ * recon, nghost (0 = minimum), char_limit, floors, roe_fallback, status, impl as in hydro_solve_*; max_speed, next_max_speed,
+ * workspace are ignored.  work: device scratch of hydro_advance_workspace_bytes(...), 256-byte aligned, caller-owned.
+ * elapsed: device double or NULL; the sum of the steps' dt is ADDED to it (by a one-thread kernel on `stream`).
+ * Asynchronous on `stream`, no host synchronisation, capturable in a CUDA graph.  Errors as hydro_solve_*, plus
+ * HYDRO_E_COUNT (steps < 0), HYDRO_E_WORKSPACE (work too small), HYDRO_E_VALUE (opts NULL or cfl <= 0). */
+HYDRO_API size_t hydro_advance_workspace_bytes(int nx, int ny, int nz, int precision_bytes, int scheme, int limiter, const hydro_opts* opts);
+HYDRO_API int hydro_advance_f32(float* grid, int nx, int ny, int nz, int bc, int steps, float dh, float gamma, int scheme, int riemann,
+                                int limiter, const hydro_opts* opts, void* work, size_t work_bytes, double* elapsed, hydro_stream_t stream);
+HYDRO_API int hydro_advance_f64(double* grid, int nx, int ny, int nz, int bc, int steps, double dh, double gamma, int scheme, int riemann,
+                                int limiter, const hydro_opts* opts, void* work, size_t work_bytes, double* elapsed, hydro_stream_t stream);
 
 /* Consumer of face_flux: coarse-fine flux fix-up and fine -> coarse restriction after the fluid update of two adjacent AMR
  * levels (section 2 step 5: the stored fluxes are "only necessary in AMR"; section 4.3: the

@@ -23,7 +23,7 @@ EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64",
            "hydro_pipeline_destroy", "hydro_pipeline_solve_f32", "hydro_pipeline_solve_f64", "hydro_min_ghost",
            "hydro_solve_grid_f32", "hydro_solve_grid_f64", "hydro_gather_f32", "hydro_gather_f64", "hydro_scatter_f32", "hydro_scatter_f64",
            "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror",
-           "hydro_alu_peak_launch", "hydro_fluxfix_f32", "hydro_fluxfix_f64", "hydro_restrict_f32", "hydro_restrict_f64",
+           "hydro_alu_peak_launch", "hydro_advance_f32", "hydro_advance_f64", "hydro_advance_workspace_bytes", "hydro_fluxfix_f32", "hydro_fluxfix_f64", "hydro_restrict_f32", "hydro_restrict_f64",
            "hydro_flux_accum_f32", "hydro_flux_accum_f64")
 
 
@@ -57,6 +57,7 @@ def lib():
             getattr(L, "hydro_solve_" + name).argtypes = [vp, vp, vp, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
             getattr(L, "hydro_dt_" + name).argtypes = [vp, i, i, ft, i, vp, vp]
             getattr(L, "hydro_solve_grid_" + name).argtypes = [vp, vp, i, i, i, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
+            getattr(L, "hydro_advance_" + name).argtypes = [vp, i, i, i, i, i, ft, ft, i, i, i, C.POINTER(HydroOpts), vp, sz, vp, vp]
             getattr(L, "hydro_fluxfix_" + name).argtypes = [vp, vp, vp, vp, i, ft, ft, vp]
             getattr(L, "hydro_restrict_" + name).argtypes = [vp, vp, vp, i, vp]
             getattr(L, "hydro_flux_accum_" + name).argtypes = [vp, vp, C.c_longlong, ft, vp]
@@ -76,6 +77,8 @@ def lib():
         L.hydro_staged_workspace_bytes.argtypes = [i, i, i, i]
         L.hydro_staged_workspace_bytes.restype = sz
         L.hydro_alu_peak_launch.argtypes = [i, i, i, i, vp, C.POINTER(C.c_double), vp]
+        L.hydro_advance_workspace_bytes.argtypes = [i, i, i, i, i, i, C.POINTER(HydroOpts)]
+        L.hydro_advance_workspace_bytes.restype = sz
         L.hydro_strerror.argtypes = [i]
         L.hydro_strerror.restype = C.c_char_p
         _lib = L
@@ -106,18 +109,12 @@ def hydro_workspace_bytes(Ng, dtype, scheme, recon=PLM, impl=IMPL_AUTO, nghost=0
     return 0
 
 
-_ws_cache = {}
-
-
 def _workspace(nbytes, device):
-    """Caller-owned scratch for the staged path, cached per device and grown on demand."""
+    """A fresh caller-owned scratch tensor for the staged path (nothing is cached between calls: two calls on different
+    streams must not share scratch; pass workspace= to reuse one)."""
     if nbytes == 0:
         return None
-    w = _ws_cache.get(device)
-    if w is None or w.numel() < nbytes:
-        w = torch.empty(nbytes, dtype=torch.uint8, device=device)
-        _ws_cache[device] = w
-    return w
+    return torch.empty(nbytes, dtype=torch.uint8, device=device)
 
 
 def _suffix(t):
@@ -182,6 +179,8 @@ def hydro_solve(in_, dt, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *,
                                                   ft(dt), ft(dh), ft(gamma), scheme, riemann, limiter, C.byref(o), st)
     if rc != 0:
         raise HydroError(rc, "hydro_solve_" + sfx)
+    if ws is not None and stream is not None:
+        ws.record_stream(stream)  # the kernel may still be using it when the tensor goes back to the allocator
     return out, face_flux
 
 
@@ -317,92 +316,44 @@ def hydro_solve_grid(grid, dt, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLE
     return out
 
 
-def hydro_grid_mode(scheme, limiter, **optkw):
-    """True when hydro_solve_grid_* covers the variant: CTU with the default options."""
-    return (scheme == CTU and limiter == VANLEER and not optkw.get("char_limit") and not optkw.get("min_dens")
-            and not optkw.get("min_pres"))
+def hydro_advance_workspace_bytes(shape, dtype, scheme, limiter=VANLEER, **optkw):
+    """hydro_advance_workspace_bytes for a grid of shape (Nz, Ny, Nx)."""
+    o = make_opts(**optkw)
+    es = torch.empty((), dtype=dtype).element_size()
+    return lib().hydro_advance_workspace_bytes(shape[2], shape[1], shape[0], es, scheme, limiter, C.byref(o))
 
 
-def hydro_advance(grid, steps, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, cfl=0.5, bc=BC_PERIODIC, recon=PLM,
-                  nghost=0, status=None, graph=False, **optkw):
-    """`steps` updates of a uniform CUDA grid [5,Nz,Ny,Nx] without leaving the device: per step
-    hydro_gather -> hydro_solve (dt = cfl*dh/max_speed formed on the device; the update also reduces the wave speed
-    of the new state for the next step, so hydro_dt runs once, before the first step) -> hydro_scatter.
-    Returns (grid, t) with t a device scalar (fp64) holding the elapsed time; `grid` is updated in place.
-    No host synchronisation.  graph=True captures one step in a CUDA graph after the first step and replays it:
-    small grids are launch-bound (four launches and a memset per step)."""
-    if not nghost and hydro_grid_mode(scheme, limiter, **optkw):
-        return _advance_grid_mode(grid, steps, dh, gamma, scheme, riemann, limiter, cfl, bc, recon, status, graph, optkw)
-    g = nghost or hydro_min_ghost(scheme, recon)
-    shape = tuple(grid.shape[1:])
-    S = PS + 2 * g
-    Ng = (shape[0] // PS) * (shape[1] // PS) * (shape[2] // PS)
-    groups = torch.empty((Ng, 5, S, S, S), dtype=grid.dtype, device=grid.device)
-    out = torch.empty((Ng, 5, PS, PS, PS), dtype=grid.dtype, device=grid.device)
-    smax = torch.empty((), dtype=grid.dtype, device=grid.device)
-    snext = torch.empty((), dtype=grid.dtype, device=grid.device)
-    t = torch.zeros((), dtype=torch.float64, device=grid.device)
-    if steps <= 0:
-        return grid, t
+def hydro_advance(grid, steps, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *, cfl=0.5, bc=BC_PERIODIC, status=None,
+                  graph=False, workspace=None, elapsed=None, stream=None, **optkw):
+    """hydro_advance_f32/f64: `steps` updates of a uniform CUDA grid [5,Nz,Ny,Nx] in place, entirely on the device.
+    Returns (grid, t) with t a device fp64 scalar holding the elapsed time (`elapsed` if given: the steps' dt are added).
+    workspace: uint8 CUDA tensor of hydro_advance_workspace_bytes(...) (allocated if None).  graph=True captures the whole
+    call in a CUDA graph and replays it once (launch-bound small grids)."""
+    if not grid.is_cuda or not grid.is_contiguous() or grid.dim() != 4 or grid.shape[0] != 5:
+        raise ValueError("hydro_advance: grid must be a contiguous CUDA tensor [5,Nz,Ny,Nx]")
+    sfx, ft = _suffix(grid)
+    nz, ny, nx = grid.shape[1:]
+    o = make_opts(status=status, cfl=cfl, **optkw)
+    if workspace is None:
+        workspace = torch.empty(max(256, lib().hydro_advance_workspace_bytes(nx, ny, nz, grid.element_size(), scheme, limiter, C.byref(o))),
+                                dtype=torch.uint8, device=grid.device)
+    t = elapsed if elapsed is not None else torch.zeros((), dtype=torch.float64, device=grid.device)
 
-    def step():
-        hydro_gather(grid, g, bc, groups=groups)
-        hydro_solve(groups, 0.0, dh, gamma, scheme, riemann, limiter, out=out, face_flux=False, status=status,
-                    recon=recon, max_speed=smax, cfl=cfl, next_max_speed=snext, **optkw)
-        hydro_scatter(out, shape, grid=grid)
-        t.add_((cfl * dh) / smax.double())
-        smax.copy_(snext)
+    def call(st):
+        with torch.cuda.device(grid.device):
+            rc = getattr(lib(), "hydro_advance_" + sfx)(grid.data_ptr(), nx, ny, nz, bc, steps, ft(dh), ft(gamma), scheme, riemann,
+                                                        limiter, C.byref(o), workspace.data_ptr(), workspace.numel(), t.data_ptr(), st)
+        if rc != 0:
+            raise HydroError(rc, "hydro_advance_" + sfx)
 
-    hydro_dt(hydro_gather(grid, g, bc, groups=groups), gamma, 0, max_speed=smax)
-    step()
-    if graph and steps > 1:
+    if graph:
         cg = torch.cuda.CUDAGraph()
         torch.cuda.synchronize(grid.device)
         with torch.cuda.graph(cg):  # capture only records; nothing runs here
-            step()
-        for _ in range(steps - 1):
-            cg.replay()
+            call(torch.cuda.current_stream(grid.device).cuda_stream)
+        cg.replay()
     else:
-        for _ in range(steps - 1):
-            step()
-    return grid, t
-
-
-def _advance_grid_mode(grid, steps, dh, gamma, scheme, riemann, limiter, cfl, bc, recon, status, graph, optkw):
-    """hydro_advance through hydro_solve_grid_*: ONE launch per step (the kernel folds the ghost zones out of the grid,
-    forms dt from the previous step's fused wave-speed reduction and writes the new grid); two grids alternate."""
-    t = torch.zeros((), dtype=torch.float64, device=grid.device)
-    if steps <= 0:
-        return grid, t
-    other = torch.empty_like(grid)
-    sp = [torch.empty((), dtype=grid.dtype, device=grid.device) for _ in range(2)]
-    hydro_dt(hydro_gather(grid, 0, bc), gamma, 0, max_speed=sp[0])  # interiors only: the wave speed of the start state
-    bufs = [grid, other]
-
-    def step(k):
-        hydro_solve_grid(bufs[k & 1], 0.0, dh, gamma, scheme, riemann, limiter, bc=bc, out=bufs[(k + 1) & 1], status=status,
-                         recon=recon, max_speed=sp[k & 1], cfl=cfl, next_max_speed=sp[(k + 1) & 1], **optkw)
-        t.add_((cfl * dh) / sp[k & 1].double())
-
-    if graph and steps > 2:
-        step(0)
-        cg = torch.cuda.CUDAGraph()
-        torch.cuda.synchronize(grid.device)
-        with torch.cuda.graph(cg):  # two steps per replay: the buffers alternate
-            step(1)
-            step(2)
-        pairs, rest = divmod(steps - 1, 2)
-        for _ in range(pairs):
-            cg.replay()
-        if rest:
-            step(1)
-        last = 1 if steps % 2 else 0
-    else:
-        for k in range(steps):
-            step(k)
-        last = steps & 1
-    if last:  # the result sits in the scratch grid: hand it back in the caller's tensor
-        grid.copy_(other)
+        call(_stream(grid, stream))
     return grid, t
 
 

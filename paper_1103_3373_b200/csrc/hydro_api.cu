@@ -12,6 +12,10 @@
 
 namespace hydro {
 
+// gather / scatter of hydro_grid.cu, for hydro_advance
+template <class R> int gather_impl_fwd(const R* grid, R* groups, int nx, int ny, int nz, int nghost, int bc, cudaStream_t st);
+template <class R> int scatter_impl_fwd(const R* out, R* grid, int nx, int ny, int nz, cudaStream_t st);
+
 // ---- dispatch tables ---------------------------------------------------------------------------
 #define DECL_STAGED(R, S, RC, RS) extern template cudaError_t launch_staged<R, S, RC, RS>(const SolveArgs<R>&);
 #define DECL_LEAN(R, S, RC, RS) extern template cudaError_t launch_lean<R, S, RC, RS>(const SolveArgs<R>&);
@@ -161,7 +165,8 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   const int g = (o && o->nghost) ? o->nghost : gmin;
   if (g < gmin || g > 8) return HYDRO_E_GHOST;
   const double theta = (o && o->minmod_coeff != 0.0f) ? (double)o->minmod_coeff : 1.5;
-  if (!(gamma > R(1)) || !(dh > R(0)) || !(dt >= R(0)) || !(theta >= 1.0 && theta <= 2.0)) return HYDRO_E_VALUE;
+  const bool device_dt = o && o->max_speed;  // then the `dt` argument is ignored (hydro.h): do not validate it
+  if (!(gamma > R(1)) || !(dh > R(0)) || (!device_dt && !(dt >= R(0))) || !(theta >= 1.0 && theta <= 2.0)) return HYDRO_E_VALUE;
   if (o && (!(o->min_dens >= 0.0) || !(o->min_pres >= 0.0))) return HYDRO_E_VALUE;
   if (o && o->max_speed && (!(o->cfl > 0.0) || ((uintptr_t)o->max_speed & (sizeof(R) - 1)))) return HYDRO_E_VALUE;
   if (o && o->next_max_speed && (((uintptr_t)o->next_max_speed & (sizeof(R) - 1)) || o->next_max_speed == o->max_speed)) return HYDRO_E_ALIGN;
@@ -169,7 +174,7 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   par.gamma = gamma;
   par.gm1 = gamma - R(1);
   par.igm1 = R(1) / par.gm1;
-  par.nu = dt / dh;
+  par.nu = device_dt ? R(0) : dt / dh;
   par.hnu = R(0.5) * par.nu;
   par.theta = (R)theta;
   par.min_dens = o ? (R)o->min_dens : R(0);
@@ -194,7 +199,10 @@ static int solve_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, i
   Plan pl;
   const int rc = make_plan<R>(in, out, ff, Ng, dt, dh, gamma, scheme, riemann, limiter, o, true, a.par, pl);
   if (rc != HYDRO_OK) return rc;
-  if (Ng == 0) return HYDRO_OK;
+  if (Ng == 0) {  // no-op, but the reduction of an empty update is defined: 0, as hydro_dt of no groups
+    if (a.par.next_speed) return (int)cudaMemsetAsync(a.par.next_speed, 0, sizeof(R), st);
+    return HYDRO_OK;
+  }
   a.in = in;
   a.out = out;
   a.face_flux = ff;
@@ -263,6 +271,105 @@ static int solve_grid_impl(const R* gin, R* gout, int nx, int ny, int nz, int bc
   return (int)lean_fn<R>(scheme, pl.recon, riemann)(a);
 }
 
+// variants hydro_solve_grid_* covers (one launch per step, ghost zones folded out of the grid by the fused kernel)
+static bool grid_mode_ok(int scheme, int limiter, const hydro_opts* o) {
+  const bool fast = limiter == LIM_VANLEER && !(o && o->char_limit) && !(o && o->min_dens > 0.0) && !(o && o->min_pres > 0.0);
+  return scheme == SCHEME_CTU && fast;
+}
+
+// ---- hydro_advance: the multi-step driver of a uniform grid, entirely on the device ----------------
+// elapsed time: t += cfl dh / max_speed in fp64, by one thread on the stream (the solver kernels take dt/dh = cfl / max_speed
+// from the same scalar, hydro_opts::max_speed)
+template <class R> __global__ void advance_time_kernel(double* t, const R* max_speed, double cfl_dh) { *t += cfl_dh / (double)*max_speed; }
+
+constexpr size_t ADV_HEAD = 256;  // workspace head: two speed scalars (ping-pong) at offsets 0 and 64
+template <class R> static size_t advance_bytes(int nx, int ny, int nz, int scheme, int limiter, const hydro_opts* o) {
+  const size_t cells = (size_t)nx * ny * nz, Ng = cells / (PS * PS * PS);
+  if (grid_mode_ok(scheme, limiter, o) && !(o && o->nghost)) return ADV_HEAD + 5 * cells * sizeof(R);  // the second grid
+  const int recon = o ? o->recon : 0;
+  const int g = (o && o->nghost) ? o->nghost : min_ghost(scheme, recon);
+  const size_t S = PS + 2 * g;
+  size_t b = ADV_HEAD + Ng * 5 * (S * S * S + (size_t)PS * PS * PS) * sizeof(R);  // padded groups + updated interiors
+  b = (b + 255) & ~(size_t)255;
+  if (!lean_fits((int)sizeof(R), scheme, recon, g) || (o && o->impl == HYDRO_IMPL_STAGED))
+    b += hydro_staged_workspace_bytes((int)(Ng < 0x7fffffff ? Ng : 0x7fffffff), (int)sizeof(R), scheme, recon);
+  return b;
+}
+
+template <class R>
+static int advance_impl(R* grid, int nx, int ny, int nz, int bc, int steps, R dh, R gamma, int scheme, int riemann, int limiter,
+                        const hydro_opts* o, void* work, size_t work_bytes, double* t_accum, cudaStream_t st) {
+  if (steps < 0) return HYDRO_E_COUNT;
+  if (nx < 0 || ny < 0 || nz < 0 || nx % PS || ny % PS || nz % PS) return HYDRO_E_VALUE;
+  if (bc < 0 || bc > 1) return HYDRO_E_ENUM;
+  if (scheme < 0 || scheme > 2 || riemann < 0 || riemann > 3 || limiter < 0 || limiter > 3) return HYDRO_E_ENUM;
+  if (!o || !(o->cfl > 0.0)) return HYDRO_E_VALUE;
+  if (o->recon < 0 || o->recon > 1) return HYDRO_E_ENUM;
+  const size_t cells = (size_t)nx * ny * nz;
+  if (steps == 0 || cells == 0) return HYDRO_OK;
+  if (!grid || !work) return HYDRO_E_NULL;
+  if (((uintptr_t)grid & 15) || ((uintptr_t)work & 255) || (t_accum && ((uintptr_t)t_accum & 7))) return HYDRO_E_ALIGN;
+  if (work_bytes < advance_bytes<R>(nx, ny, nz, scheme, limiter, o)) return HYDRO_E_WORKSPACE;
+  const long long Ngl = (long long)(cells / (PS * PS * PS));
+  if (Ngl > 0x7fffffffLL / 64) return HYDRO_E_COUNT;
+  const int Ng = (int)Ngl;
+  unsigned char* w = static_cast<unsigned char*>(work);
+  R* sp[2] = {reinterpret_cast<R*>(w), reinterpret_cast<R*>(w + 64)};
+  hydro_opts oo = *o;
+  oo.max_speed = nullptr;
+  oo.next_max_speed = nullptr;
+  const double cfl_dh = o->cfl * (double)dh;
+  int rc;
+  if (grid_mode_ok(scheme, limiter, o) && !o->nghost) {  // an explicit ghost width asks for the group path
+    R* other = reinterpret_cast<R*>(w + ADV_HEAD);
+    R* buf[2] = {grid, other};
+    // wave speed of the start state: the interiors only (a gather with ghost width 0 into the second grid, used as scratch)
+    rc = gather_impl_fwd<R>(grid, other, nx, ny, nz, 0, bc, st);
+    if (rc != HYDRO_OK) return rc;
+    rc = dt_impl<R>(other, Ng, 0, gamma, 0, sp[0], st);
+    if (rc != HYDRO_OK) return rc;
+    for (int k = 0; k < steps; ++k) {
+      oo.max_speed = sp[k & 1];
+      oo.next_max_speed = sp[(k + 1) & 1];
+      if (t_accum) advance_time_kernel<R><<<1, 1, 0, st>>>(t_accum, sp[k & 1], cfl_dh);
+      rc = solve_grid_impl<R>(buf[k & 1], buf[(k + 1) & 1], nx, ny, nz, bc, R(0), dh, gamma, scheme, riemann, limiter, &oo, st);
+      if (rc != HYDRO_OK) return rc;
+    }
+    if (steps & 1) {  // the result sits in the scratch grid: hand it back in the caller's
+      const cudaError_t e = cudaMemcpyAsync(grid, other, 5 * cells * sizeof(R), cudaMemcpyDeviceToDevice, st);
+      if (e != cudaSuccess) return (int)e;
+    }
+    return HYDRO_OK;
+  }
+  const int recon = o->recon;
+  const int g = o->nghost ? o->nghost : min_ghost(scheme, recon);
+  if (g < min_ghost(scheme, recon) || g > 8) return HYDRO_E_GHOST;
+  const size_t S = PS + 2 * g;
+  R* groups = reinterpret_cast<R*>(w + ADV_HEAD);
+  R* out = groups + (size_t)Ng * 5 * S * S * S;
+  size_t used = ADV_HEAD + (size_t)Ng * 5 * (S * S * S + (size_t)PS * PS * PS) * sizeof(R);
+  used = (used + 255) & ~(size_t)255;
+  oo.nghost = g;
+  oo.workspace = w + used;
+  oo.workspace_bytes = work_bytes - used;
+  for (int k = 0; k < steps; ++k) {
+    rc = gather_impl_fwd<R>(grid, groups, nx, ny, nz, g, bc, st);
+    if (rc != HYDRO_OK) return rc;
+    if (k == 0) {
+      rc = dt_impl<R>(groups, Ng, g, gamma, 0, sp[0], st);
+      if (rc != HYDRO_OK) return rc;
+    }
+    oo.max_speed = sp[k & 1];
+    oo.next_max_speed = sp[(k + 1) & 1];
+    if (t_accum) advance_time_kernel<R><<<1, 1, 0, st>>>(t_accum, sp[k & 1], cfl_dh);
+    rc = solve_impl<R>(groups, out, nullptr, Ng, R(0), dh, gamma, scheme, riemann, limiter, &oo, st);
+    if (rc != HYDRO_OK) return rc;
+    rc = scatter_impl_fwd<R>(out, grid, nx, ny, nz, st);
+    if (rc != HYDRO_OK) return rc;
+  }
+  return HYDRO_OK;
+}
+
 }  // namespace hydro
 
 // ---- the host-buffer streaming pipeline ---------------------------------------
@@ -296,6 +403,7 @@ static int pipeline_solve(hydro_pipeline* p, const R* in, R* out, R* ff, int Ng,
   if (pl.impl == HYDRO_IMPL_STAGED) {
     const size_t need = hydro_staged_workspace_bytes(p->chunk, p->prec, scheme, pl.recon);
     if (p->ws_bytes < need) {  // (re)allocate per-stream scratch once for this variant
+      p->ws_bytes = 0;  // nothing usable until every stream has its new scratch
       for (auto& w : p->d_ws) { if (w) cudaFree(w); w = nullptr; }
       for (auto& w : p->d_ws) if (cudaMalloc(&w, need) != cudaSuccess) return (int)cudaErrorMemoryAllocation;
       p->ws_bytes = need;
@@ -304,29 +412,36 @@ static int pipeline_solve(hydro_pipeline* p, const R* in, R* out, R* ff, int Ng,
   if (status_host) cudaMemsetAsync(p->d_status, 0, 3 * sizeof(long long), p->streams[0]);
   if (max_speed_host) cudaMemsetAsync(p->d_speed, 0, p->ns * sizeof(double), p->streams[0]);
   if (status_host || max_speed_host) cudaStreamSynchronize(p->streams[0]);
+  // on any failure: wait for the copies already in flight into the caller's buffers before returning the error
+  auto fail = [p](int code) {
+    for (auto s2 : p->streams) cudaStreamSynchronize(s2);
+    return code;
+  };
   int s = 0;
   for (int n0 = 0; n0 < Ng; n0 += p->chunk, s = (s + 1) % p->ns) {
     const int n = (Ng - n0 < p->chunk) ? Ng - n0 : p->chunk;
     cudaStream_t st = p->streams[s];
     cudaError_t e = cudaMemcpyAsync(p->d_in[s], in + (size_t)n0 * p->in_elems, (size_t)n * p->in_elems * sizeof(R),
                                     cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) return (int)e;
+    if (e != cudaSuccess) return fail((int)e);
     oo.workspace = p->d_ws[s];
     oo.workspace_bytes = p->ws_bytes;
     rc = solve_impl<R>((const R*)p->d_in[s], (R*)p->d_out[s], ff ? (R*)p->d_ff[s] : nullptr, n, dt, dh, gamma, scheme,
                        riemann, limiter, &oo, st);
-    if (rc != HYDRO_OK) return rc;
-    if (max_speed_host) {  // next step's CFL reduction while the chunk is still on the device
+    if (rc != HYDRO_OK) return fail(rc);
+    if (max_speed_host) {  // next step's CFL reduction while the chunk is still on the device: a running
+      // maximum per stream over its chunks (the update's fused reduction overwrites its scalar per launch; next to the PCIe
+      // copies this extra pass over `out` in HBM costs nothing measurable)
       rc = dt_impl<R>((const R*)p->d_out[s], n, 0, gamma, 0, reinterpret_cast<R*>(static_cast<double*>(p->d_speed) + s), st, true);
-      if (rc != HYDRO_OK) return rc;
+      if (rc != HYDRO_OK) return fail(rc);
     }
     e = cudaMemcpyAsync(out + (size_t)n0 * p->out_elems, p->d_out[s], (size_t)n * p->out_elems * sizeof(R),
                         cudaMemcpyDeviceToHost, st);
-    if (e != cudaSuccess) return (int)e;
+    if (e != cudaSuccess) return fail((int)e);
     if (ff) {
       e = cudaMemcpyAsync(ff + (size_t)n0 * p->ff_elems, p->d_ff[s], (size_t)n * p->ff_elems * sizeof(R),
                           cudaMemcpyDeviceToHost, st);
-      if (e != cudaSuccess) return (int)e;
+      if (e != cudaSuccess) return fail((int)e);
     }
   }
   for (auto st : p->streams) {
@@ -415,6 +530,23 @@ int hydro_solve_grid_f32(const float* grid_in, float* grid_out, int nx, int ny, 
 int hydro_solve_grid_f64(const double* grid_in, double* grid_out, int nx, int ny, int nz, int bc, double dt, double dh, double gamma,
                          int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream) {
   return hydro::solve_grid_impl<double>(grid_in, grid_out, nx, ny, nz, bc, dt, dh, gamma, scheme, riemann, limiter, opts, (cudaStream_t)stream);
+}
+size_t hydro_advance_workspace_bytes(int nx, int ny, int nz, int precision_bytes, int scheme, int limiter, const hydro_opts* opts) {
+  if (nx < 0 || ny < 0 || nz < 0 || nx % hydro::PS || ny % hydro::PS || nz % hydro::PS) return 0;
+  if (scheme < 0 || scheme > 2 || limiter < 0 || limiter > 3) return 0;
+  if (precision_bytes == 4) return hydro::advance_bytes<float>(nx, ny, nz, scheme, limiter, opts);
+  if (precision_bytes == 8) return hydro::advance_bytes<double>(nx, ny, nz, scheme, limiter, opts);
+  return 0;
+}
+int hydro_advance_f32(float* grid, int nx, int ny, int nz, int bc, int steps, float dh, float gamma, int scheme, int riemann, int limiter,
+                      const hydro_opts* opts, void* work, size_t work_bytes, double* elapsed, hydro_stream_t stream) {
+  return hydro::advance_impl<float>(grid, nx, ny, nz, bc, steps, dh, gamma, scheme, riemann, limiter, opts, work, work_bytes, elapsed,
+                                    (cudaStream_t)stream);
+}
+int hydro_advance_f64(double* grid, int nx, int ny, int nz, int bc, int steps, double dh, double gamma, int scheme, int riemann,
+                      int limiter, const hydro_opts* opts, void* work, size_t work_bytes, double* elapsed, hydro_stream_t stream) {
+  return hydro::advance_impl<double>(grid, nx, ny, nz, bc, steps, dh, gamma, scheme, riemann, limiter, opts, work, work_bytes, elapsed,
+                                     (cudaStream_t)stream);
 }
 int hydro_dt_f32(const float* u, int Ng, int nghost, float gamma, int norm, float* max_speed, hydro_stream_t stream) {
   return hydro::dt_impl<float>(u, Ng, nghost, gamma, norm, max_speed, (cudaStream_t)stream);

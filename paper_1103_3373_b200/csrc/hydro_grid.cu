@@ -109,6 +109,18 @@ template <class R> static int scatter_impl(const R* out, R* grid, int nx, int ny
   return (int)cudaGetLastError();
 }
 
+// entry points for hydro_advance (hydro_api.cu)
+template <class R> int gather_impl_fwd(const R* grid, R* groups, int nx, int ny, int nz, int nghost, int bc, cudaStream_t st) {
+  return gather_impl<R>(grid, groups, nx, ny, nz, nghost, bc, st);
+}
+template <class R> int scatter_impl_fwd(const R* out, R* grid, int nx, int ny, int nz, cudaStream_t st) {
+  return scatter_impl<R>(out, grid, nx, ny, nz, st);
+}
+template int gather_impl_fwd<float>(const float*, float*, int, int, int, int, int, cudaStream_t);
+template int gather_impl_fwd<double>(const double*, double*, int, int, int, int, int, cudaStream_t);
+template int scatter_impl_fwd<float>(const float*, float*, int, int, int, cudaStream_t);
+template int scatter_impl_fwd<double>(const double*, double*, int, int, int, cudaStream_t);
+
 }  // namespace hydro
 
 extern "C" {

@@ -17,10 +17,12 @@ def shard_range(Ng, rank, world):
 
 def global_max(speed):
     """In-place MAX all-reduce of the hydro_dt scalar (tensor on the rank's device).  NaN (a bad cell on any
-    rank) must win, as it does inside hydro_dt: collectives do not promise NaN propagation, so it is sent as +inf."""
+    rank) must win, as it does inside hydro_dt: collectives do not promise NaN propagation, so it travels as +inf and is
+    turned back into NaN afterwards (hydro_solve would read +inf as dt = 0 and silently do an identity update)."""
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
         return speed
     flag = torch.isnan(speed)
     speed.copy_(torch.where(flag, torch.full_like(speed, float("inf")), speed))
     dist.all_reduce(speed, op=dist.ReduceOp.MAX)
+    speed.copy_(torch.where(torch.isinf(speed), torch.full_like(speed, float("nan")), speed))
     return speed
