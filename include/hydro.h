@@ -204,6 +204,24 @@ HYDRO_API int hydro_restrict_f64(const double* fine_out, double* coarse_out, con
 HYDRO_API int hydro_flux_accum_f32(float* acc, const float* face_flux, long long n, float w, hydro_stream_t stream);
 HYDRO_API int hydro_flux_accum_f64(double* acc, const double* face_flux, long long n, double w, hydro_stream_t stream);
 
+/* The directionally SPLIT relaxing-TVD update: the scheme of the original GAMER ("RTVD; Jin & Xin
+ * 1995 ... with directional splitting") that the paper times next to the unsplit schemes as the contrast with one-dimensional
+ * stencils and low arithmetic intensity.  Same batch layouts as hydro_solve_* (in [Ng][5][S^3] with
+ * nghost >= 3, out [Ng][5][16^3], face_flux [Ng][9][5][16 x 16] or NULL).  Reading S26 of DESIGN.md: every conserved variable is
+ * split into right / left movers (c U +- F_d(U)) / 2 with the freezing speed c = |v_d| + c_s of its cell; one sweep = a
+ * first-order predictor to dt/2 and a corrector with van-Leer-limited MUSCL fluxes of the movers evaluated at the predicted
+ * state; one call = three sweeps with the same dt in the order x, y, z (order 0) or z, y, x (order 1; alternate them from step
+ * to step).  face_flux receives the corrector flux of each direction's sweep at the faces f = 0, 8, 16 (the flux that sweep
+ * used, so that the flux balance of hydro_solve_* holds).  opts: nghost (0 => 3), status ([1] counts non-positive rho / P),
+ * max_speed + cfl (dt formed on the device), workspace + workspace_bytes REQUIRED: hydro_rtvd_workspace_bytes(Ng, precision)
+ * (at least one slot of 5 x (22 x 22 x 16 + 22 x 16 x 16) elements; the kernel runs one CTA per slot).  No Riemann solver, no
+ * limiter choice, no floors.  Errors as hydro_solve_* (HYDRO_E_GHOST: nghost < 3; HYDRO_E_WORKSPACE; HYDRO_E_ENUM: order). */
+HYDRO_API size_t hydro_rtvd_workspace_bytes(int Ng, int precision_bytes);
+HYDRO_API int hydro_rtvd_solve_f32(const float* in, float* out, float* face_flux, int Ng, float dt, float dh, float gamma, int order,
+                                   const hydro_opts* opts, hydro_stream_t stream);
+HYDRO_API int hydro_rtvd_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int order,
+                                   const hydro_opts* opts, hydro_stream_t stream);
+
 /* Sizes and capabilities. */
 HYDRO_API int hydro_min_ghost(int scheme, int recon);                 /* 2/3 (MHM, CTU with PLM/PPM), 3/4 (VL)   */
 HYDRO_API int hydro_has_fused(int precision_bytes, int scheme, int recon, int riemann); /* 1 if a fused kernel exists */

@@ -9,7 +9,8 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "hydro_oracle.cpp")
-SRCS = [SRC, os.path.join(HERE, "amr_oracle.cpp")]  # the fluid update; the flux fix-up / restriction that consume its fluxes
+SRCS = [SRC, os.path.join(HERE, "amr_oracle.cpp"),  # the fluid update; the flux fix-up / restriction that consume its fluxes
+        os.path.join(HERE, "rtvd_oracle.cpp")]       # the directionally split relaxing-TVD update (the paper's contrast scheme)
 LIB = os.path.join(HERE, "liboracle.so")
 
 

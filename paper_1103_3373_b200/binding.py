@@ -24,7 +24,7 @@ EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64",
            "hydro_solve_grid_f32", "hydro_solve_grid_f64", "hydro_gather_f32", "hydro_gather_f64", "hydro_scatter_f32", "hydro_scatter_f64",
            "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror",
            "hydro_alu_peak_launch", "hydro_advance_f32", "hydro_advance_f64", "hydro_advance_workspace_bytes", "hydro_fluxfix_f32", "hydro_fluxfix_f64", "hydro_restrict_f32", "hydro_restrict_f64",
-           "hydro_flux_accum_f32", "hydro_flux_accum_f64")
+           "hydro_flux_accum_f32", "hydro_flux_accum_f64", "hydro_rtvd_solve_f32", "hydro_rtvd_solve_f64", "hydro_rtvd_workspace_bytes")
 
 
 class HydroOpts(C.Structure):
@@ -58,6 +58,7 @@ def lib():
             getattr(L, "hydro_dt_" + name).argtypes = [vp, i, i, ft, i, vp, vp]
             getattr(L, "hydro_solve_grid_" + name).argtypes = [vp, vp, i, i, i, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
             getattr(L, "hydro_advance_" + name).argtypes = [vp, i, i, i, i, i, ft, ft, i, i, i, C.POINTER(HydroOpts), vp, sz, vp, vp]
+            getattr(L, "hydro_rtvd_solve_" + name).argtypes = [vp, vp, vp, i, ft, ft, ft, i, C.POINTER(HydroOpts), vp]
             getattr(L, "hydro_fluxfix_" + name).argtypes = [vp, vp, vp, vp, i, ft, ft, vp]
             getattr(L, "hydro_restrict_" + name).argtypes = [vp, vp, vp, i, vp]
             getattr(L, "hydro_flux_accum_" + name).argtypes = [vp, vp, C.c_longlong, ft, vp]
@@ -77,6 +78,8 @@ def lib():
         L.hydro_staged_workspace_bytes.argtypes = [i, i, i, i]
         L.hydro_staged_workspace_bytes.restype = sz
         L.hydro_alu_peak_launch.argtypes = [i, i, i, i, vp, C.POINTER(C.c_double), vp]
+        L.hydro_rtvd_workspace_bytes.argtypes = [i, i]
+        L.hydro_rtvd_workspace_bytes.restype = sz
         L.hydro_advance_workspace_bytes.argtypes = [i, i, i, i, i, i, C.POINTER(HydroOpts)]
         L.hydro_advance_workspace_bytes.restype = sz
         L.hydro_strerror.argtypes = [i]
@@ -184,6 +187,40 @@ def hydro_solve(in_, dt, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLEER, *,
     return out, face_flux
 
 
+def _stream(t, stream):
+    return (stream or torch.cuda.current_stream(t.device)).cuda_stream
+
+
+def hydro_rtvd_solve(in_, dt, dh, gamma, order=0, *, out=None, face_flux=True, status=None, workspace=None, stream=None,
+                     max_speed=None, cfl=0.0):
+    """hydro_rtvd_solve_f32/f64: one directionally split relaxing-TVD step (sweeps x,y,z for order 0; z,y,x for order 1) of
+    in_[Ng,5,S,S,S] (ghost width >= 3).  Returns (out, face_flux or None).  workspace: uint8 CUDA tensor of
+    hydro_rtvd_workspace_bytes(Ng, precision) (allocated if None)."""
+    if not in_.is_cuda or not in_.is_contiguous() or in_.dim() != 5 or in_.shape[1] != 5:
+        raise ValueError("hydro_rtvd_solve: in_ must be a contiguous CUDA tensor [Ng,5,S,S,S]")
+    sfx, ft = _suffix(in_)
+    Ng, S = in_.shape[0], in_.shape[2]
+    g = (S - PS) // 2
+    if out is None:
+        out = torch.empty((Ng, 5, PS, PS, PS), dtype=in_.dtype, device=in_.device)
+    if face_flux is True:
+        face_flux = torch.empty((Ng, 9, 5, PS, PS), dtype=in_.dtype, device=in_.device)
+    elif face_flux is False:
+        face_flux = None
+    if workspace is None:
+        workspace = torch.empty(max(16, lib().hydro_rtvd_workspace_bytes(Ng, in_.element_size())), dtype=torch.uint8, device=in_.device)
+    o = make_opts(nghost=g, status=status, workspace=workspace, max_speed=max_speed, cfl=cfl)
+    with torch.cuda.device(in_.device):
+        rc = getattr(lib(), "hydro_rtvd_solve_" + sfx)(in_.data_ptr(), out.data_ptr(),
+                                                       face_flux.data_ptr() if face_flux is not None else None, Ng, ft(dt), ft(dh),
+                                                       ft(gamma), order, C.byref(o), _stream(in_, stream))
+    if rc != 0:
+        raise HydroError(rc, "hydro_rtvd_solve_" + sfx)
+    if stream is not None:
+        workspace.record_stream(stream)
+    return out, face_flux
+
+
 def hydro_dt(u, gamma, norm=0, *, max_speed=None, stream=None):
     """hydro_dt_f32/f64: device scalar tensor holding the maximum wave speed over interior cells."""
     if not u.is_cuda or not u.is_contiguous() or u.dim() != 5 or u.shape[1] != 5:
@@ -214,10 +251,6 @@ def hydro_alu_peak_launch(kind, blocks, threads, iters, scratch, *, stream=None)
     if rc != 0:
         raise HydroError(rc, "hydro_alu_peak_launch")
     return ops.value
-
-
-def _stream(t, stream):
-    return (stream or torch.cuda.current_stream(t.device)).cuda_stream
 
 
 def hydro_fluxfix(coarse_out, coarse_flux, fine_flux, faces, dt_c, dh_c, *, stream=None):

@@ -1,0 +1,190 @@
+// hydro_rtvd.cu -- the directionally SPLIT relaxing-TVD update of a batch of patch groups: the scheme of
+// the original GAMER (Jin & Xin 1995) that the paper times next to its unsplit schemes as the contrast with low
+// arithmetic intensity ("for the directionally split schemes ... the integration only requires 1D stencils").
+// Reading S26 of DESIGN.md (formulas in oracle/rtvd_oracle.cpp's header, restated here independently): every conserved variable
+// is split into a right- and a left-moving part advected with the freezing speed c = |v_d| + c_s; midpoint Runge-Kutta with a
+// first-order predictor and a van-Leer-limited MUSCL corrector; three sweeps per step, x,y,z (order 0) or z,y,x (order 1).
+//
+// Organisation: persistent CTAs, one patch group at a time; a thread owns one pencil of a sweep and marches along it with a
+// register window (two limiter stencils of movers, the predictor flux, the last corrector flux), so that every cell's movers
+// are evaluated once.  Sweep 1 reads `in`, sweep 3 writes `out`; the two intermediate boxes (only the range later sweeps still
+// need: 22x22x16 and 22x16x16 cells) live in a caller-supplied scratch slot per CTA that stays L2-resident.  ~110 flops against
+// ~85 bytes of HBM traffic per cell update: HBM-bound, unlike the Riemann-solver schemes.  Part of the CUDA product path.
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "../../include/hydro.h"
+#include "hydro_math.cuh"
+
+namespace hydro {
+
+constexpr int RT_G = 3, RT_W = PS + 2 * RT_G, RT_NT = 256;
+
+template <class R> struct Mv { V5<R> fr, fl; };
+// right / left movers of one cell for a sweep along D: (c U +- F_D(U)) / 2
+template <int D, class R> __device__ __forceinline__ Mv<R> rt_movers(const V5<R>& U, R gamma, int& bad) {
+  const R ir = m_rcp(U[0]);
+  const R vx = U[1] * ir, vy = U[2] * ir, vz = U[3] * ir;
+  const R P = (gamma - R(1)) * (U[4] - R(0.5) * U[0] * ((vx * vx + vy * vy) + vz * vz));
+  bad += (U[0] > R(0) && P > R(0)) ? 0 : 1;
+  const R vn = D == 0 ? vx : (D == 1 ? vy : vz);
+  const R c = m_abs(vn) + m_sqrt(gamma * P * ir);
+  V5<R> F;
+  F[0] = U[0] * vn; F[1] = U[1] * vn; F[2] = U[2] * vn; F[3] = U[3] * vn; F[4] = (U[4] + P) * vn;
+  F[1 + D] = F[1 + D] + P;
+  Mv<R> m;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    m.fr[q] = R(0.5) * (c * U[q] + F[q]);
+    m.fl[q] = R(0.5) * (c * U[q] - F[q]);
+  }
+  return m;
+}
+template <class R> __device__ __forceinline__ R rt_phi(R a, R b) {
+  const R p = a * b;
+  return p > R(0) ? m_div(p + p, a + b) : R(0);
+}
+
+// One sweep along D of the pencils (a, b), a in [0, na), b in [0, nb).  src cell (q, a, b, x) at src[q sq + a sa + b sb + x sx],
+// x = 0 .. 21; dst likewise for the 16 updated cells x - 3.  ff: plane base of direction D (3 planes x 5 x 256) or nullptr;
+// (a - fa0, b - fb0) are the in-plane interior coordinates of the pencil (lower axis fastest).
+template <int D, class R>
+__device__ __forceinline__ void rt_sweep(const R* __restrict__ src, size_t sq, int sa, int sb, int sx, R* __restrict__ dst, size_t dq,
+                                         int da, int db, int dx, int na, int nb, int fa0, int fb0, R* __restrict__ ff, R nu, R gamma,
+                                         int& bad) {
+  for (int pidx = threadIdx.x; pidx < na * nb; pidx += RT_NT) {
+    const int b = pidx / na, a = pidx - b * na;
+    const R* s = src + (size_t)a * sa + (size_t)b * sb;
+    R* d = dst + (size_t)a * da + (size_t)b * db;
+    const int ta = a - fa0, tb = b - fb0;
+    R* fp = (ff && ta >= 0 && ta < PS && tb >= 0 && tb < PS) ? ff + tb * PS + ta : nullptr;
+    V5<R> Uprev, frp, Glo, fr1a, fr1b, fl1b, Hlo;  // U[x-1], m[x-1].fr, G at the lower face of x-1, corrector windows
+    Mv<R> m1p;      // movers of u1[x-2]
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { Uprev[q] = frp[q] = Glo[q] = fr1a[q] = fr1b[q] = fl1b[q] = Hlo[q] = R(0); m1p.fr[q] = m1p.fl[q] = R(0); }
+#pragma unroll 1
+    for (int x = 0; x < RT_W; ++x) {
+      V5<R> U;
+#pragma unroll
+      for (int q = 0; q < 5; ++q) U[q] = s[q * sq + (size_t)x * sx];
+      const Mv<R> m = rt_movers<D>(U, gamma, bad);
+      if (x >= 1) {
+        V5<R> G;  // predictor flux at the face between x-1 and x
+#pragma unroll
+        for (int q = 0; q < 5; ++q) G[q] = frp[q] - m.fl[q];
+        if (x >= 2) {  // u1 of cell x-1, its movers, the corrector flux at the lower face of cell x-2, the update of cell x-3
+          V5<R> u1;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) u1[q] = Uprev[q] - R(0.5) * nu * (G[q] - Glo[q]);
+          const Mv<R> m1 = rt_movers<D>(u1, gamma, bad);  // cell x-1
+          if (x >= 5) {  // face f = x-2: right movers of cells f-2, f-1, f (fr1a, fr1b, m1p.fr), left movers of f-1, f, f+1 (fl1b, m1p.fl, m1.fl)
+            V5<R> H;
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+              const R frh = fr1b[q] + rt_phi(R(0.5) * (fr1b[q] - fr1a[q]), R(0.5) * (m1p.fr[q] - fr1b[q]));
+              const R flh = m1p.fl[q] - rt_phi(R(0.5) * (m1p.fl[q] - fl1b[q]), R(0.5) * (m1.fl[q] - m1p.fl[q]));
+              H[q] = frh - flh;
+            }
+            const int f = x - 2 - RT_G;  // face index of the group: 0 .. 16
+            if (fp && (f & 7) == 0) {
+#pragma unroll
+              for (int q = 0; q < 5; ++q) fp[((f >> 3) * 5 + q) * (PS * PS)] = H[q];
+            }
+            if (x >= 6) {  // cell x-3 = interior cell f-1
+#pragma unroll
+              for (int q = 0; q < 5; ++q)  // U[x-3] is re-read (an L1 hit) rather than carried through the window
+                d[q * dq + (size_t)(x - 3 - RT_G) * dx] = s[q * sq + (size_t)(x - 3) * sx] - nu * (H[q] - Hlo[q]);
+            }
+            Hlo = H;
+          }
+          fr1a = fr1b; fr1b = m1p.fr; fl1b = m1p.fl; m1p = m1;
+        }
+        Glo = G;
+      }
+      Uprev = U; frp = m.fr;
+    }
+  }
+}
+
+template <class R>
+__global__ void __launch_bounds__(RT_NT, sizeof(R) == 4 ? 2 : 1)
+rtvd_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, R nu_arg, R gamma, int order,
+            const R* __restrict__ max_speed, R cfl, R* __restrict__ scratch, long long* status) {
+  R nu = nu_arg;
+  if (max_speed) nu = m_div(cfl, __ldg(max_speed));
+  const int S = PS + 2 * g, o = g - RT_G;
+  const size_t nS = (size_t)S * S * S;
+  constexpr size_t N1 = (size_t)RT_W * RT_W * PS, N2 = (size_t)RT_W * PS * PS, NI = (size_t)PS * PS * PS;
+  R* s1 = scratch + (size_t)blockIdx.x * 5 * (N1 + N2);
+  R* s2 = s1 + 5 * N1;
+  int bad = 0;
+  for (int grp = blockIdx.x; grp < Ng; grp += gridDim.x) {
+    const R* gin = in + (size_t)grp * 5 * nS + ((size_t)o * S + o) * S + o;  // first cell of the 22^3 work box
+    R* gout = out + (size_t)grp * 5 * NI;
+    R* gff = face_flux ? face_flux + (size_t)grp * 9 * 5 * PS * PS : nullptr;
+    if (order == 0) {
+      // x: pencils (j, k) of the padded box -> s1[q][k 22][j 22][i 16];  y: pencils (i, k) -> s2[q][k 22][j 16][i 16];  z: (i, j) -> out
+      rt_sweep<0, R>(gin, nS, S, S * S, 1, s1, N1, PS, RT_W * PS, 1, RT_W, RT_W, RT_G, RT_G, gff, nu, gamma, bad);
+      __syncthreads();
+      rt_sweep<1, R>(s1, N1, 1, RT_W * PS, PS, s2, N2, 1, PS * PS, PS, PS, RT_W, 0, RT_G, gff ? gff + 3 * 5 * PS * PS : nullptr, nu, gamma, bad);
+      __syncthreads();
+      rt_sweep<2, R>(s2, N2, 1, PS, PS * PS, gout, NI, 1, PS, PS * PS, PS, PS, 0, 0, gff ? gff + 6 * 5 * PS * PS : nullptr, nu, gamma, bad);
+    } else {
+      // z: pencils (i, j) of the padded box -> s1[q][k 16][j 22][i 22];  y: pencils (i, k) -> s2[q][k 16][j 16][i 22];  x: (j, k) -> out
+      rt_sweep<2, R>(gin, nS, 1, S, S * S, s1, N1, 1, RT_W, RT_W * RT_W, RT_W, RT_W, RT_G, RT_G, gff ? gff + 6 * 5 * PS * PS : nullptr, nu, gamma, bad);
+      __syncthreads();
+      rt_sweep<1, R>(s1, N1, 1, RT_W * RT_W, RT_W, s2, N2, 1, PS * RT_W, RT_W, RT_W, PS, RT_G, 0, gff ? gff + 3 * 5 * PS * PS : nullptr, nu, gamma, bad);
+      __syncthreads();
+      rt_sweep<0, R>(s2, N2, RT_W, PS * RT_W, 1, gout, NI, PS, PS * PS, 1, PS, PS, 0, 0, gff, nu, gamma, bad);
+    }
+    __syncthreads();  // the next group overwrites s1 / s2
+  }
+  if (status) {
+#pragma unroll
+    for (int ofs = 16; ofs > 0; ofs >>= 1) bad += __shfl_xor_sync(0xffffffffu, bad, ofs);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(reinterpret_cast<unsigned long long*>(status + 1), (unsigned long long)bad);
+  }
+}
+
+constexpr int RT_MAX_SLOTS = 148 * 4;
+inline size_t rtvd_slot_bytes(size_t elem) { return 5 * ((size_t)RT_W * RT_W * PS + (size_t)RT_W * PS * PS) * elem; }
+
+template <class R>
+static int rtvd_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, int order, const hydro_opts* o, cudaStream_t st) {
+  if (Ng < 0) return HYDRO_E_COUNT;
+  if (order < 0 || order > 1) return HYDRO_E_ENUM;
+  const int g = (o && o->nghost) ? o->nghost : RT_G;
+  if (g < RT_G || g > 8) return HYDRO_E_GHOST;
+  const bool device_dt = o && o->max_speed;
+  if (!(gamma > R(1)) || !(dh > R(0)) || (!device_dt && !(dt >= R(0))) || (device_dt && !(o->cfl > 0.0))) return HYDRO_E_VALUE;
+  if (Ng == 0) return HYDRO_OK;
+  if (!in || !out) return HYDRO_E_NULL;
+  if (((uintptr_t)in & 15) || ((uintptr_t)out & 15) || ((uintptr_t)ff & 15)) return HYDRO_E_ALIGN;
+  const size_t slot = rtvd_slot_bytes(sizeof(R));
+  if (!o || !o->workspace || ((uintptr_t)o->workspace & 15) || o->workspace_bytes < slot) return HYDRO_E_WORKSPACE;
+  long long slots = (long long)(o->workspace_bytes / slot);
+  if (slots > RT_MAX_SLOTS) slots = RT_MAX_SLOTS;
+  if (slots > Ng) slots = Ng;
+  rtvd_kernel<R><<<(unsigned)slots, RT_NT, 0, st>>>(in, out, ff, Ng, g, device_dt ? R(0) : dt / dh, gamma, order,
+                                                   device_dt ? static_cast<const R*>(o->max_speed) : nullptr, device_dt ? (R)o->cfl : R(0),
+                                                   static_cast<R*>(o->workspace), o->status);
+  return (int)cudaGetLastError();
+}
+
+}  // namespace hydro
+
+extern "C" {
+size_t hydro_rtvd_workspace_bytes(int Ng, int precision_bytes) {
+  if (Ng <= 0 || (precision_bytes != 4 && precision_bytes != 8)) return 0;
+  const size_t slots = Ng < hydro::RT_MAX_SLOTS ? (size_t)Ng : (size_t)hydro::RT_MAX_SLOTS;
+  return slots * hydro::rtvd_slot_bytes((size_t)precision_bytes);
+}
+int hydro_rtvd_solve_f32(const float* in, float* out, float* face_flux, int Ng, float dt, float dh, float gamma, int order,
+                         const hydro_opts* opts, hydro_stream_t stream) {
+  return hydro::rtvd_impl<float>(in, out, face_flux, Ng, dt, dh, gamma, order, opts, (cudaStream_t)stream);
+}
+int hydro_rtvd_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int order,
+                         const hydro_opts* opts, hydro_stream_t stream) {
+  return hydro::rtvd_impl<double>(in, out, face_flux, Ng, dt, dh, gamma, order, opts, (cudaStream_t)stream);
+}
+}
