@@ -245,6 +245,21 @@ def run_table(args):
                                      "cell_updates_per_s": Ng * CELLS / (ms * 1e-3),
                                      "fused": bool(B.hydro_fused_fits(tdt, scheme, recon, g))})
                         del u, out, ff
+        # the directionally split relaxing-TVD scheme (the low-arithmetic-intensity contrast): HBM-bound
+        peaks = load_json(os.path.join(ROOT, "MEASURED_PEAKS.json"), {}) or {}
+        hbm = float(peaks.get("hbm_gbs") or 6650.0)
+        for tdt in (torch.float32, torch.float64):
+            es = 4 if tdt == torch.float32 else 8
+            u = wl.amr_batch(Ng, g=3, gamma=GAMMA, seed=0, dtype=str(tdt).replace("torch.", ""), device=dev)
+            out = torch.empty((Ng, 5, 16, 16, 16), dtype=tdt, device=dev)
+            ff = torch.empty((Ng, 9, 5, 16, 16), dtype=tdt, device=dev)
+            ws = torch.empty(B.lib().hydro_rtvd_workspace_bytes(Ng, es), dtype=torch.uint8, device=dev)
+            ms = ev(lambda: B.hydro_rtvd_solve(u, 0.05, DH, GAMMA, 0, out=out, face_flux=ff, workspace=ws))
+            byt = es * Ng * (5 * 22 ** 3 + 5 * CELLS + 45 * 256)
+            rows.append({"precision": "fp32" if es == 4 else "fp64", "scheme": "RTVD (split)", "recon": "-", "riemann": "-", "ms": ms,
+                         "cell_updates_per_s": Ng * CELLS / (ms * 1e-3), "fused": True,
+                         "hbm_gbs": byt / ms / 1e6, "hbm_frac": byt / ms / 1e6 / hbm})
+            del u, out, ff, ws
         print(json.dumps({"table": "variants", "groups": Ng, "limiter": "van Leer", "rows": rows}))
         return
     for N, tdt in ((512, torch.float32), (256, torch.float64)):
