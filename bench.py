@@ -235,6 +235,9 @@ def run_table(args):
                     for rs in (3, 2, 1, 0):
                         if scheme != 2 and rs in (1, 0):
                             continue
+                        if args.only and args.only.lower() != ",".join((names[scheme], "PPM" if recon else "PLM", rn[rs],
+                                                                         "fp32" if tdt == torch.float32 else "fp64")).lower():
+                            continue
                         g = B.hydro_min_ghost(scheme, recon)
                         u = wl.amr_batch(Ng, g=g, gamma=GAMMA, seed=0, dtype=str(tdt).replace("torch.", ""), device=dev)
                         out = torch.empty((Ng, 5, 16, 16, 16), dtype=tdt, device=dev)
@@ -250,6 +253,8 @@ def run_table(args):
         hbm = float(peaks.get("hbm_gbs") or 6650.0)
         for tdt in (torch.float32, torch.float64):
             es = 4 if tdt == torch.float32 else 8
+            if args.only and args.only.lower() != "rtvd,-,-," + ("fp32" if es == 4 else "fp64"):
+                continue
             u = wl.amr_batch(Ng, g=3, gamma=GAMMA, seed=0, dtype=str(tdt).replace("torch.", ""), device=dev)
             out = torch.empty((Ng, 5, 16, 16, 16), dtype=tdt, device=dev)
             ff = torch.empty((Ng, 9, 5, 16, 16), dtype=tdt, device=dev)
@@ -402,6 +407,8 @@ def main():
     ap.add_argument("--table", default=None, choices=("variants", "grid", "peaks", "counters"),
                     help="instead of the bench line: one JSON line with per-variant hydro_solve timings (4096 groups), or with the\n"
                          "uniform-grid kernels (gather / scatter bandwidth, whole-step rates); context for DESIGN.md, profiles/")
+    ap.add_argument("--only", default=None, help="--table variants: run ONE row, e.g. CTU,PPM,exact,fp32 or RTVD,-,-,fp32 (the ncu\n"
+                    "captures of the other kernels under profiles/ are taken with it)")
     ap.add_argument("--rep-f32", default=None, help="--table counters: ncu report of the fp32 dominant kernel")
     ap.add_argument("--rep-f64", default=None, help="--table counters: ncu report of the fp64 dominant kernel")
     args = ap.parse_args()

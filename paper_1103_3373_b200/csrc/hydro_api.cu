@@ -52,45 +52,69 @@ template <class R> static LaunchFn<R> lean_fn(int scheme, int recon, int rs) {
 // Non-negative IEEE values order like their bit patterns, and the canonical NaN pattern is larger
 // than +inf, so one integer atomicMax per CTA yields "max, or NaN if any cell was bad".
 constexpr int DT_NT = 256;
-constexpr int DT_ROWS_PER_THREAD = 4;  // independent 16-cell rows in flight per half-warp
 
+template <class R> struct Vec2;
+template <> struct Vec2<float> { using T = float2; };
+template <> struct Vec2<double> { using T = double2; };
+
+// wave speed of one cell, as bits: max-ordered, NaN pattern for a non-positive state (see above)
+template <class R> __device__ __forceinline__ typename Bits<R>::U dt_cell(R rho, R mx, R my, R mz, R E, R gamma, int norm) {
+  const R ir = m_rcp(rho);
+  const R vx = mx * ir, vy = my * ir, vz = mz * ir;
+  const R P = (gamma - R(1)) * (E - R(0.5) * rho * ((vx * vx + vy * vy) + vz * vz));
+  const R c = m_sqrt(gamma * P * ir);
+  const R ax = m_abs(vx), ay = m_abs(vy), az = m_abs(vz);
+  const R s = norm == 0 ? m_max(m_max(ax, ay), az) + c : ((ax + ay) + az) + R(3) * c;
+  const bool bad = !(rho > R(0)) || !(P > R(0)) || !(s == s);
+  return bad ? Bits<R>::nan() : Bits<R>::of(s);
+}
+
+// A warp takes one "span": the 16 interior rows j of one z plane of one group, which are 16 S CONSECUTIVE elements per variable
+// (the ghost columns between them included), and reads them as two-element vectors -- every load instruction of the warp
+// is one contiguous 256 / 512-byte piece.  Ghost columns are masked after the load.  The interior rows of a plane share
+// their 32-byte sectors with the ghost columns, so what HBM must deliver per interior cell is (16 + 2 g) / 16 of the
+// algorithmic 5 sizeof(R) bytes: the ceiling of this kernel by algorithmic bytes is 16 / (16 + 2 g) of the copy peak (73 % at g = 3).
 template <class R>
-__global__ void __launch_bounds__(DT_NT) dt_kernel(const R* __restrict__ u, long long nrows, int g, R gamma, int norm,
+__global__ void __launch_bounds__(DT_NT) dt_kernel(const R* __restrict__ u, long long nspans, int g, R gamma, int norm,
                                                    typename Bits<R>::U* __restrict__ result) {
   using U = typename Bits<R>::U;
+  using V = typename Vec2<R>::T;
   const int S = PS + 2 * g;
   const size_t nS = (size_t)S * S * S;
-  const int lane16 = threadIdx.x & 15;
-  const long long hw = ((long long)blockIdx.x * DT_NT + threadIdx.x) >> 4;  // global half-warp id
-  const long long nhw = ((long long)gridDim.x * DT_NT) >> 4;
+  const int lane = threadIdx.x & 31;
+  const long long warp = ((long long)blockIdx.x * DT_NT + threadIdx.x) >> 5, nwarps = ((long long)gridDim.x * DT_NT) >> 5;
+  const int npieces = PS * S / 2;  // two-element pieces per span
   U best = 0;
-  // a "row" = the 16 interior cells (fixed j,k) of one group: 16 consecutive elements per variable
-  for (long long r0 = hw * DT_ROWS_PER_THREAD; r0 < nrows; r0 += nhw * DT_ROWS_PER_THREAD) {
-    R v[DT_ROWS_PER_THREAD][5];
+  for (long long sp = warp; sp < nspans; sp += nwarps) {
+    const long long grp = sp >> 4;
+    const int k = (int)(sp & 15);
+    const V* b = reinterpret_cast<const V*>(u + (size_t)grp * 5 * nS + ((size_t)(k + g) * S + g) * S);
+    for (int p0 = 0; p0 < npieces; p0 += 32 * 4) {
+      V v[4][5];
 #pragma unroll
-    for (int t = 0; t < DT_ROWS_PER_THREAD; ++t) {
-      const long long r = r0 + t;
-      if (r < nrows) {
-        const long long grp = r >> 8;
-        const int j = (int)(r & 15), k = (int)((r >> 4) & 15);
-        const R* b = u + (size_t)grp * 5 * nS + ((size_t)(k + g) * S + (j + g)) * S + g + lane16;
+      for (int t = 0; t < 4; ++t) {
+        const int pc = p0 + t * 32 + lane;
 #pragma unroll
-        for (int q = 0; q < 5; ++q) v[t][q] = __ldg(b + q * nS);
-      } else {
-        v[t][0] = R(1); v[t][1] = v[t][2] = v[t][3] = R(0); v[t][4] = R(1);
+        for (int q = 0; q < 5; ++q) {
+          if (pc < npieces) v[t][q] = __ldg(b + q * (nS / 2) + pc);
+          else { v[t][q].x = R(1); v[t][q].y = R(1); }
+        }
       }
-    }
 #pragma unroll
-    for (int t = 0; t < DT_ROWS_PER_THREAD; ++t) {
-      const R rho = v[t][0], ir = m_rcp(rho);
-      const R vx = v[t][1] * ir, vy = v[t][2] * ir, vz = v[t][3] * ir;
-      const R P = (gamma - R(1)) * (v[t][4] - R(0.5) * rho * ((vx * vx + vy * vy) + vz * vz));
-      const R c = m_sqrt(gamma * P * ir);
-      const R ax = m_abs(vx), ay = m_abs(vy), az = m_abs(vz);
-      const R s = norm == 0 ? m_max(m_max(ax, ay), az) + c : ((ax + ay) + az) + R(3) * c;
-      const bool bad = !(rho > R(0)) || !(P > R(0)) || !(s == s);
-      const U bits = bad ? Bits<R>::nan() : Bits<R>::of(s);
-      best = bits > best ? bits : best;
+      for (int t = 0; t < 4; ++t) {
+        const int pc = p0 + t * 32 + lane;
+        if (pc < npieces) {
+          const int e = 2 * pc, i0 = e % S;  // column of the first element of the piece within its row (S is even: same row)
+          if (i0 >= g && i0 < g + PS) {
+            const U bits = dt_cell<R>(v[t][0].x, v[t][1].x, v[t][2].x, v[t][3].x, v[t][4].x, gamma, norm);
+            best = bits > best ? bits : best;
+          }
+          if (i0 + 1 >= g && i0 + 1 < g + PS) {
+            const U bits = dt_cell<R>(v[t][0].y, v[t][1].y, v[t][2].y, v[t][3].y, v[t][4].y, gamma, norm);
+            best = bits > best ? bits : best;
+          }
+        }
+      }
     }
   }
 #pragma unroll
@@ -134,11 +158,11 @@ static int dt_impl(const R* u, int Ng, int nghost, R gamma, int norm, R* max_spe
     if (e != cudaSuccess) return (int)e;
   }
   if (Ng == 0) return HYDRO_OK;
-  const long long nrows = (long long)Ng * PS * PS;
-  long long blocks = (nrows * 16 / DT_ROWS_PER_THREAD + DT_NT - 1) / DT_NT;
+  const long long nspans = (long long)Ng * PS;  // one per (group, interior z plane)
+  long long blocks = (nspans * 32 + DT_NT - 1) / DT_NT;
   const long long cap = (long long)sm_count() * 8;
   if (blocks > cap) blocks = cap;
-  dt_kernel<R><<<(unsigned)blocks, DT_NT, 0, st>>>(u, nrows, nghost, gamma, norm,
+  dt_kernel<R><<<(unsigned)blocks, DT_NT, 0, st>>>(u, nspans, nghost, gamma, norm,
                                                   reinterpret_cast<typename Bits<R>::U*>(max_speed));
   return (int)cudaGetLastError();
 }
