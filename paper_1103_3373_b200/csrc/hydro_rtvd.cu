@@ -48,6 +48,9 @@ template <class R> __device__ __forceinline__ R rt_phi(R a, R b) {
 // One sweep along D of the pencils (a, b), a in [0, na), b in [0, nb).  src cell (q, a, b, x) at src[q sq + a sa + b sb + x sx],
 // x = 0 .. 21; dst likewise for the 16 updated cells x - 3.  ff: plane base of direction D (3 planes x 5 x 256) or nullptr;
 // (a - fa0, b - fb0) are the in-plane interior coordinates of the pencil (lower axis fastest).
+// The march is unrolled by six -- the period of its register windows (three cells of right movers, three of left movers, two
+// predictor / corrector fluxes) -- so that the windows rotate by renaming, not by moves (the rolled loop spent 29 % of its
+// instructions on MOV), and the next cell's five loads are issued before the current cell's arithmetic.
 template <int D, class R>
 __device__ __forceinline__ void rt_sweep(const R* __restrict__ src, size_t sq, int sa, int sb, int sx, R* __restrict__ dst, size_t dq,
                                          int da, int db, int dx, int na, int nb, int fa0, int fb0, R* __restrict__ ff, R nu, R gamma,
@@ -58,50 +61,69 @@ __device__ __forceinline__ void rt_sweep(const R* __restrict__ src, size_t sq, i
     R* d = dst + (size_t)a * da + (size_t)b * db;
     const int ta = a - fa0, tb = b - fb0;
     R* fp = (ff && ta >= 0 && ta < PS && tb >= 0 && tb < PS) ? ff + tb * PS + ta : nullptr;
-    V5<R> Uprev, frp, Glo, fr1a, fr1b, fl1b, Hlo;  // U[x-1], m[x-1].fr, G at the lower face of x-1, corrector windows
-    Mv<R> m1p;      // movers of u1[x-2]
+    V5<R> Uw[2], frw[2], Gw[2], Hw[2];  // U, right movers of U, predictor flux, corrector flux: current and previous
+    V5<R> r1[3], l1[3];                 // right / left movers of the predicted state u1, cells x-1, x-2, x-3 (slot = cell % 3)
+    V5<R> Unext;
 #pragma unroll
-    for (int q = 0; q < 5; ++q) { Uprev[q] = frp[q] = Glo[q] = fr1a[q] = fr1b[q] = fl1b[q] = Hlo[q] = R(0); m1p.fr[q] = m1p.fl[q] = R(0); }
+    for (int q = 0; q < 5; ++q) {
+      Uw[0][q] = Uw[1][q] = frw[0][q] = frw[1][q] = Gw[0][q] = Gw[1][q] = Hw[0][q] = Hw[1][q] = R(0);
+      r1[0][q] = r1[1][q] = r1[2][q] = l1[0][q] = l1[1][q] = l1[2][q] = R(0);
+      Unext[q] = s[q * sq];
+    }
 #pragma unroll 1
-    for (int x = 0; x < RT_W; ++x) {
-      V5<R> U;
+    for (int x0 = 0; x0 < RT_W; x0 += 6) {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) U[q] = s[q * sq + (size_t)x * sx];
-      const Mv<R> m = rt_movers<D>(U, gamma, bad);
-      if (x >= 1) {
-        V5<R> G;  // predictor flux at the face between x-1 and x
+      for (int u = 0; u < 6; ++u) {
+        const int x = x0 + u;
+        if (x < RT_W) {
+          V5<R>& U = Uw[u & 1];
+          const V5<R>& Uprev = Uw[(u + 1) & 1];
+          U = Unext;
+          if (x + 1 < RT_W) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) G[q] = frp[q] - m.fl[q];
-        if (x >= 2) {  // u1 of cell x-1, its movers, the corrector flux at the lower face of cell x-2, the update of cell x-3
-          V5<R> u1;
-#pragma unroll
-          for (int q = 0; q < 5; ++q) u1[q] = Uprev[q] - R(0.5) * nu * (G[q] - Glo[q]);
-          const Mv<R> m1 = rt_movers<D>(u1, gamma, bad);  // cell x-1
-          if (x >= 5) {  // face f = x-2: right movers of cells f-2, f-1, f (fr1a, fr1b, m1p.fr), left movers of f-1, f, f+1 (fl1b, m1p.fl, m1.fl)
-            V5<R> H;
-#pragma unroll
-            for (int q = 0; q < 5; ++q) {
-              const R frh = fr1b[q] + rt_phi(R(0.5) * (fr1b[q] - fr1a[q]), R(0.5) * (m1p.fr[q] - fr1b[q]));
-              const R flh = m1p.fl[q] - rt_phi(R(0.5) * (m1p.fl[q] - fl1b[q]), R(0.5) * (m1.fl[q] - m1p.fl[q]));
-              H[q] = frh - flh;
-            }
-            const int f = x - 2 - RT_G;  // face index of the group: 0 .. 16
-            if (fp && (f & 7) == 0) {
-#pragma unroll
-              for (int q = 0; q < 5; ++q) fp[((f >> 3) * 5 + q) * (PS * PS)] = H[q];
-            }
-            if (x >= 6) {  // cell x-3 = interior cell f-1
-#pragma unroll
-              for (int q = 0; q < 5; ++q)  // U[x-3] is re-read (an L1 hit) rather than carried through the window
-                d[q * dq + (size_t)(x - 3 - RT_G) * dx] = s[q * sq + (size_t)(x - 3) * sx] - nu * (H[q] - Hlo[q]);
-            }
-            Hlo = H;
+            for (int q = 0; q < 5; ++q) Unext[q] = s[q * sq + (size_t)(x + 1) * sx];
           }
-          fr1a = fr1b; fr1b = m1p.fr; fl1b = m1p.fl; m1p = m1;
+          const Mv<R> m = rt_movers<D>(U, gamma, bad);
+          if (x >= 1) {
+            V5<R>& G = Gw[u & 1];  // predictor flux at the face between x-1 and x
+            const V5<R>& Glo = Gw[(u + 1) & 1];
+#pragma unroll
+            for (int q = 0; q < 5; ++q) G[q] = frw[(u + 1) & 1][q] - m.fl[q];
+            if (x >= 2) {  // u1 of cell x-1, its movers, the corrector flux at the lower face of cell x-2, the update of cell x-3
+              V5<R> u1;
+#pragma unroll
+              for (int q = 0; q < 5; ++q) u1[q] = Uprev[q] - R(0.5) * nu * (G[q] - Glo[q]);
+              const Mv<R> m1 = rt_movers<D>(u1, gamma, bad);  // cell x-1 -> slot (u + 5) % 3
+              constexpr int dummy = 0; (void)dummy;
+              const int c1 = (u + 5) % 3, c2 = (u + 4) % 3, c3 = (u + 3) % 3;  // slots of cells x-1, x-2, x-3 (compile time: u is)
+              V5<R> fr4 = r1[c1];  // right movers of cell x-4 still sit in the slot cell x-1 takes
+              r1[c1] = m1.fr;
+              l1[c1] = m1.fl;
+              if (x >= 5) {  // face f = x-2: right movers of cells x-4, x-3, x-2; left movers of cells x-3, x-2, x-1
+                V5<R>& H = Hw[u & 1];
+                const V5<R>& Hlo = Hw[(u + 1) & 1];
+#pragma unroll
+                for (int q = 0; q < 5; ++q) {
+                  const R frh = r1[c3][q] + rt_phi(R(0.5) * (r1[c3][q] - fr4[q]), R(0.5) * (r1[c2][q] - r1[c3][q]));
+                  const R flh = l1[c2][q] - rt_phi(R(0.5) * (l1[c2][q] - l1[c3][q]), R(0.5) * (l1[c1][q] - l1[c2][q]));
+                  H[q] = frh - flh;
+                }
+                const int f = x - 2 - RT_G;  // face index of the group: 0 .. 16
+                if (fp && (f & 7) == 0) {
+#pragma unroll
+                  for (int q = 0; q < 5; ++q) fp[((f >> 3) * 5 + q) * (PS * PS)] = H[q];
+                }
+                if (x >= 6) {  // cell x-3 = interior cell f-1; U[x-3] is re-read (an L1 hit) rather than carried through the window
+#pragma unroll
+                  for (int q = 0; q < 5; ++q)
+                    d[q * dq + (size_t)(x - 3 - RT_G) * dx] = s[q * sq + (size_t)(x - 3) * sx] - nu * (H[q] - Hlo[q]);
+                }
+              }
+            }
+          }
+          frw[u & 1] = m.fr;
         }
-        Glo = G;
       }
-      Uprev = U; frp = m.fr;
     }
   }
 }
@@ -146,7 +168,7 @@ rtvd_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_
   }
 }
 
-constexpr int RT_MAX_SLOTS = 148 * 4;
+constexpr int RT_MAX_SLOTS = 148 * 2;  // 296 slots x 267 KB (fp32) stay in the 126 MB L2; 592 spilled 1.2 GB of scratch writes to HBM
 inline size_t rtvd_slot_bytes(size_t elem) { return 5 * ((size_t)RT_W * RT_W * PS + (size_t)RT_W * PS * PS) * elem; }
 
 template <class R>
