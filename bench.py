@@ -381,6 +381,22 @@ def run_peaks(args, B, dev):
         burst = max(ops * w / sum(ts[k:k + w]) for k in range(0, n - w + 1))
         out["kinds"][kind] = {"ops_per_launch": ops, "launches": n, "sustained_tops": ops * n / sum(ts) / 1e12,
                               "burst_tops": burst / 1e12, "clocks": sampler.summary()}
+    # issue probes: the same arithmetic issued as scalar FFMA pairs or as packed FFMA2, inside the instruction mix of the kernels
+    out["issue_probe"] = {"_what": "TFLOP/s of the FP32 part of each mix (higher = the mix issues faster); scalar vs packed side by side"}
+    for sc, pk in (("2ffma_shf", "ffma2_shf"), ("6ffma_sel_shf", "3ffma2_sel_shf"), ("8ffma_sel_mufu_shf", "4ffma2_sel_mufu_shf")):
+        row = {}
+        for kind in (sc, pk):
+            ops = B.hydro_alu_peak_launch(kind, blocks, threads, iters, scratch)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                B.hydro_alu_peak_launch(kind, blocks, threads, iters, scratch)
+            e1.record()
+            torch.cuda.synchronize()
+            row[kind] = ops * 5 / (e0.elapsed_time(e1) * 1e-3) / 1e12
+        row["packed_over_scalar"] = row[pk] / row[sc]
+        out["issue_probe"][sc + " vs " + pk] = row
     k = out["kinds"]
     out["fp32_tflops"] = max(k["ffma"]["sustained_tops"], k["ffma2"]["sustained_tops"], k["ffma_const"]["sustained_tops"])
     out["fp32_tflops_ffma"] = k["ffma"]["sustained_tops"]

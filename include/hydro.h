@@ -239,6 +239,8 @@ HYDRO_API const char* hydro_strerror(int code);
  * 8 x 16 independent operations of one kind, on `stream`; the caller times it with CUDA events.
  *   kind 0 FFMA (register operands)   1 FFMA2 (fma.rn.f32x2)   2 DFMA   3 FMUL / FADD alternating
  *        4 FFMA : FMNMX 1:1           5 FFMA2 : FMNMX 1:1      6 MUFU.RSQ   7 FFMA with constant-bank operands
+ *        8 / 9: (2 FFMA | 1 FFMA2) + SHF   10 / 11: (6 FFMA | 3 FFMA2) + FSETP + FSEL + SHF   12 / 13: (8 FFMA | 4 FFMA2) +
+ *        FSETP + FSEL + MUFU + SHF -- equal arithmetic in scalar and packed form (does FFMA2 relieve the issue port?)
  * scratch: device buffer of >= blocks*threads*8 bytes (never written in practice); *ops_per_launch (host, may be NULL)
  * receives the floating-point operations of the timed kind per launch (FMA = 2; for kinds 4, 5 those of the FMAs only;
  * kind 6: MUFU operations).  Errors: HYDRO_E_ENUM, HYDRO_E_VALUE (threads not a multiple of 32 in [32,512]), HYDRO_E_NULL. */

@@ -238,7 +238,8 @@ def hydro_dt(u, gamma, norm=0, *, max_speed=None, stream=None):
     return max_speed
 
 
-PEAK_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "fmul_fadd": 3, "ffma_fmnmx": 4, "ffma2_fmnmx": 5, "mufu": 6, "ffma_const": 7}
+PEAK_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "fmul_fadd": 3, "ffma_fmnmx": 4, "ffma2_fmnmx": 5, "mufu": 6, "ffma_const": 7,
+              "2ffma_shf": 8, "ffma2_shf": 9, "6ffma_sel_shf": 10, "3ffma2_sel_shf": 11, "8ffma_sel_mufu_shf": 12, "4ffma2_sel_mufu_shf": 13}
 
 
 def hydro_alu_peak_launch(kind, blocks, threads, iters, scratch, *, stream=None):

@@ -112,12 +112,61 @@ __global__ void __launch_bounds__(512) peak_mufu(float* out, float a, int iters)
   if (s == 123.456f) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// kinds 8-13: does the packed FFMA2 relieve the ISSUE port?  Equal arithmetic as 2 x FFMA or 1 x FFMA2 per unit, mixed with the
+// other instruction classes of the hydro kernels (NA x (FSETP + FSEL), NM x MUFU.RSQ, NI x SHF, all on independent chains).
+// Measured on B200 (profiles/alu_peaks.json "issue_probe"): the packed form is never faster -- FFMA2 holds the issue port like
+// two FFMAs -- which is why the fused kernels do not use it.
+__device__ __forceinline__ float fma1(float a, float b, float c) { float r; asm volatile("fma.rn.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c)); return r; }
+template <int PACKED, int NF, int NA, int NM, int NI>
+__global__ void __launch_bounds__(512) issue_probe(float* out, float a0, float b0, int iters) {
+  constexpr int CH = 8;
+  const float t = 1e-9f * threadIdx.x;
+  const float a = a0 + t, b = b0 - t;
+  int sh = threadIdx.x & 7;
+  const uint64_t A = pk2(a, a + 1e-3f), B = pk2(b, b - 1e-3f);
+  float acc[CH * 2], alt[CH], mu[CH];
+  uint64_t acc2[CH];
+  int ia[CH];
+#pragma unroll
+  for (int c = 0; c < CH; ++c) {
+    acc[2 * c] = a * (threadIdx.x + c); acc[2 * c + 1] = b * c; acc2[c] = pk2(acc[2 * c], acc[2 * c + 1]);
+    alt[c] = b + c; ia[c] = threadIdx.x + c; mu[c] = 1.5f + c;
+  }
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+#pragma unroll
+      for (int c = 0; c < CH; ++c) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          if (PACKED) acc2[c] = fma2(acc2[c], A, B);
+          else { acc[2 * c] = fma1(acc[2 * c], a, b); acc[2 * c + 1] = fma1(acc[2 * c + 1], a, b); }
+        }
+#pragma unroll
+        for (int f = 0; f < NA; ++f) {
+          const float o = alt[(c + 1 + f) % CH];
+          asm volatile("{.reg .pred p; setp.gt.f32 p, %0, %1; selp.f32 %0, %1, %2, p;}" : "+f"(alt[c]) : "f"(o), "f"(b));
+        }
+#pragma unroll
+        for (int f = 0; f < NM; ++f) { float r; asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(mu[c])); mu[c] = r; }
+#pragma unroll
+        for (int f = 0; f < NI; ++f) asm volatile("shf.l.wrap.b32 %0, %0, %0, %1;" : "+r"(ia[c]) : "r"(sh));
+      }
+    }
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int c = 0; c < CH; ++c) { float x, y; upk2(acc2[c], x, y); s += x + y + acc[2 * c] + acc[2 * c + 1] + alt[c] + mu[c] + (float)ia[c]; }
+  if (s == 123.456f) out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace hydro
 
 extern "C" int hydro_alu_peak_launch(int kind, int blocks, int threads, int iters, void* scratch, double* ops_per_launch,
                                      hydro_stream_t stream) {
   using namespace hydro;
-  if (kind < 0 || kind > 7) return HYDRO_E_ENUM;
+  if (kind < 0 || kind > 13) return HYDRO_E_ENUM;
   if (blocks < 1 || threads < 32 || threads > 512 || (threads & 31) || iters < 1) return HYDRO_E_VALUE;
   if (!scratch) return HYDRO_E_NULL;
   cudaStream_t st = (cudaStream_t)stream;
@@ -131,7 +180,18 @@ extern "C" int hydro_alu_peak_launch(int kind, int blocks, int threads, int iter
     case 4: peak_f32<4><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); break;          // flops of the FFMAs only
     case 5: peak_f32x2<5><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); per = 4.0; break;
     case 7: peak_f32<7><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); break;
+    // issue probes: ops_per_launch = the FP32 flops of the unit (4 per FFMA pair / FFMA2); 8 chains x 4 unrolls per iteration
+    case 8: issue_probe<0, 1, 0, 0, 1><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); per = 1.0; break;   // 2 FFMA + SHF
+    case 9: issue_probe<1, 1, 0, 0, 1><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); per = 1.0; break;   // FFMA2 + SHF
+    case 10: issue_probe<0, 3, 1, 0, 1><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); per = 3.0; break;  // 6 FFMA + FSETP/FSEL + SHF
+    case 11: issue_probe<1, 3, 1, 0, 1><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); per = 3.0; break;  // 3 FFMA2 + ...
+    case 12: issue_probe<0, 4, 1, 1, 1><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); per = 4.0; break;  // 8 FFMA + FSETP/FSEL + MUFU + SHF
+    case 13: issue_probe<1, 4, 1, 1, 1><<<blocks, threads, 0, st>>>((float*)scratch, 1.0000001f, 1e-9f, iters); per = 4.0; break;  // 4 FFMA2 + ...
     default: peak_mufu<<<blocks, threads, 0, st>>>((float*)scratch, 1.5f, iters); per = 1.0; break;
+  }
+  if (kind >= 8) {  // issue probes: 8 chains x 4 unrolls per pass instead of 16 x 8; `per` = FFMA pairs per unit, 4 flops each
+    if (ops_per_launch) *ops_per_launch = (double)blocks * threads * iters * 4 * 8 * per * 4.0;
+    return (int)cudaGetLastError();
   }
   if (ops_per_launch) *ops_per_launch = inst * per;
   return (int)cudaGetLastError();
