@@ -41,6 +41,12 @@ namespace hydro {
 #ifndef LEAN_ROLE_SPLIT
 #define LEAN_ROLE_SPLIT 0
 #endif
+#ifndef LEAN_OPAQUE
+#define LEAN_OPAQUE 1
+#endif
+#ifndef LEAN_GC_F64
+#define LEAN_GC_F64 0  // measured: the fp64 kernel (ten warps per SM, latency-bound) is 3 % slower with it despite 2 % fewer instructions
+#endif
 #ifndef LEAN_ONE_WAITER
 #define LEAN_ONE_WAITER 1  // 1: one lane polls the plane's mbarrier before barrier 1; 0: every thread polls it in phase D
 #endif
@@ -106,8 +112,8 @@ template <class R> struct LeanCtx {
 };
 
 // The whole march of one role over this CTA's groups.  All roles execute the same sequence of CTA barriers.
-template <class R, int RECON, int RS, int FAST, int GRID, int ROLE>
-__device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>& p, int ii, int jj) {
+template <class R, int RECON, int RS, int FAST, int GRID, int ROLE, int GC>
+__device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>& p, int ii, int jj, const int tid) {
   using Op = LeanOps<R, RECON, RS, FAST>;
   constexpr int GW = 2 + RECON, RW = 1 + RECON, SWP = PS + 2 * GW, WPL = SWP * SWP, NW = 2 * RW + 1, NPL = PS + 2 * GW;
   // PPM tiles are trimmed so that two fp32 CTAs (or one fp64 CTA) fit: one raw landing plane instead of two, and the
@@ -120,11 +126,22 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
   using FC = Fld<R, NC>;   // an exchange field LOX .. FY (one entry per column)
   // the column lies inside the interior range along x / y; with ROLE_ANY these are run-time flags of one code stream
   // (three specialised streams cost more in instruction-cache misses than they save: profiles/r2_ctu_diet.md)
+#if LEAN_OPAQUE
+  // the role is a property of the WARP (warps 0-7 interior, 8 the x ring, 9 the y ring): taken from a warp broadcast, the
+  // flags are uniform values and every role test is a uniform branch (no BSSY / BSYNC, no per-lane predicate re-derived
+  // from tid at each use)
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const bool in_i = ROLE == ROLE_ANY ? (warp != PS * PS / 32) : ROLE != ROLE_XR;
+  const bool in_j = ROLE == ROLE_ANY ? (warp != PS * PS / 32 + 1) : ROLE != ROLE_YR;
+#else
   const bool in_i = ROLE == ROLE_ANY ? (ii >= 1 && ii <= PS) : ROLE != ROLE_XR;
   const bool in_j = ROLE == ROLE_ANY ? (jj >= 1 && jj <= PS) : ROLE != ROLE_YR;
+#endif
   const bool INT = in_i && in_j, XR = !in_i, YR = !in_j;
 
-  const int g = cx.g;
+  // ghost width: a compile-time constant in the specialised instantiations (GC >= 0; grid mode: always GW), so that plane and
+  // variable strides fold into immediate offsets
+  const int g = GRID ? GW : (GC >= 0 ? GC : cx.g);
   const int S = PS + 2 * g;
   const int SS = S * S;
   const size_t nS = (size_t)SS * S;
@@ -137,7 +154,6 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
     return gio.bc == 0 ? (c < 0 ? c + N : (c >= N ? c - N : c)) : (c < 0 ? 0 : (c >= N ? N - 1 : c));
   };
 
-  const int tid = threadIdx.x;
   const int col = jj * FT + ii;
   const int wb = (jj + GW - 1) * SWP + (ii + GW - 1);  // own index in a primitive plane
   // ---- per-thread shared addresses (vector part; the scalar part of the same cell sits at + d?s)
@@ -182,6 +198,9 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
   const int my_groups = (cx.Ng - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int total_planes = my_groups * NPL;
   auto issue = [&](int n) {  // the feeder lane only
+#if LEAN_OPAQUE
+    asm volatile("" : "+r"(n));  // keeps the descriptor arithmetic below inside the feeder's branch (hoisted, every warp would run it)
+#endif
     if (n >= total_planes) return;
     const int m = n / NPL, pl = n - m * NPL;
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
@@ -238,18 +257,37 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
     if (GRID) { cp_async_wait<NRAW - 1>(); __syncthreads(); }
     else mbar_wait(cx.bar + (nseq % NRAW), (uint32_t)((nseq / NRAW) & 1));
   };
-  // con->prim of the next raw plane into the ring slot whose own-cell address is wslot (all threads; cells tid, tid + NT)
-  auto convert = [&](uint32_t wslot) {
-    const R* rp = cx.raw + (size_t)(nseq % NRAW) * 5 * SS;
-    const uint32_t base = wslot - 16u * (uint32_t)wb;  // start of the slot
+  // con->prim of the next raw plane into the ring slot whose own-cell address is wslot (all threads; cells tid and, for the
+  // first CR2 threads from CR0 on, tid + CSH: CSH is a whole number of plane rows, so that both cells of a thread share the
+  // column and the raw offset of the second is the first's plus a uniform constant)
+  constexpr int CSH = (NT / SWP) * SWP, CR0 = NT - CSH, CR2 = WPL - CSH;  // PLM: 320, 0, 80; PPM: 308, 12, 176
+  uint32_t roff0;                                             // byte offset of cell tid in a raw plane (per variable: + q SS)
+  {
+    const int b = tid / SWP, a = tid - b * SWP;
+    roff0 = (uint32_t)((b + off) * S + (a + off)) * ES;
+#if LEAN_OPAQUE
+    asm volatile("" : "+r"(roff0));
+#endif
+  }
+  // Destination: cell tid of a ring slot sits at (z16, z16 + dzs) -- the thread's own z-state entry -- plus the compile-time
+  // distance between the two arrays plus the slot's CTA-uniform offset: no per-thread address is formed for it.
+  constexpr uint32_t RZV = (uint32_t)(NWS * 5 * WPL) * ES;               // sm_zs - sm_ring
+  auto convert = [&](uint32_t slot_off) {
+    const uint32_t rp = cx.sm_raw + (uint32_t)(nseq % NRAW) * (uint32_t)(5 * SS) * ES + roff0;
+    const uint32_t dv = z16 + slot_off - RZV, ds = dv + dzs + (FW::SD - FZ::SD);
+    const uint32_t sS = (uint32_t)SS * ES;
+    {
+      V5<R> U;
 #pragma unroll
-    for (int r = 0; r < (WPL + NT - 1) / NT; ++r) {
-      const int idx = tid + r * NT;
-      if ((r + 1) * NT <= WPL || idx < WPL) {
-        const int b = idx / SWP, a = idx - b * SWP;
-        const V5<R> W = Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c, trk);
-        FW::st(base + 16u * (uint32_t)idx, base + FW::SD + ES * (uint32_t)idx, W);
-      }
+      for (int q = 0; q < 5; ++q) U[q] = *sm_ptr<const R>(rp + (uint32_t)q * sS);
+      FW::st(dv, ds, Op::c2p(U, p, c, trk));
+    }
+    if (tid >= CR0 && tid < CR2) {
+      const uint32_t rp1 = rp + (uint32_t)((CSH / SWP) * S) * ES;
+      V5<R> U;
+#pragma unroll
+      for (int q = 0; q < 5; ++q) U[q] = *sm_ptr<const R>(rp1 + (uint32_t)q * sS);
+      FW::st(dv + 16u * CSH, ds + ES * CSH, Op::c2p(U, p, c, trk));
     }
   };
   // after the barrier that follows a conversion: refill the raw stage it consumed
@@ -308,7 +346,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
     V5<R> Wold;  // RC: W(t+1-RW) at the thread's own column
     if (RC) {
       landed_all();
-      convert(wv(0));
+      convert(wo[0]);
       __syncthreads();
       refill();
       Wold = FW::ld(wv(0), wv(0) + dws);
@@ -317,7 +355,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
 #pragma unroll
     for (int k = 0; k < NWS; ++k) {
       landed_all();
-      convert(wv(k));
+      convert(wo[k]);
       __syncthreads();
       refill();
     }
@@ -387,7 +425,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
                  Op::template riemann_scaled<1>(FC::ld(fyv + LF_UPY * CF - 16u * FT, fys + LF_UPY * CF - ES * FT), FC::ld(fyv + LF_LOY * CF, fys + LF_LOY * CF), p, c, p.hnu));
       }
       if (!LEAN_ONE_WAITER && !GRID && conv) mbar_wait(cx.bar + (nseq % NRAW), (uint32_t)((nseq / NRAW) & 1));
-      if (conv) convert(wv(0));  // the oldest shared-memory plane: last read in B / C of this step
+      if (conv) convert(wo[0]);  // the oldest shared-memory plane: last read in B / C of this step
       __syncthreads();  // barrier 2
       if (conv) refill();
 
@@ -501,7 +539,7 @@ __device__ __forceinline__ void ctu_lean_role(const LeanCtx<R>& cx, const Par<R>
 #undef znxt
 }
 
-template <class R, int RECON, int RS, int FAST, int MINB, int GRID>
+template <class R, int RECON, int RS, int FAST, int MINB, int GRID, int GC>
 __global__ void __launch_bounds__(LEAN_NT, MINB)
 ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, Par<R> p,
                 const R* __restrict__ max_speed, R cfl, long long* status, GridIO<R> gio) {
@@ -519,13 +557,30 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   R* zs = ring + NWS * 5 * WPL;                        // [2][2] fields of NT cells: private traced z states (lo, up) of planes t, t+1
   R* xy = zs + 4 * 5 * NT;                             // [6] fields of NC cells: LOX UPX LOY UPY FX FY
   cx.raw = xy + 6 * 5 * NC;                            // [2][5][SS] landing zone of the bulk copies (SoA as in HBM)
+#if LEAN_OPAQUE
+  // the shared-window address of the tile is formed ONCE and made opaque: ptxas otherwise re-derives it (S2UR SR_CgaCtaId,
+  // UMOV, ULEA) at every use inside the loop instead of holding one register
+  uint32_t sb = smem_u32(smem);
+  asm volatile("" : "+r"(sb));
+  cx.sm_bar = sb;
+  cx.sm_ring = sb + 64u;
+  cx.sm_zs = cx.sm_ring + (uint32_t)(sizeof(R) * NWS * 5 * WPL);
+  cx.sm_xy = cx.sm_zs + (uint32_t)(sizeof(R) * 4 * 5 * NT);
+  cx.sm_raw = cx.sm_xy + (uint32_t)(sizeof(R) * 6 * 5 * NC);
+#else
   cx.sm_bar = smem_u32(smem);
   cx.sm_ring = smem_u32(ring);
   cx.sm_zs = smem_u32(zs);
   cx.sm_xy = smem_u32(xy);
   cx.sm_raw = smem_u32(cx.raw);
+#endif
 
+#if LEAN_OPAQUE
+  int tid = threadIdx.x;
+  asm volatile("" : "+r"(tid));  // one register instead of an S2R at every re-derivation
+#else
   const int tid = threadIdx.x;
+#endif
   if (tid == 0) {
     mbar_init(cx.bar, 1);
     mbar_init(cx.bar + 1, 1);
@@ -541,17 +596,21 @@ ctu_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   else if (tid < PS * PS + 32) { const int l = tid - PS * PS; jj = 1 + (l >> 1); ii = (l & 1) ? FT - 1 : 0; }
   else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
   if (LEAN_ROLE_SPLIT) {
-    if (tid < PS * PS) ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_INT>(cx, p, ii, jj);
-    else if (tid < PS * PS + 32) ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_XR>(cx, p, ii, jj);
-    else ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_YR>(cx, p, ii, jj);
+    if (tid < PS * PS) ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_INT, GC>(cx, p, ii, jj, tid);
+    else if (tid < PS * PS + 32) ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_XR, GC>(cx, p, ii, jj, tid);
+    else ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_YR, GC>(cx, p, ii, jj, tid);
   } else {
-    ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_ANY>(cx, p, ii, jj);
+    ctu_lean_role<R, RECON, RS, FAST, GRID, ROLE_ANY, GC>(cx, p, ii, jj, tid);
   }
 }
 
 // persistent grid: SMs x resident CTAs per SM (occupancy API), capped at Ng
-template <class R, int RECON, int RS, int FAST, int MINB, int GRID = 0> cudaError_t launch_ctu_lean(const SolveArgs<R>& a) {
-  auto kern = ctu_lean_kernel<R, RECON, RS, FAST, MINB, GRID>;
+template <class R, int RECON, int RS, int FAST, int MINB, int GRID = 0, int GC = -1> cudaError_t launch_ctu_lean(const SolveArgs<R>& a) {
+  // the default options at the ghost width of the AMR batches (g = 3, BASELINE.json configs[2] and [4]) have their own instantiation
+  if constexpr (FAST && !GRID && GC < 0 && (sizeof(R) == 4 || LEAN_GC_F64)) {
+    if (a.g == 3) return launch_ctu_lean<R, RECON, RS, FAST, MINB, GRID, 3>(a);
+  }
+  auto kern = ctu_lean_kernel<R, RECON, RS, FAST, MINB, GRID, GC>;
   const size_t smem = lean_smem_bytes(sizeof(R), RECON, a.g);
   if (smem > SMEM_MAX_OPTIN) return cudaErrorInvalidConfiguration;
   static int sms = 0;
