@@ -148,9 +148,11 @@ HYDRO_API int hydro_scatter_f64(const double* out, double* grid, int nx, int ny,
 /* One update of a UNIFORM grid in one launch (no gather / scatter pass, no group buffers): the fused kernel fetches the
  * planes of every patch group from grid_in [5][nz][ny][nx] directly, ghost zones of width hydro_min_ghost() folded at the
  * domain boundary (bc 0 periodic, 1 outflow), and writes the updated cells to grid_out (same shape; must not be grid_in).
- * opts as in hydro_solve_* (nghost, workspace and impl ignored; face fluxes are not produced).  Available for the
- * default options of the CTU scheme (van Leer limiter on primitive variables, no floors); otherwise returns
- * HYDRO_E_NOFUSED and the caller uses hydro_gather_* -> hydro_solve_* -> hydro_scatter_*. */
+ * opts as in hydro_solve_* (nghost, workspace and impl ignored; face fluxes are not produced).  Available for every scheme
+ * (MHM, VL, CTU), reconstruction, Riemann solver and limiter option; the one exception is VL with positivity floors
+ * (min_dens / min_pres > 0), which returns HYDRO_E_NOFUSED: the caller then uses hydro_gather_* -> hydro_solve_* ->
+ * hydro_scatter_*.  Results equal that three-call path bit for bit with the default options (van Leer limiter on
+ * primitive variables, no floors) and to a few ulp otherwise. */
 HYDRO_API int hydro_solve_grid_f32(const float* grid_in, float* grid_out, int nx, int ny, int nz, int bc, float dt, float dh,
                          float gamma, int scheme, int riemann, int limiter, const hydro_opts* opts, hydro_stream_t stream);
 HYDRO_API int hydro_solve_grid_f64(const double* grid_in, double* grid_out, int nx, int ny, int nz, int bc, double dt, double dh,

@@ -333,7 +333,7 @@ def hydro_solve_grid(grid, dt, dh, gamma, scheme=CTU, riemann=ROE, limiter=VANLE
                      stream=None, **optkw):
     """hydro_solve_grid_f32/f64: one update of a uniform CUDA grid [5,Nz,Ny,Nx] in one launch (no gather / scatter).
     Returns the updated grid (`out`, allocated if None; must not be `grid`).  Raises HydroError(HYDRO_E_NOFUSED)
-    for variants without the grid mode (anything but CTU with the default options)."""
+    for the one variant without a grid mode (VL with positivity floors)."""
     if not grid.is_cuda or not grid.is_contiguous() or grid.dim() != 4 or grid.shape[0] != 5:
         raise ValueError("hydro_solve_grid: grid must be a contiguous CUDA tensor [5,Nz,Ny,Nx]")
     sfx, ft = _suffix(grid)

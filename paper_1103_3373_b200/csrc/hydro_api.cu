@@ -255,7 +255,16 @@ static int solve_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, i
   return (int)lean_fn<R>(scheme, pl.recon, riemann)(a);
 }
 
-// One update of a uniform grid in ONE launch: the fused CTU kernel fetches its planes from grid_in (ghost zones folded
+// variants hydro_solve_grid_* covers (one launch per step, ghost zones folded out of the grid by the fused kernels): every
+// scheme, reconstruction, solver and limiter option; the one exception is VL with positivity floors, whose half step re-reads
+// U^n of ghost cells from the batch (hydro_lean_vl.cuh S2) -- that combination takes the group path
+static bool grid_mode_ok(int scheme, int limiter, const hydro_opts* o) {
+  (void)limiter;
+  const bool floors = o && (o->min_dens > 0.0 || o->min_pres > 0.0);
+  return !(scheme == SCHEME_VL && floors);
+}
+
+// One update of a uniform grid in ONE launch: the fused kernel fetches its planes from grid_in (ghost zones folded
 // at the domain boundary) and writes the updated cells into grid_out; no gather / scatter pass, no group buffers.
 template <class R>
 static int solve_grid_impl(const R* gin, R* gout, int nx, int ny, int nz, int bc, R dt, R dh, R gamma, int scheme, int riemann,
@@ -273,8 +282,7 @@ static int solve_grid_impl(const R* gin, R* gout, int nx, int ny, int nz, int bc
   oo.impl = HYDRO_IMPL_FUSED;
   const int rc = make_plan<R>(gin, gout, nullptr, (int)Ng, dt, dh, gamma, scheme, riemann, limiter, &oo, true, a.par, pl);
   if (rc != HYDRO_OK) return rc;
-  const bool fast = limiter == LIM_VANLEER && !oo.char_limit && !(oo.min_dens > 0.0) && !(oo.min_pres > 0.0);
-  if (scheme != SCHEME_CTU || !fast) return HYDRO_E_NOFUSED;  // callers fall back to gather -> hydro_solve -> scatter
+  if (!grid_mode_ok(scheme, limiter, &oo)) return HYDRO_E_NOFUSED;  // callers fall back to gather -> hydro_solve -> scatter
   if (Ng == 0) return HYDRO_OK;
   a.in = nullptr;
   a.out = nullptr;
@@ -295,11 +303,6 @@ static int solve_grid_impl(const R* gin, R* gout, int nx, int ny, int nz, int bc
   return (int)lean_fn<R>(scheme, pl.recon, riemann)(a);
 }
 
-// variants hydro_solve_grid_* covers (one launch per step, ghost zones folded out of the grid by the fused kernel)
-static bool grid_mode_ok(int scheme, int limiter, const hydro_opts* o) {
-  const bool fast = limiter == LIM_VANLEER && !(o && o->char_limit) && !(o && o->min_dens > 0.0) && !(o && o->min_pres > 0.0);
-  return scheme == SCHEME_CTU && fast;
-}
 
 // ---- hydro_advance: the multi-step driver of a uniform grid, entirely on the device ----------------
 // elapsed time: t += cfl dh / max_speed in fp64, by one thread on the stream (the solver kernels take dt/dh = cfl / max_speed

@@ -15,6 +15,7 @@
 #include <cstdint>
 #include "hydro_launch.cuh"
 #include "hydro_lean_ctu.cuh"
+#include "hydro_lean_grid.cuh"
 
 namespace hydro {
 
@@ -64,20 +65,23 @@ template <class R, int RECON, int RS, int FAST> struct MhmOps {
   }
 };
 
-template <class R, int RECON, int RS, int FAST, int MINB>
+template <class R, int RECON, int RS, int FAST, int MINB, int GRID>
 __global__ void __launch_bounds__(LEAN_NT, MINB)
-mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, Par<R> p,
-                const R* __restrict__ max_speed, R cfl, long long* status) {
+mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g_arg, Par<R> p,
+                const R* __restrict__ max_speed, R cfl, long long* status, GridIO<R> gio) {
   using Op = LeanOps<R, RECON, RS, FAST>;
   using Mo = MhmOps<R, RECON, RS, FAST>;
   constexpr int GW = 2 + RECON, RW = 1 + RECON, SWP = PS + 2 * GW, WPL = SWP * SWP, NW = 2 * RW + 1, NPL = PS + 2 * GW;
   constexpr int NC = LEAN_COLS, NT = LEAN_NT, FT = PS + 2;
   apply_device_dt(p, max_speed, cfl);
 
+  const int g = GRID ? GW : g_arg;  // grid mode: the ghost zones come from the grid, always at the minimum width
   const int S = PS + 2 * g;
   const int SS = S * S;
   const size_t nS = (size_t)SS * S;
   const int off = g - GW;  // unused outer ghost layers
+  // grid mode: plane / variable strides of the grids
+  const size_t N2 = (size_t)(gio.Gy * PS) * (gio.Gx * PS), N3 = N2 * (gio.Gz * PS);
 
   extern __shared__ __align__(16) unsigned char smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
@@ -116,14 +120,19 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     fence_async_smem();
   }
   __syncthreads();
-  if (tid == 0) { issue(0); issue(1); }
+  GridFeed<R, SWP, NPL, NT> gf;
+  gf.reset();
+  if (GRID) { gf.feed(gio, my_groups, raw, tid); gf.feed(gio, my_groups, raw + 5 * WPL, tid); }
+  else if (tid == 0) { issue(0); issue(1); }
 
   Cnt c = {0, 0, 0};
   typename Bits<R>::U best = 0;  // running maximum of the updated cells' wave speed (next_max_speed)
   int nseq = 0;
+  // grid mode: a thread waits for its own copies of raw plane nseq; the CTA barrier that follows publishes the plane
+  auto landed = [&]() { if (GRID) cp_async_wait<1>(); };
   auto convert = [&](int slot) {
     const int st = nseq & 1;
-    mbar_wait(bar + st, (uint32_t)((nseq >> 1) & 1));
+    if (!GRID) mbar_wait(bar + st, (uint32_t)((nseq >> 1) & 1));
     const R* rp = raw + (size_t)st * 5 * SS;
     R* wp = ring + slot * 5 * WPL;
     for (int idx = tid; idx < WPL; idx += NT) {
@@ -132,7 +141,8 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     }
   };
   auto refill = [&]() {
-    if (tid == 0) { fence_async_smem(); issue(nseq + 2); }
+    if (GRID) gf.feed(gio, my_groups, raw + (size_t)(nseq & 1) * 5 * SS, tid);
+    else if (tid == 0) { fence_async_smem(); issue(nseq + 2); }
     ++nseq;
   };
 
@@ -142,10 +152,18 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
 
   for (int m = 0; m < my_groups; ++m) {
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
+    // own cell of plane 0 in `in` / `out`, or (grid mode, interior columns) in the grids: plane stride SS / 256 or N2, variable stride nS / 4096 or N3
     const R* gin0 = in + grp * 5 * nS + ((size_t)g * S + (jj - 1 + g)) * S + (ii - 1 + g);
     R* gout0 = out + grp * 5 * PS * PS * PS + (jj - 1) * PS + (ii - 1);
+    if (GRID) {
+      const size_t cell = interior ? grid_cell0(gio, grp, ii - 1, jj - 1) : 0;
+      gin0 = gio.gin + cell;
+      gout0 = gio.gout + cell;
+    }
+    const size_t pstr_in = GRID ? N2 : (size_t)SS, vstr_in = GRID ? N3 : nS;
     R* gff = face_flux ? face_flux + grp * 9 * 5 * PS * PS : nullptr;
     for (int k = 0; k < NW; ++k) {  // prologue: planes -1-RW .. -1+RW
+      if (GRID) { landed(); __syncthreads(); }
       convert(k);
       __syncthreads();
       refill();
@@ -163,9 +181,9 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
         V5<R> Uold;
         const bool upd = interior && t >= 1;
         if (upd) {
-          const R* gin = gin0 + (t - 1) * SS;
+          const R* gin = gin0 + (size_t)(t - 1) * pstr_in;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += nS; }
+          for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += vstr_in; }
         }
         const R* wpl = ring + slot[RW] * 5 * WPL;
         const V5<R> W0 = ldv(wpl, WPL, wb);
@@ -216,13 +234,21 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
               const V5<R> Wn = Op::c2p(U, p, c);
               if (p.next_speed) track_speed(Wn, p, best);
               if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
-              st5(gout0 + (t - 1) * PS * PS, PS * PS * PS, U);
+              if (GRID) {
+                R* d = gout0 + (size_t)(t - 1) * N2;
+#pragma unroll
+                for (int q = 0; q < 5; ++q) { *d = U[q]; d += N3; }
+              } else {
+                st5(gout0 + (t - 1) * PS * PS, PS * PS * PS, U);
+              }
             }
             Dz = Fz;
           }
           if (t < PS) uzc = Op::correct(upz, inc, p, c);
         }
       }
+      const bool conv = t + RW + 1 <= PS - 1 + GW;  // plane t+RW+1 replaces plane t-RW (read for the last time in P1)
+      if (conv) landed();
       __syncthreads();  // barrier A
 
       // ================= P2: F_x(t), F_y(t), boundary-flux stores; con->prim of the next plane =================
@@ -238,7 +264,6 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
           if (gff && ((jj - 1) & 7) == 0) st5(gff + (size_t)((3 + ((jj - 1) >> 3)) * 5) * 256 + t * PS + (ii - 1), 256, f);
         }
       }
-      const bool conv = t + RW + 1 <= PS - 1 + GW;  // plane t+RW+1 replaces plane t-RW (read for the last time in P1)
       if (conv) convert(sl);
       __syncthreads();  // barrier B
       if (conv) refill();
@@ -257,8 +282,8 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   flush_speed(best, p.next_speed);
 }
 
-template <class R, int RECON, int RS, int FAST, int MINB> cudaError_t launch_mhm_lean(const SolveArgs<R>& a) {
-  auto kern = mhm_lean_kernel<R, RECON, RS, FAST, MINB>;
+template <class R, int RECON, int RS, int FAST, int MINB, int GRID = 0> cudaError_t launch_mhm_lean(const SolveArgs<R>& a) {
+  auto kern = mhm_lean_kernel<R, RECON, RS, FAST, MINB, GRID>;
   const size_t smem = mhm_smem_bytes(sizeof(R), RECON, a.g);
   if (smem > SMEM_MAX_OPTIN) return cudaErrorInvalidConfiguration;
   static int sms = 0;
@@ -276,7 +301,7 @@ template <class R, int RECON, int RS, int FAST, int MINB> cudaError_t launch_mhm
   if (per_sm < 1) return cudaErrorInvalidConfiguration;
   long long grid = (long long)sms * per_sm;
   if (grid > a.Ng) grid = a.Ng;
-  kern<<<(unsigned)grid, LEAN_NT, smem, a.stream>>>(a.in, a.out, a.face_flux, a.Ng, a.g, a.par, a.max_speed, a.cfl, a.status);
+  kern<<<(unsigned)grid, LEAN_NT, smem, a.stream>>>(a.in, a.out, a.face_flux, a.Ng, a.g, a.par, a.max_speed, a.cfl, a.status, a.grid);
   return cudaGetLastError();
 }
 

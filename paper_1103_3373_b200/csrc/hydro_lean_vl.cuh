@@ -17,13 +17,14 @@
 #include <cstdint>
 #include "hydro_launch.cuh"
 #include "hydro_lean_mhm.cuh"
+#include "hydro_lean_grid.cuh"
 
 namespace hydro {
 
-template <class R, int RECON, int RS, int FAST>
+template <class R, int RECON, int RS, int FAST, int GRID>
 __global__ void __launch_bounds__(VL_NT(RECON), 1)
-vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, Par<R> p,
-               const R* __restrict__ max_speed, R cfl, long long* status) {
+vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g_arg, Par<R> p,
+               const R* __restrict__ max_speed, R cfl, long long* status, GridIO<R> gio) {
   using Op = LeanOps<R, RECON, RS, FAST>;
   using Mo = MhmOps<R, RECON, RS, FAST>;
   constexpr int RW = 1 + RECON, E = RW + 1, GW = E + 1, NW = 2 * RW + 1, NPL = PS + 2 * GW;
@@ -36,10 +37,12 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
   static_assert(2 * FPL <= 4 * NC, "first-pass flux fields must fit in LOX..UPY");
   apply_device_dt(p, max_speed, cfl);
 
+  const int g = GRID ? GW : g_arg;  // grid mode: the ghost zones come from the grid, always at the minimum width
   const int S = PS + 2 * g;
   const int SS = S * S;
   const size_t nS = (size_t)SS * S;
   const int off = g - GW;
+  const size_t N2 = (size_t)(gio.Gy * PS) * (gio.Gx * PS), N3 = N2 * (gio.Gz * PS);  // grid mode: plane / variable strides
 
   extern __shared__ __align__(16) unsigned char smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
@@ -92,13 +95,18 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     fence_async_smem();
   }
   __syncthreads();
-  if (tid == 0) issue(0);
+  GridFeed<R, SW, NPL, NT> gf;
+  gf.reset();
+  if (GRID) gf.feed(gio, my_groups, raw, tid);
+  else if (tid == 0) issue(0);
 
   Cnt c = {0, 0, 0};
   typename Bits<R>::U best = 0;  // running maximum of the updated cells' wave speed (next_max_speed)
   int nseq = 0;
+  // grid mode: a thread waits for its own copies of the raw plane; the CTA barrier that follows publishes the plane
+  auto landed = [&]() { if (GRID) cp_async_wait<0>(); };
   auto convert = [&]() {
-    mbar_wait(bar, (uint32_t)(nseq & 1));
+    if (!GRID) mbar_wait(bar, (uint32_t)(nseq & 1));
     const R* rp = raw;
     R* wp = wpl;
     for (int idx = tid; idx < WPL; idx += NT) {
@@ -107,7 +115,8 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     }
   };
   auto refill = [&]() {
-    if (tid == 0) { fence_async_smem(); issue(nseq + 1); }
+    if (GRID) gf.feed(gio, my_groups, raw, tid);
+    else if (tid == 0) { fence_async_smem(); issue(nseq + 1); }
     ++nseq;
   };
 
@@ -119,12 +128,20 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
     const R* gin0 = in + grp * 5 * nS + ((size_t)g * S + (cj + g)) * S + (ci + g);
     R* gout0 = out + grp * 5 * PS * PS * PS + cj * PS + ci;
+    if (GRID) {  // U^n and the result live in the grids (interior columns only)
+      const size_t cell0 = c_int ? grid_cell0(gio, grp, ci, cj) : 0;
+      gin0 = gio.gin + cell0;
+      gout0 = gio.gout + cell0;
+    }
+    const size_t pstr_in = GRID ? N2 : (size_t)SS, vstr_in = GRID ? N3 : nS;
     R* gff = face_flux ? face_flux + grp * 9 * 5 * PS * PS : nullptr;
     // ---- prologue: plane -GW (only its own-column values are needed, as W(a-1) of the first step), then plane -E
+    if (GRID) { landed(); __syncthreads(); }
     convert();
     __syncthreads();
     refill();
     if (c_int) Wprev = ldv(wpl, WPL, wb);
+    if (GRID) landed();
     __syncthreads();
     convert();
     __syncthreads();
@@ -179,9 +196,10 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
           // is U^n to rounding -- unless a floor changed them: then the raw conserved state is re-read (L2-resident)
           V5<R> U;
           if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) {
-            const R* gp = gin0 + (ptrdiff_t)ap * SS;
+            // (the arm cells of a floored grid-mode run would need folded addresses: hydro_solve_grid_* does not take floors with VL)
+            const R* gp = gin0 + (ptrdiff_t)ap * (ptrdiff_t)pstr_in;
 #pragma unroll
-            for (int q = 0; q < 5; ++q) { U[q] = __ldg(gp); gp += nS; }
+            for (int q = 0; q < 5; ++q) { U[q] = __ldg(gp); gp += vstr_in; }
           } else {
             U = prim2cons(Wprev, p);
           }
@@ -202,9 +220,9 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
         V5<R> Uold;
         const bool upd = interior && b >= 1;
         if (upd) {
-          const R* gin = gin0 + (b - 1) * SS;
+          const R* gin = gin0 + (size_t)(b - 1) * pstr_in;
 #pragma unroll
-          for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += nS; }
+          for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += vstr_in; }
         }
         const R* hp = hring + ((b + E) % NW) * 5 * HPL;
         const V5<R> H0 = ldv(hp, HPL, hb);
@@ -242,13 +260,21 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
               const V5<R> Wn = Op::c2p(U, p, c);
               if (p.next_speed) track_speed(Wn, p, best);
               if (!FAST && (p.min_dens > R(0) || p.min_pres > R(0))) U = prim2cons(Wn, p);
-              st5(gout0 + (b - 1) * PS * PS, PS * PS * PS, U);
+              if (GRID) {
+                R* d = gout0 + (size_t)(b - 1) * N2;
+#pragma unroll
+                for (int q = 0; q < 5; ++q) { *d = U[q]; d += N3; }
+              } else {
+                st5(gout0 + (b - 1) * PS * PS, PS * PS * PS, U);
+              }
             }
             Dz = Fz;
           }
           if (b < PS) uzc = uz;
         }
       }
+      const bool conv = a + 1 <= PS - 1 + GW;
+      if (conv) landed();
       __syncthreads();  // barrier 3
 
       // ================= S4: F_x(b), F_y(b), boundary-flux stores; con->prim of plane a+1 =================
@@ -264,7 +290,6 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
           if (gff && ((jj - 1) & 7) == 0) st5(gff + (size_t)((3 + ((jj - 1) >> 3)) * 5) * 256 + b * PS + (ii - 1), 256, f);
         }
       }
-      const bool conv = a + 1 <= PS - 1 + GW;
       if (conv) convert();  // plane a+1 replaces plane a, read for the last time in S1
       __syncthreads();  // barrier 4
       if (conv) refill();
@@ -282,8 +307,8 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
   flush_speed(best, p.next_speed);
 }
 
-template <class R, int RECON, int RS, int FAST> cudaError_t launch_vl_lean(const SolveArgs<R>& a) {
-  auto kern = vl_lean_kernel<R, RECON, RS, FAST>;
+template <class R, int RECON, int RS, int FAST, int GRID = 0> cudaError_t launch_vl_lean(const SolveArgs<R>& a) {
+  auto kern = vl_lean_kernel<R, RECON, RS, FAST, GRID>;
   const size_t smem = vl_smem_bytes(sizeof(R), RECON, a.g);
   if (smem > SMEM_MAX_OPTIN) return cudaErrorInvalidConfiguration;
   static int sms = 0;
@@ -296,7 +321,7 @@ template <class R, int RECON, int RS, int FAST> cudaError_t launch_vl_lean(const
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const int grid = a.Ng < sms ? a.Ng : sms;
-  kern<<<(unsigned)grid, VL_NT(RECON), smem, a.stream>>>(a.in, a.out, a.face_flux, a.Ng, a.g, a.par, a.max_speed, a.cfl, a.status);
+  kern<<<(unsigned)grid, VL_NT(RECON), smem, a.stream>>>(a.in, a.out, a.face_flux, a.Ng, a.g, a.par, a.max_speed, a.cfl, a.status, a.grid);
   return cudaGetLastError();
 }
 

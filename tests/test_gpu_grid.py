@@ -120,6 +120,8 @@ def test_config4_kh_full_size_properties(B, scheme):
     for recon in (0, 1):
         for riemann in (ROE, HLLC):
             status = torch.zeros(3, dtype=torch.int64, device="cuda")
+            # all 12 variants run in grid mode (one launch per step): the workspace is the second grid, no group buffers
+            assert B.hydro_advance_workspace_bytes((N, N, N), torch.float32, scheme, VANLEER, recon=recon) == 256 + 5 * N ** 3 * 4
             U, t = B.hydro_advance(U0.clone(), steps, 1.0 / N, gamma, scheme, riemann, VANLEER, cfl=0.3, recon=recon,
                                    status=status)
             assert status.cpu().tolist()[1] == 0 and torch.isfinite(U).all().item()
@@ -188,14 +190,51 @@ def test_solve_grid_equals_gather_solve_scatter(B, dtype, bc, recon, riemann):
     assert st_a.tolist() == st_b.tolist() and na.item() == nb.item()
 
 
+# round 2: every scheme and the non-default options (limiters, characteristic limiting, floors) in grid mode against
+# gather -> hydro_solve -> scatter (the group path is what the parity tests compare with the oracle): bitwise for the default
+# options, a few ulp for the others
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+@pytest.mark.parametrize("scheme,recon,riemann,limiter,kw", (
+    (0, 0, ROE, VANLEER, {}), (0, 1, HLLC, VANLEER, {}), (0, 0, ROE, 0, {}), (0, 1, ROE, 3, dict(char_limit=1)),
+    (0, 0, HLLC, VANLEER, dict(min_dens=1e-3, min_pres=1e-3)),
+    (1, 0, ROE, VANLEER, {}), (1, 1, HLLC, VANLEER, {}), (1, 0, ROE, 2, {}), (1, 1, ROE, 0, dict(char_limit=1)),
+    (2, 0, ROE, 0, {}), (2, 1, HLLC, 2, dict(char_limit=1)), (2, 0, ROE, VANLEER, dict(min_dens=1e-3, min_pres=1e-3)),
+    (2, 0, 1, 3, {})))
+def test_solve_grid_all_schemes_and_options(B, dtype, scheme, recon, riemann, limiter, kw):
+    import torch
+    gamma = 1.4
+    for bc in (0, 1):
+        U0 = torch.from_numpy(wl.kh_grid((32, 48, 64), gamma=gamma, seed=5, dtype=dtype)).cuda()
+        g = B.hydro_min_ghost(scheme, recon)
+        groups = B.hydro_gather(U0, g, bc)
+        smax = B.hydro_dt(groups, gamma, 1)
+        dt = 0.8 * (1.0 / 64) / float(smax.item())
+        st_a = torch.zeros(3, dtype=torch.int64, device="cuda")
+        st_b = torch.zeros(3, dtype=torch.int64, device="cuda")
+        na = torch.zeros((), dtype=U0.dtype, device="cuda")
+        nb = torch.zeros((), dtype=U0.dtype, device="cuda")
+        out, _ = B.hydro_solve(groups, dt, 1.0 / 64, gamma, scheme, riemann, limiter, recon=recon, face_flux=False, status=st_a,
+                               next_max_speed=na, impl=B.IMPL_FUSED, **kw)
+        ref = B.hydro_scatter(out, tuple(U0.shape[1:]))
+        got = B.hydro_solve_grid(U0, dt, 1.0 / 64, gamma, scheme, riemann, limiter, bc=bc, recon=recon, status=st_b, next_max_speed=nb, **kw)
+        if limiter == VANLEER and not kw:
+            # default options: the kernels' own arithmetic (hydro_lean_math.cuh, explicit FMAs) is the same instruction sequence
+            assert torch.equal(got, ref)
+            assert na.item() == nb.item()
+        else:
+            # the other options run the generic arithmetic of hydro_math.cuh, written as plain a * b + c: the two template
+            # instantiations may contract different multiply-add pairs into FMAs, so they agree to a few ulp, not bitwise
+            eps = float(np.finfo(dtype).eps)
+            assert (got.double() - ref.double()).abs().max().item() <= 8 * eps * ref.abs().max().item()
+            assert abs(na.item() - nb.item()) <= 8 * eps * abs(na.item())
+        assert st_a.tolist() == st_b.tolist()
+
+
 def test_solve_grid_unsupported_variants(B):
     import torch
     U = torch.ones((5, 16, 16, 16), device="cuda")
-    for kw in (dict(scheme=0), dict(scheme=1), dict(limiter=0), dict(char_limit=1), dict(min_dens=1e-3)):
-        a = dict(scheme=CTU, limiter=VANLEER)
-        a.update(kw)
-        sch, lim = a.pop("scheme"), a.pop("limiter")
-        with pytest.raises(B.HydroError):
-            B.hydro_solve_grid(U, 0.01, 1.0, 1.4, sch, ROE, lim, **a)
+    # the one variant without a grid mode: VL with positivity floors (its half step re-reads U^n of ghost cells from the batch)
+    with pytest.raises(B.HydroError):
+        B.hydro_solve_grid(U, 0.01, 1.0, 1.4, 1, ROE, VANLEER, min_dens=1e-3)
     with pytest.raises(B.HydroError):
         B.hydro_solve_grid(U, 0.01, 1.0, 1.4, CTU, ROE, VANLEER, out=U)
