@@ -15,51 +15,90 @@
 namespace hydro {
 
 constexpr int GRID_NT = 256;
+constexpr int GATHER_BRICK = 4;  // 8 measured the same; plain x-y-z order reads the z ghost zones from HBM twice
 
-// one CTA per (group, variable), GATHER_PL z planes of the padded group per pass: warp w fetches the rows j = w, w+8, ...
-// of all those planes (lane = x, so a lane's source column is computed once; all loads of a pass are in flight
-// together), the planes are staged in shared memory and leave as 16-byte pieces: GATHER_PL destination planes are
-// GATHER_PL * S*S contiguous elements starting on a 16-byte boundary.
+// One CTA per patch group.  A thread owns up to MAXE PAIRS of in-plane positions (j, i), (j, i + 1) of the padded group (S is
+// even, so a pair never straddles a row) -- consecutive threads own consecutive destination pairs, so every store instruction
+// of a warp is one contiguous 256- (512-) byte piece -- and forms their folded source offsets ONCE: they are the same for
+// all S z planes and all five variables, so that the loop over the 5 S planes is nothing but loads and paired stores off a
+// uniform plane base (GATHER_UN planes, 4 GATHER_UN loads per thread, in flight together).  The two sources of a pair are loaded separately (they are not
+// adjacent where the ghost zone wraps around the domain).  Round 1's kernel (rows staged through shared memory) spent 27
+// warp instructions per 22-element row on index arithmetic and predicates and was bound by instruction ISSUE (72 % of the
+// issue slots busy at 3.1 TB/s); this one needs about 3.  CTAs walk the groups in bricks of 4 x 4 x 4, so that the ghost
+// zones a group shares with its neighbours along z are still in L2 when the neighbour reads them (in plain x-y-z order they
+// are one whole z layer of groups -- hundreds of MB of traffic -- apart and came from HBM twice).
+template <class R> struct Pair;
+template <> struct Pair<float> { using type = float2; };
+template <> struct Pair<double> { using type = double2; };
 template <class R>
 __global__ void __launch_bounds__(GRID_NT) gather_kernel(const R* __restrict__ grid, R* __restrict__ groups, int Gx, int Gy, int Gz,
                                                           int g, int bc) {
-  constexpr int VEC = 16 / sizeof(R), NWARP = GRID_NT / 32, MAXR = (32 + NWARP - 1) / NWARP;  // rows per warp and plane
-  constexpr int GATHER_PL = 4;  // planes per pass (8 measured slower: ragged last pass, fewer resident CTAs)
-  __shared__ __align__(16) R tile[GATHER_PL * 32 * 32];
+  using P2 = typename Pair<R>::type;
+  constexpr int MAXE = (32 * 32 / 2 + GRID_NT - 1) / GRID_NT;  // S <= 32
+  constexpr int GATHER_UN = 2, BR = GATHER_BRICK;
   const int S = PS + 2 * g, SS = S * S, Nx = Gx * PS, Ny = Gy * PS, Nz = Gz * PS;
-  const int v = blockIdx.x % 5, n = blockIdx.x / 5;
-  const int gx = n % Gx, gy = (n / Gx) % Gy, gz = n / (Gx * Gy);
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // brick order: full bricks first (x fastest inside a brick), then the ragged remainder in plain order
+  int gx, gy, gz;
+  {
+    const int bx = Gx / BR, by = Gy / BR, bz = Gz / BR, nfull = bx * by * bz * BR * BR * BR;
+    int n = blockIdx.x;
+    if (n < nfull) {
+      const int in = n % (BR * BR * BR), b = n / (BR * BR * BR);
+      gx = (b % bx) * BR + in % BR; gy = ((b / bx) % by) * BR + (in / BR) % BR; gz = (b / (bx * by)) * BR + in / (BR * BR);
+    } else {  // groups outside the full bricks, enumerated in x-y-z order
+      n -= nfull;
+      const int fx = bx * BR, fy = by * BR, fz = bz * BR;
+      gx = gy = gz = 0;
+      for (int z = 0, c = 0; z < Gz; ++z)
+        for (int y = 0; y < Gy; ++y) {
+          const int skip = (z < fz && y < fy) ? fx : 0, cnt = Gx - skip;
+          if (n < c + cnt) { gx = skip + (n - c); gy = y; gz = z; z = Gz; break; }
+          c += cnt;
+        }
+    }
+  }
+  const int n = (gz * Gy + gy) * Gx + gx;
   auto fold = [bc](int c, int N) {  // periodic wrap or zero-gradient clamp (ghost width <= 8 < 16 <= N)
     return bc == 0 ? (c < 0 ? c + N : (c >= N ? c - N : c)) : (c < 0 ? 0 : (c >= N ? N - 1 : c));
   };
-  const R* src = grid + (size_t)v * Nz * Ny * Nx + fold(gx * PS - g + lane, Nx);
-  size_t yo[MAXR];  // source row offsets of this warp's rows
+  int s0[MAXE], s1[MAXE];  // source offsets within a z plane of the grid of the pair's two elements; s0 = -1: no pair
 #pragma unroll
-  for (int r = 0; r < MAXR; ++r) yo[r] = (size_t)fold(gy * PS - g + min(warp + r * NWARP, S - 1), Ny) * Nx;
-  uint4* dst = reinterpret_cast<uint4*>(groups + ((size_t)n * 5 + v) * S * SS);
-  for (int k0 = 0; k0 < S; k0 += GATHER_PL) {
-    const int np = min(GATHER_PL, S - k0);
-    R val[GATHER_PL][MAXR];
+  for (int r = 0; r < MAXE; ++r) {
+    const int idx = 2 * ((int)threadIdx.x + r * GRID_NT);
+    const int j = idx / S, i = idx - j * S;
+    const int row = fold(gy * PS - g + j, Ny) * Nx;
+    s0[r] = idx < SS ? row + fold(gx * PS - g + i, Nx) : -1;
+    s1[r] = row + fold(gx * PS - g + i + 1, Nx);
+  }
+  // byte offsets of the S source planes within a variable (folded along z), formed once per CTA
+  __shared__ long long zoff[32];
+  const size_t N2 = (size_t)Ny * Nx;
+  if (threadIdx.x < S) zoff[threadIdx.x] = (long long)((size_t)fold(gz * PS - g + (int)threadIdx.x, Nz) * N2 * sizeof(R));
+  __syncthreads();
+  P2* dst = reinterpret_cast<P2*>(groups + (size_t)n * 5 * S * SS) + threadIdx.x;
+  const char* vp = reinterpret_cast<const char*>(grid);
+  const size_t vstride = (size_t)Nz * N2 * sizeof(R);
+  const int half = SS / 2;
+  for (int v = 0; v < 5; ++v) {
+    for (int k0 = 0; k0 < S; k0 += GATHER_UN) {  // S is even: GATHER_UN = 2 leaves no remainder
+      P2 val[GATHER_UN][MAXE];
 #pragma unroll
-    for (int q = 0; q < GATHER_PL; ++q) {
-      const R* sp = src + (size_t)fold(gz * PS - g + min(k0 + q, S - 1), Nz) * Ny * Nx;
+      for (int u = 0; u < GATHER_UN; ++u) {
+        const R* sp = reinterpret_cast<const R*>(vp + zoff[k0 + u]);
+        asm volatile("" : "+l"(sp));  // a finished plane base: every load address is then ONE wide multiply-add off it
 #pragma unroll
-      for (int r = 0; r < MAXR; ++r) val[q][r] = (lane < S) ? __ldg(sp + yo[r]) : R(0);
+        for (int r = 0; r < MAXE; ++r)
+          if (s0[r] >= 0) { val[u][r].x = __ldg(sp + s0[r]); val[u][r].y = __ldg(sp + s1[r]); }
+      }
+#pragma unroll
+      for (int u = 0; u < GATHER_UN; ++u) {
+#pragma unroll
+        for (int r = 0; r < MAXE; ++r)
+          if (s0[r] >= 0) dst[u * half + r * GRID_NT] = val[u][r];
+      }
+      dst += GATHER_UN * half;
     }
-    __syncthreads();  // the previous pass has left the tile
-    if (lane < S) {
-#pragma unroll
-      for (int q = 0; q < GATHER_PL; ++q)
-#pragma unroll
-        for (int r = 0; r < MAXR; ++r) {
-          const int j = warp + r * NWARP;
-          if (j < S && q < np) tile[q * SS + j * S + lane] = val[q][r];
-        }
-    }
-    __syncthreads();
-    const uint4* t4 = reinterpret_cast<const uint4*>(tile);
-    for (int q = threadIdx.x; q < np * SS / VEC; q += GRID_NT) dst[(size_t)k0 * (SS / VEC) + q] = t4[q];
+    vp += vstride;
   }
 }
 
@@ -92,8 +131,8 @@ static int gather_impl(const R* grid, R* groups, int nx, int ny, int nz, int ngh
   if (Ng == 0) return HYDRO_OK;
   if (!grid || !groups) return HYDRO_E_NULL;
   if (((uintptr_t)grid & 15) || ((uintptr_t)groups & 15)) return HYDRO_E_ALIGN;
-  const long long blocks = Ng * 5;
-  if (blocks > 0x7fffffffLL) return HYDRO_E_COUNT;
+  const long long blocks = Ng;
+  if (blocks * 5 > 0x7fffffffLL || (long long)nx * ny > 0x7fffffffLL) return HYDRO_E_COUNT;
   gather_kernel<R><<<(unsigned)blocks, GRID_NT, 0, st>>>(grid, groups, nx / PS, ny / PS, nz / PS, nghost, bc);
   return (int)cudaGetLastError();
 }
