@@ -134,3 +134,45 @@ def test_config2_full_size_against_the_oracle(B, oracle):
     assert st_r[1] == 0 and st_g[1] == 0
     assert err_l1(Ug[None], Ur[None]) <= steps * TOL32
     assert abs(tg - tr) <= 1e-4 * tr
+
+
+# ---- SURVEY 8(f)-2 beyond device memory (section 3.1: "the maximum simulation scale will not be limited by the
+# relatively small memory in GPUs"): a HOST data set larger than the device memory that is free while it runs goes through
+# hydro_pipeline_solve.  A ballast allocation takes all but ~3 GB of the device first, so that the 7.9 GB of host input + output
+# (32768 groups, g = 2, fp32, no face fluxes) could not be resident; the pipeline needs only its few chunk buffers.  The host
+# batch is a 256-group seeded batch tiled 128 times, so every tile must reproduce the device path's bits of that batch.
+def test_pipeline_data_set_larger_than_free_device_memory(B):
+    import torch
+    gamma, g, nb, reps = 5.0 / 3.0, 2, 256, 128
+    S = PS + 2 * g
+    base = wl.amr_batch(nb, g=g, gamma=gamma, seed=21, dtype="float32")
+    dev_out, _ = B.hydro_solve(base.cuda(), 0.05, 1.0, gamma, CTU, ROE, VANLEER, face_flux=False)
+    ref = dev_out.cpu()
+    del dev_out
+    Ng = nb * reps
+    hin = torch.empty((Ng, 5, S, S, S), dtype=torch.float32).pin_memory()
+    hout = torch.zeros((Ng, 5, PS, PS, PS), dtype=torch.float32).pin_memory()
+    hin.view(reps, nb, 5, S, S, S)[:] = base
+    host_bytes = hin.numel() * 4 + hout.numel() * 4
+    pipe = B.HydroPipeline(torch.float32, g, groups_per_chunk=512, nstreams=4)
+    # warm the pipeline's own buffers with a small call, then fill the device
+    pipe.solve(hin[:1024], hout[:1024], None, 0.05, 1.0, gamma, CTU, ROE, VANLEER)
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free, _total = torch.cuda.mem_get_info()
+    keep = 3 << 30
+    ballast = torch.empty(max(free - keep, 0), dtype=torch.uint8, device="cuda") if free > keep else None
+    free_now, _ = torch.cuda.mem_get_info()
+    assert host_bytes > free_now, (host_bytes, free_now)   # the data set cannot be resident
+    hout.zero_()
+    st = torch.zeros(3, dtype=torch.int64)
+    pipe.solve(hin, hout, None, 0.05, 1.0, gamma, CTU, ROE, VANLEER, status=st)
+    pipe.close()
+    del ballast
+    torch.cuda.empty_cache()
+    assert st.tolist()[1] == 0
+    got = hout.view(reps, nb, 5, PS, PS, PS)
+    for r in (0, 1, 63, 64, 127):
+        assert torch.equal(got[r], ref), r
+    # every tile equals the first (cheap reduction over the whole output)
+    assert torch.equal(got.sum(dim=0, dtype=torch.float64), got[0].double() * reps)
