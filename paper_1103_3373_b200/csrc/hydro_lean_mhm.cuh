@@ -65,7 +65,7 @@ template <class R, int RECON, int RS, int FAST> struct MhmOps {
   }
 };
 
-template <class R, int RECON, int RS, int FAST, int MINB, int GRID>
+template <class R, int RECON, int RS, int FAST, int MINB, int GRID, int GC>
 __global__ void __launch_bounds__(LEAN_NT, MINB)
 mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g_arg, Par<R> p,
                 const R* __restrict__ max_speed, R cfl, long long* status, GridIO<R> gio) {
@@ -75,7 +75,9 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   constexpr int NC = LEAN_COLS, NT = LEAN_NT, FT = PS + 2;
   apply_device_dt(p, max_speed, cfl);
 
-  const int g = GRID ? GW : g_arg;  // grid mode: the ghost zones come from the grid, always at the minimum width
+  // ghost width: grid mode takes the ghost zones from the grid at the minimum width; GC >= 0: compiled in (strides fold into
+  // immediate offsets)
+  const int g = GRID ? GW : (GC >= 0 ? GC : g_arg);
   const int S = PS + 2 * g;
   const int SS = S * S;
   const size_t nS = (size_t)SS * S;
@@ -88,21 +90,40 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   R* ring = reinterpret_cast<R*>(smem + 64);           // [NW] fields of WPL cells: primitive planes t-RW .. t+RW
   R* xy = ring + NW * 5 * WPL;                         // [6] fields of NC cells: LOX UPX LOY UPY FX FY
   R* raw = xy + 6 * 5 * NC;                            // [2][5][SS] landing zone of the bulk copies
-  auto fld = [&](int k) { return xy + k * 5 * NC; };
+  // every shared-memory access below is LDS / STS [R + immediate] off 32-bit shared addresses formed once (hydro_ptx.cuh Fld<>);
+  // the window base and tid are opaque so that ptxas holds them instead of re-deriving them (S2UR / S2R) at every use
+  using FW = Fld<R, WPL>;  // a primitive plane of the ring
+  using FC = Fld<R, NC>;   // an exchange field LOX .. FY
+  constexpr uint32_t ES = sizeof(R), CF = FC::BYTES;
+  uint32_t sb = smem_u32(smem);
+  asm volatile("" : "+r"(sb));
+  const uint32_t sm_ring = sb + 64u, sm_xy = sm_ring + (uint32_t)(NW * 5 * WPL) * ES, sm_raw = sm_xy + (uint32_t)(6 * 5 * NC) * ES;
+  (void)ring; (void)xy;
 
-  const int tid = threadIdx.x;
+  int tid = threadIdx.x;
+  asm volatile("" : "+r"(tid));
   // warps 0-7: interior columns (two rows of 16 per warp); warp 8: x ring (i = -1, 16); warp 9: y ring (j = -1, 16)
   int ii, jj;
   if (tid < PS * PS) { jj = 1 + (tid >> 4); ii = 1 + (tid & 15); }
   else if (tid < PS * PS + 32) { const int l = tid - PS * PS; jj = 1 + (l >> 1); ii = (l & 1) ? FT - 1 : 0; }
   else { const int l = tid - PS * FT; jj = (l < PS) ? 0 : FT - 1; ii = 1 + (l & (PS - 1)); }
   const int col = jj * FT + ii;
-  const bool in_i = ii >= 1 && ii <= PS, in_j = jj >= 1 && jj <= PS, interior = in_i && in_j;
+  // the role is a property of the warp (0-7 interior, 8 the x ring, 9 the y ring): flags from a warp broadcast
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+  const bool in_i = warp != PS * PS / 32, in_j = warp != PS * PS / 32 + 1, interior = in_i && in_j;
   const int wb = (jj + GW - 1) * SWP + (ii + GW - 1);
+  // per-thread addresses: own cell in ring slot 0 (vector part, scalar part at + dws), own column in LOX (cv, cs)
+  const uint32_t w16 = sm_ring + 16u * (uint32_t)wb, dws = FW::SD - (16u - ES) * (uint32_t)wb;
+  const uint32_t cv = sm_xy + 16u * (uint32_t)col, cs = cv + FC::SD - (16u - ES) * (uint32_t)col;
+  uint32_t wo[NW];  // CTA-uniform byte offsets of the ring slots holding planes t-RW .. t+RW; rotate once per step
+#pragma unroll
+  for (int k = 0; k < NW; ++k) wo[k] = (uint32_t)k * FW::BYTES;
+  const bool feeder = tid == PS * FT;  // lane 0 of the least loaded warp issues the bulk copies and waits for them
 
   const int my_groups = (Ng - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int total_planes = my_groups * NPL;
-  auto issue = [&](int n) {  // thread 0 only
+  auto issue = [&](int n) {  // the feeder lane only
+    asm volatile("" : "+r"(n));  // keeps the descriptor arithmetic inside the feeder's branch
     if (n >= total_planes) return;
     const int m = n / NPL, pl = n - m * NPL;
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
@@ -123,26 +144,47 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   GridFeed<R, SWP, NPL, NT> gf;
   gf.reset();
   if (GRID) { gf.feed(gio, my_groups, raw, tid); gf.feed(gio, my_groups, raw + 5 * WPL, tid); }
-  else if (tid == 0) { issue(0); issue(1); }
+  else if (feeder) { issue(0); issue(1); }
 
   Cnt c = {0, 0, 0};
   typename Bits<R>::U best = 0;  // running maximum of the updated cells' wave speed (next_max_speed)
   int nseq = 0;
-  // grid mode: a thread waits for its own copies of raw plane nseq; the CTA barrier that follows publishes the plane
-  auto landed = [&]() { if (GRID) cp_async_wait<1>(); };
-  auto convert = [&](int slot) {
-    const int st = nseq & 1;
-    if (!GRID) mbar_wait(bar + st, (uint32_t)((nseq >> 1) & 1));
-    const R* rp = raw + (size_t)st * 5 * SS;
-    R* wp = ring + slot * 5 * WPL;
-    for (int idx = tid; idx < WPL; idx += NT) {
-      const int b = idx / SWP, a = idx - b * SWP;
-      stv(wp, WPL, idx, Op::c2p(ld5(rp + (b + off) * S + (a + off), SS), p, c));
+  // raw plane nseq has landed: grid mode: a thread waits for its own copies; batch mode: the feeder lane polls the mbarrier.
+  // The CTA barrier that follows publishes the plane to all threads.
+  auto landed = [&]() {
+    if (GRID) cp_async_wait<1>();
+    else if (feeder) mbar_wait(bar + (nseq & 1), (uint32_t)((nseq >> 1) & 1));
+  };
+  // con->prim of raw plane nseq into the ring slot at byte offset slot_off: cells tid and, for CR0 <= tid < CR2, tid + CSH
+  // (CSH a whole number of plane rows: both cells of a thread share the column, one raw offset serves both)
+  constexpr int CSH = (NT / SWP) * SWP, CR0 = NT - CSH, CR2 = WPL - CSH;
+  uint32_t roff0;
+  {
+    const int b = tid / SWP, a = tid - b * SWP;
+    roff0 = (uint32_t)((b + off) * S + (a + off)) * ES;
+    asm volatile("" : "+r"(roff0));
+  }
+  auto convert = [&](uint32_t slot_off) {
+    const uint32_t rp = sm_raw + (uint32_t)(nseq & 1) * (uint32_t)(5 * SS) * ES + roff0;
+    const uint32_t dv = sm_ring + slot_off + 16u * (uint32_t)tid, ds = sm_ring + slot_off + FW::SD + ES * (uint32_t)tid;
+    const uint32_t sS = (uint32_t)SS * ES;
+    {
+      V5<R> U;
+#pragma unroll
+      for (int q = 0; q < 5; ++q) U[q] = *sm_ptr<const R>(rp + (uint32_t)q * sS);
+      FW::st(dv, ds, Op::c2p(U, p, c));
+    }
+    if (tid >= CR0 && tid < CR2) {
+      const uint32_t rp1 = rp + (uint32_t)((CSH / SWP) * S) * ES;
+      V5<R> U;
+#pragma unroll
+      for (int q = 0; q < 5; ++q) U[q] = *sm_ptr<const R>(rp1 + (uint32_t)q * sS);
+      FW::st(dv + 16u * CSH, ds + ES * CSH, Op::c2p(U, p, c));
     }
   };
   auto refill = [&]() {
     if (GRID) gf.feed(gio, my_groups, raw + (size_t)(nseq & 1) * 5 * SS, tid);
-    else if (tid == 0) { fence_async_smem(); issue(nseq + 2); }
+    else if (feeder) { fence_async_smem(); issue(nseq + 2); }
     ++nseq;
   };
 
@@ -163,19 +205,16 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
     const size_t pstr_in = GRID ? N2 : (size_t)SS, vstr_in = GRID ? N3 : nS;
     R* gff = face_flux ? face_flux + grp * 9 * 5 * PS * PS : nullptr;
     for (int k = 0; k < NW; ++k) {  // prologue: planes -1-RW .. -1+RW
-      if (GRID) { landed(); __syncthreads(); }
-      convert(k);
+      landed();
+      __syncthreads();
+      convert(wo[k]);
       __syncthreads();
       refill();
     }
-    int sl = 0;  // ring slot of plane t-RW
 
 #pragma unroll 1
     for (int t = -1; t <= PS; ++t) {
       const bool tin = t >= 0 && t < PS;
-      int slot[NW];
-#pragma unroll
-      for (int s = 0; s < NW; ++s) slot[s] = (sl + s < NW) ? sl + s : sl + s - NW;
       // ================= P1: face states of plane t, Hancock half step, F_z(t), update of plane t-1 =================
       if (tin || interior) {
         V5<R> Uold;
@@ -185,43 +224,43 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
 #pragma unroll
           for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += vstr_in; }
         }
-        const R* wpl = ring + slot[RW] * 5 * WPL;
-        const V5<R> W0 = ldv(wpl, WPL, wb);
+        const uint32_t w0 = w16 + wo[RW], s0 = w0 + dws;
+        const V5<R> W0 = FW::ld(w0, s0);
         V5<R> lox, upx, loy, upy, loz, upz, inc;
         {
-          const V5<R> Wb = ldv(wpl, WPL, wb - 1), Wc = ldv(wpl, WPL, wb + 1);
+          const V5<R> Wb = FW::ld(w0 - 16u, s0 - ES), Wc = FW::ld(w0 + 16u, s0 + ES);
           V5<R> Wa = Wb, Wd = Wc;
-          if (RECON == RECON_PPM) { Wa = ldv(wpl, WPL, wb - 2); Wd = ldv(wpl, WPL, wb + 2); }
+          if (RECON == RECON_PPM) { Wa = FW::ld(w0 - 32u, s0 - 2 * ES); Wd = FW::ld(w0 + 32u, s0 + 2 * ES); }
           Mo::template recon<0>(Wa, Wb, W0, Wc, Wd, p, lox, upx);
           const V5<R> fu = Mo::template flux<0>(upx, p), fl = Mo::template flux<0>(lox, p);
 #pragma unroll
           for (int q = 0; q < 5; ++q) inc[q] = fu[q] - fl[q];
         }
         {
-          const V5<R> Wb = ldv(wpl, WPL, wb - SWP), Wc = ldv(wpl, WPL, wb + SWP);
+          const V5<R> Wb = FW::ld(w0 - 16u * SWP, s0 - ES * SWP), Wc = FW::ld(w0 + 16u * SWP, s0 + ES * SWP);
           V5<R> Wa = Wb, Wd = Wc;
-          if (RECON == RECON_PPM) { Wa = ldv(wpl, WPL, wb - 2 * SWP); Wd = ldv(wpl, WPL, wb + 2 * SWP); }
+          if (RECON == RECON_PPM) { Wa = FW::ld(w0 - 32u * SWP, s0 - 2 * ES * SWP); Wd = FW::ld(w0 + 32u * SWP, s0 + 2 * ES * SWP); }
           Mo::template recon<1>(Wa, Wb, W0, Wc, Wd, p, loy, upy);
           const V5<R> fu = Mo::template flux<1>(upy, p), fl = Mo::template flux<1>(loy, p);
 #pragma unroll
           for (int q = 0; q < 5; ++q) inc[q] = inc[q] + (fu[q] - fl[q]);
         }
         {
-          const V5<R> Wb = ldv(ring + slot[RW - 1] * 5 * WPL, WPL, wb), Wc = ldv(ring + slot[RW + 1] * 5 * WPL, WPL, wb);
+          const V5<R> Wb = FW::ld(w16 + wo[RW - 1], w16 + wo[RW - 1] + dws), Wc = FW::ld(w16 + wo[RW + 1], w16 + wo[RW + 1] + dws);
           V5<R> Wa = Wb, Wd = Wc;
-          if (RECON == RECON_PPM) { Wa = ldv(ring + slot[0] * 5 * WPL, WPL, wb); Wd = ldv(ring + slot[2 * RW] * 5 * WPL, WPL, wb); }
+          if (RECON == RECON_PPM) { Wa = FW::ld(w16 + wo[0], w16 + wo[0] + dws); Wd = FW::ld(w16 + wo[2 * RW], w16 + wo[2 * RW] + dws); }
           Mo::template recon<2>(Wa, Wb, W0, Wc, Wd, p, loz, upz);
           const V5<R> fu = Mo::template flux<2>(upz, p), fl = Mo::template flux<2>(loz, p);
 #pragma unroll
           for (int q = 0; q < 5; ++q) inc[q] = p.hnu * (inc[q] + (fu[q] - fl[q]));
         }
         if (tin && in_j) {
-          stv(fld(LF_LOX), NC, col, Op::correct(lox, inc, p, c));
-          stv(fld(LF_UPX), NC, col, Op::correct(upx, inc, p, c));
+          FC::st(cv + LF_LOX * CF, cs + LF_LOX * CF, Op::correct(lox, inc, p, c));
+          FC::st(cv + LF_UPX * CF, cs + LF_UPX * CF, Op::correct(upx, inc, p, c));
         }
         if (tin && in_i) {
-          stv(fld(LF_LOY), NC, col, Op::correct(loy, inc, p, c));
-          stv(fld(LF_UPY), NC, col, Op::correct(upy, inc, p, c));
+          FC::st(cv + LF_LOY * CF, cs + LF_LOY * CF, Op::correct(loy, inc, p, c));
+          FC::st(cv + LF_UPY * CF, cs + LF_UPY * CF, Op::correct(upy, inc, p, c));
         }
         if (interior) {
           if (t >= 0) {
@@ -254,36 +293,45 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
       // ================= P2: F_x(t), F_y(t), boundary-flux stores; con->prim of the next plane =================
       if (tin) {
         if (in_j && ii >= 1) {
-          const V5<R> f = Op::template riemann<0>(ldv(fld(LF_UPX), NC, col - 1), ldv(fld(LF_LOX), NC, col), p, c);
-          stv(fld(LF_FX), NC, col, f);
+          const V5<R> f = Op::template riemann<0>(FC::ld(cv + LF_UPX * CF - 16u, cs + LF_UPX * CF - ES), FC::ld(cv + LF_LOX * CF, cs + LF_LOX * CF), p, c);
+          FC::st(cv + LF_FX * CF, cs + LF_FX * CF, f);
           if (gff && ((ii - 1) & 7) == 0) st5(gff + (size_t)(((ii - 1) >> 3) * 5) * 256 + t * PS + (jj - 1), 256, f);
         }
         if (in_i && jj >= 1) {
-          const V5<R> f = Op::template riemann<1>(ldv(fld(LF_UPY), NC, col - FT), ldv(fld(LF_LOY), NC, col), p, c);
-          stv(fld(LF_FY), NC, col, f);
+          const V5<R> f = Op::template riemann<1>(FC::ld(cv + LF_UPY * CF - 16u * FT, cs + LF_UPY * CF - ES * FT), FC::ld(cv + LF_LOY * CF, cs + LF_LOY * CF), p, c);
+          FC::st(cv + LF_FY * CF, cs + LF_FY * CF, f);
           if (gff && ((jj - 1) & 7) == 0) st5(gff + (size_t)((3 + ((jj - 1) >> 3)) * 5) * 256 + t * PS + (ii - 1), 256, f);
         }
       }
-      if (conv) convert(sl);
+      if (conv) convert(wo[0]);
       __syncthreads();  // barrier B
       if (conv) refill();
 
       // ================= P3: carried x+y flux difference of plane t minus F_z(t) =================
       if (tin && interior) {
-        const V5<R> x1 = ldv(fld(LF_FX), NC, col + 1), x0 = ldv(fld(LF_FX), NC, col);
-        const V5<R> y1 = ldv(fld(LF_FY), NC, col + FT), y0 = ldv(fld(LF_FY), NC, col);
+        const V5<R> x1 = FC::ld(cv + LF_FX * CF + 16u, cs + LF_FX * CF + ES), x0 = FC::ld(cv + LF_FX * CF, cs + LF_FX * CF);
+        const V5<R> y1 = FC::ld(cv + LF_FY * CF + 16u * FT, cs + LF_FY * CF + ES * FT), y0 = FC::ld(cv + LF_FY * CF, cs + LF_FY * CF);
 #pragma unroll
         for (int q = 0; q < 5; ++q) Dz[q] = ((x1[q] - x0[q]) + (y1[q] - y0[q])) - Dz[q];
       }
-      sl = (sl + 1 < NW) ? sl + 1 : 0;
+      {  // the ring slots rotate: the plane converted in P2 is now the newest
+        const uint32_t w = wo[0];
+#pragma unroll
+        for (int k = 0; k + 1 < NW; ++k) wo[k] = wo[k + 1];
+        wo[NW - 1] = w;
+      }
     }
   }
   flush_counters(c, status);
   flush_speed(best, p.next_speed);
 }
 
-template <class R, int RECON, int RS, int FAST, int MINB, int GRID = 0> cudaError_t launch_mhm_lean(const SolveArgs<R>& a) {
-  auto kern = mhm_lean_kernel<R, RECON, RS, FAST, MINB, GRID>;
+template <class R, int RECON, int RS, int FAST, int MINB, int GRID = 0, int GC = -1> cudaError_t launch_mhm_lean(const SolveArgs<R>& a) {
+  // the default options at the ghost width of the AMR batches (g = 3) have their own fp32 instantiation (hydro_lean_ctu.cuh)
+  if constexpr (FAST && !GRID && GC < 0 && sizeof(R) == 4) {
+    if (a.g == 3) return launch_mhm_lean<R, RECON, RS, FAST, MINB, GRID, 3>(a);
+  }
+  auto kern = mhm_lean_kernel<R, RECON, RS, FAST, MINB, GRID, GC>;
   const size_t smem = mhm_smem_bytes(sizeof(R), RECON, a.g);
   if (smem > SMEM_MAX_OPTIN) return cudaErrorInvalidConfiguration;
   static int sms = 0;
