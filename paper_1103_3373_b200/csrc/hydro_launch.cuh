@@ -60,10 +60,14 @@ constexpr size_t mhm_smem_bytes(size_t elem, int recon, int g) {
 }
 // fused VL kernel (hydro_lean_vl.cuh): plus cells within E = recon + 2 of the interior + one warp of boundary faces
 constexpr int VL_NT(int recon) { return 320 + 64 * (recon + 1) + 32; }
-// mbarriers | one primitive plane | W-half ring | LOX UPX LOY UPY FX FY | one raw plane
+// merged schedule (two CTA barriers per plane instead of four; its first-pass fluxes need two fields of their own): fp32 only.
+// Measured per 4096 groups: fp32 VL+PLM+Roe 1.87 -> 1.81 ms; fp64 5.08 -> 5.21 ms (and fp64 + PPM has no room for the fields)
+constexpr bool vl_merged(size_t elem, int recon) { return (void)recon, elem == 4; }
+// mbarriers | one primitive plane | W-half ring | LOX UPX LOY UPY FX FY | (merged: F1_x F1_y) | one raw plane
 constexpr size_t vl_smem_bytes(size_t elem, int recon, int g) {
   const size_t S = PS + 2 * g, SW = PS + 2 * (recon + 3), SH = PS + 2 * (recon + 2), NW = 2 * (1 + recon) + 1;
-  return 64 + elem * (5 * S * S + 5 * SW * SW + NW * 5 * SH * SH + (size_t)30 * LEAN_COLS);
+  const size_t SF = PS + 2 * (recon + 2) + 1, FPL = (SF * SF + 3) / 4 * 4;
+  return 64 + elem * (5 * S * S + 5 * SW * SW + NW * 5 * SH * SH + (size_t)30 * LEAN_COLS + (vl_merged(elem, recon) ? 2 * 5 * FPL : 0));
 }
 constexpr bool lean_available(int precision_bytes, int scheme, int recon) {
   (void)precision_bytes; (void)recon;

@@ -21,7 +21,7 @@
 
 namespace hydro {
 
-template <class R, int RECON, int RS, int FAST, int GRID>
+template <class R, int RECON, int RS, int FAST, int GRID, int MERGE>
 __global__ void __launch_bounds__(VL_NT(RECON), 1)
 vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g_arg, Par<R> p,
                const R* __restrict__ max_speed, R cfl, long long* status, GridIO<R> gio) {
@@ -35,6 +35,10 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
   constexpr int NP = 320 + 64 * (E - 1);                // plus cells; then one warp of boundary-face jobs
   constexpr int NT = 320 + 64 * (RECON + 1) + 32;  // == VL_NT(RECON)
   static_assert(2 * FPL <= 4 * NC, "first-pass flux fields must fit in LOX..UPY");
+  // MERGE: the two stages share their barrier intervals (two CTA barriers per plane instead of four): stage 2 then runs one more
+  // plane behind (b = a - 2 - RW) and the first-pass fluxes get their own fields.  The W-half ring needs no extra plane: S2
+  // overwrites plane b - RW in the interval AFTER the one in which S3 read it for the last time.
+  constexpr int NH = NW;
   apply_device_dt(p, max_speed, cfl);
 
   const int g = GRID ? GW : g_arg;  // grid mode: the ghost zones come from the grid, always at the minimum width
@@ -47,11 +51,12 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
   extern __shared__ __align__(16) unsigned char smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
   R* wpl = reinterpret_cast<R*>(smem + 64);            // one field of WPL cells: primitive plane a (W(a-1) lives in registers)
-  R* hring = wpl + 5 * WPL;                       // [NW] fields of HPL cells: W-half planes b-RW .. b+RW
-  R* xy = hring + NW * 5 * HPL;                        // [6] fields of NC cells: LOX UPX LOY UPY FX FY
-  R* raw = xy + 6 * 5 * NC;                            // [5][SS] one landing plane: a step is long against a plane load
-  R* f1x = xy;                                         // first-pass fluxes alias LOX.. (FPL cells each)
-  R* f1y = xy + 5 * FPL;
+  R* hring = wpl + 5 * WPL;                       // [NH] fields of HPL cells: W-half planes b-RW .. b+RW
+  R* xy = hring + NH * 5 * HPL;                        // [6] fields of NC cells: LOX UPX LOY UPY FX FY
+  R* f1own = xy + 6 * 5 * NC;                          // MERGE: [2] fields of FPL cells, the first-pass fluxes
+  R* raw = f1own + (MERGE ? 2 * 5 * FPL : 0);          // [5][SS] one landing plane: a step is long against a plane load
+  R* f1x = MERGE ? f1own : xy;                         // not merged: the first-pass fluxes alias LOX.. (disjoint lifetimes)
+  R* f1y = f1x + 5 * FPL;
   auto fld = [&](int k) { return xy + k * 5 * NC; };
 
   const int tid = threadIdx.x;
@@ -148,16 +153,21 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     refill();
 
 #pragma unroll 1
-    for (int a = -E; a <= PS + E; ++a) {
+    for (int a = -E; a <= PS + E + MERGE; ++a) {
+      const bool a_s1 = !MERGE || a <= PS + E;     // merged: one more step, which only drains stage 2
       const bool a_in = a >= 0 && a < PS;          // plane a holds arm cells
       const bool a_xy = a < PS + E;                // plane a needs its in-plane first-pass fluxes
       const R* wa = wpl;
       // arm cells (outside the interior columns) live in planes 0..15 only, but need W(-1) and F1_z at faces 0 and 16
-      const bool act1 = cell && (c_int || (a >= -1 && a <= PS));
-      const bool zf = cell && (c_int || (a >= 0 && a <= PS));
+      const bool act1 = a_s1 && cell && (c_int || (a >= -1 && a <= PS));
+      const bool zf = a_s1 && cell && (c_int || (a >= 0 && a <= PS));
       const bool xyf = cell && a_xy && (c_int || a_in);
-      // ================= S1: first-order fluxes of plane a (PAPER.md:46) =================
+      const int b = a - 1 - RW - MERGE;            // plane of stage 2
+      const bool b_in = b >= 0 && b < PS;
+      const bool conv = a + 1 <= PS - 1 + GW;      // plane a+1 replaces plane a in S4 (last read in S1)
       V5<R> W0, f1z;
+      auto stage1 = [&]() {
+      // ================= S1: first-order fluxes of plane a (PAPER.md:46) =================
       if (act1) {
         W0 = ldv(wa, WPL, wb);
         if (xyf) {
@@ -177,8 +187,8 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
           stv(f1y, FPL, (edge + E) * SF + (r + E), Op::template riemann<1>(ldv(wa, WPL, yw - SW), ldv(wa, WPL, yw), p, c));
         }
       }
-      __syncthreads();  // barrier 1
-
+      };
+      auto stage2 = [&]() {
       // ================= S2: half-step state of plane a-1 -> W-half ring =================
       if (act1) {
         V5<R> s1;
@@ -205,17 +215,15 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
           }
 #pragma unroll
           for (int q = 0; q < 5; ++q) U[q] = U[q] - p.hnu * (s1prev[q] + (f1z[q] - f1zprev[q]));
-          stv(hring + ((ap + E) % NW) * 5 * HPL, HPL, hb, Op::c2p(U, p, c));
+          stv(hring + ((ap + E) % NH) * 5 * HPL, HPL, hb, Op::c2p(U, p, c));
         }
         Wprev = W0;
         s1prev = s1;
         f1zprev = f1z;
       }
-      __syncthreads();  // barrier 2
-
+      };
+      auto stage3 = [&]() {
       // ================= S3: face states of W-half plane b, F_z(b), update of plane b-1 =================
-      const int b = a - 1 - RW;
-      const bool b_in = b >= 0 && b < PS;
       if (s2 && b >= -1 && (b_in || interior)) {
         V5<R> Uold;
         const bool upd = interior && b >= 1;
@@ -224,7 +232,7 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
 #pragma unroll
           for (int q = 0; q < 5; ++q) { Uold[q] = __ldg(gin); gin += vstr_in; }
         }
-        const R* hp = hring + ((b + E) % NW) * 5 * HPL;
+        const R* hp = hring + ((b + E) % NH) * 5 * HPL;
         const V5<R> H0 = ldv(hp, HPL, hb);
         if (b_in && in_j) {
           const V5<R> Wb = ldv(hp, HPL, hb - 1), Wc = ldv(hp, HPL, hb + 1);
@@ -243,11 +251,11 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
           stv(fld(LF_UPY), NC, col, u);
         }
         if (interior) {
-          const V5<R> Wb = ldv(hring + ((b - 1 + E) % NW) * 5 * HPL, HPL, hb), Wc = ldv(hring + ((b + 1 + E) % NW) * 5 * HPL, HPL, hb);
+          const V5<R> Wb = ldv(hring + ((b - 1 + E) % NH) * 5 * HPL, HPL, hb), Wc = ldv(hring + ((b + 1 + E) % NH) * 5 * HPL, HPL, hb);
           V5<R> Wa = Wb, Wd = Wc, lz, uz;
           if (RECON == RECON_PPM) {
-            Wa = ldv(hring + ((b - 2 + E) % NW) * 5 * HPL, HPL, hb);
-            Wd = ldv(hring + ((b + 2 + E) % NW) * 5 * HPL, HPL, hb);
+            Wa = ldv(hring + ((b - 2 + E) % NH) * 5 * HPL, HPL, hb);
+            Wd = ldv(hring + ((b + 2 + E) % NH) * 5 * HPL, HPL, hb);
           }
           Mo::template recon<2>(Wa, Wb, H0, Wc, Wd, p, lz, uz);
           if (b >= 0) {
@@ -273,10 +281,8 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
           if (b < PS) uzc = uz;
         }
       }
-      const bool conv = a + 1 <= PS - 1 + GW;
-      if (conv) landed();
-      __syncthreads();  // barrier 3
-
+      };
+      auto stage4 = [&]() {
       // ================= S4: F_x(b), F_y(b), boundary-flux stores; con->prim of plane a+1 =================
       if (s2 && b_in) {
         if (in_j && ii >= 1) {
@@ -290,16 +296,41 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
           if (gff && ((jj - 1) & 7) == 0) st5(gff + (size_t)((3 + ((jj - 1) >> 3)) * 5) * 256 + b * PS + (ii - 1), 256, f);
         }
       }
-      if (conv) convert();  // plane a+1 replaces plane a, read for the last time in S1
-      __syncthreads();  // barrier 4
-      if (conv) refill();
-
+      };
+      auto stage5 = [&](bool bin5) {
       // ================= S5: carried x+y flux difference of plane b minus F_z(b) =================
-      if (b_in && interior) {
+      if (bin5 && interior) {
         const V5<R> x1 = ldv(fld(LF_FX), NC, col + 1), x0 = ldv(fld(LF_FX), NC, col);
         const V5<R> y1 = ldv(fld(LF_FY), NC, col + FT), y0 = ldv(fld(LF_FY), NC, col);
 #pragma unroll
         for (int q = 0; q < 5; ++q) Dz[q] = ((x1[q] - x0[q]) + (y1[q] - y0[q])) - Dz[q];
+      }
+      };
+      if (MERGE) {
+        // two barrier intervals per plane: {S5 of the previous plane, S1 of plane a, S3 of plane b} | {S2, S4, con->prim}
+        stage5(b - 1 >= 0 && b - 1 < PS);
+        stage1();
+        stage3();
+        if (conv) landed();
+        __syncthreads();  // barrier 1
+        stage2();
+        stage4();
+        if (conv) convert();
+        __syncthreads();  // barrier 2
+        if (conv) refill();
+      } else {
+        stage1();
+        __syncthreads();  // barrier 1
+        stage2();
+        __syncthreads();  // barrier 2
+        stage3();
+        if (conv) landed();
+        __syncthreads();  // barrier 3
+        stage4();
+        if (conv) convert();  // plane a+1 replaces plane a, read for the last time in S1
+        __syncthreads();  // barrier 4
+        if (conv) refill();
+        stage5(b_in);
       }
     }
   }
@@ -308,7 +339,7 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
 }
 
 template <class R, int RECON, int RS, int FAST, int GRID = 0> cudaError_t launch_vl_lean(const SolveArgs<R>& a) {
-  auto kern = vl_lean_kernel<R, RECON, RS, FAST, GRID>;
+  auto kern = vl_lean_kernel<R, RECON, RS, FAST, GRID, vl_merged(sizeof(R), RECON) ? 1 : 0>;
   const size_t smem = vl_smem_bytes(sizeof(R), RECON, a.g);
   if (smem > SMEM_MAX_OPTIN) return cudaErrorInvalidConfiguration;
   static int sms = 0;
