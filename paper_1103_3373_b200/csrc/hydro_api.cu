@@ -198,6 +198,9 @@ static int make_plan(const void* in, const void* out, const void* ff, int Ng, R 
   par.gamma = gamma;
   par.gm1 = gamma - R(1);
   par.igm1 = R(1) / par.gm1;
+  par.ig1 = R(1) / (gamma + R(1));
+  par.ig2 = R(0.5) / gamma;
+  par.sA0 = (R)std::sqrt(2.0 / ((double)gamma + 1.0));
   par.nu = device_dt ? R(0) : dt / dh;
   par.hnu = R(0.5) * par.nu;
   par.theta = (R)theta;

@@ -296,6 +296,7 @@ __device__ __noinline__ FluxRet<R> roe_fallback_flux(R l0, R l1, R l2, R l3, R l
                                                      R igm1, int mode) {
   Par<R> p;
   p.gamma = gamma; p.gm1 = gm1; p.igm1 = igm1; p.roe_fallback = mode;
+  p.ig1 = p.ig2 = p.sA0 = R(0);  // the generic solvers of hydro_math.cuh form their own constants
   p.nu = p.hnu = p.theta = p.min_dens = p.min_pres = R(0);
   p.limiter = p.char_limit = p.next_norm = 0;
   p.next_speed = nullptr;
@@ -423,12 +424,13 @@ template <class R> __device__ __forceinline__ V5<R> lean_hlle(const V5<R>& WL, c
 // ---- c4: exact solver (Toro ch. 4; S11): the same pressure function, Newton iteration, tolerance, iteration cap and
 // sampling as hydro_math.cuh `exact`, organised for the GPU ("much more time-consuming"; it is config 5):
 //   * fully inlined, everything in registers (the round-1 version was an out-of-line call with pointer arguments);
-//   * powers through one logarithm: with w = lg2(p), (p/P_K)^e = ex2(e (w - lg2 P_K)); lg2(p) is shared by both sides and
-//     lg2(P_K) leaves the loop.  fp32 uses the SFU lg2 / ex2 approximations (relative error of z ~ 3e-8, far inside the
-//     1e-6 iteration tolerance); fp64 calls log2 / exp2 once each instead of pow twice per side;
+//   * powers as (p/P_K)^e = ex2(e lg2(p / P_K)), evaluated only on a side that is a rarefaction (with about one evaluation per
+//     solve, hoisting lg2 P_K out of the iteration cost more than it saved: in fp64 log2 was 19 % of the kernel's instructions).
+//     fp32 uses the SFU lg2 / ex2 approximations (relative error of z ~ 3e-8, far inside the 1e-6 tolerance);
 //   * the shock branch needs one rsqrt per evaluation: sqrt(A_K / (p + B_K)) = sqrt(A_K) rsqrt(p + B_K);
-//   * no re-evaluation of f after the last iterate: the last Newton step delta < tol p gives f(p + delta) = f + f' delta with a
-//     relative error of order tol^2 (1e-12 in fp32, 1e-24 in fp64), likewise z.
+//   * Halley's third-order iteration (f'' costs four more multiplies per side) and no evaluation at the accepted iterate: a step
+//     delta below 4e-3 p (fp32) / 2e-5 p (fp64) is accepted with f(p + delta) = f + f' delta + f'' delta^2 / 2 and z likewise, errors
+//     of order (delta/p)^3 -- so that smooth data need ONE evaluation per solve (plus one fp32 evaluation for the fp64 start).
 template <class R> __device__ __forceinline__ R l_lg2(R x);
 template <class R> __device__ __forceinline__ R l_ex2(R x);
 #if HYDRO_F32_IEEE
@@ -441,14 +443,15 @@ template <> __device__ __forceinline__ float l_ex2<float>(float x) { float r; as
 template <> __device__ __forceinline__ double l_lg2<double>(double x) { return log2(x); }
 template <> __device__ __forceinline__ double l_ex2<double>(double x) { return exp2(x); }
 
-template <class R> struct ExactSide { R rho, u, P, c, irc, sA, B, k, w; };
-template <class R> struct ExactConst { R gamma, gm1, igm1, ig1, mu, e1; };  // ig1 = 1/(g+1), mu = (g-1)/(g+1), e1 = (g-1)/(2g)
-template <class R> __device__ __forceinline__ ExactConst<R> exact_const(R gamma, R gm1, R igm1) {
+template <class R> struct ExactSide { R rho, u, P, c, irc, sA, B, k, iP; };
+template <class R> struct ExactConst { R gamma, gm1, igm1, ig1, mu, e1, sA0; };  // ig1 = 1/(g+1), mu = (g-1)/(g+1), e1 = (g-1)/(2g), sA0 = sqrt(2/(g+1))
+template <class R> __device__ __forceinline__ ExactConst<R> exact_const(R gamma, R gm1, R igm1, R ig1, R ig2, R sA0) {
   ExactConst<R> k;
   k.gamma = gamma; k.gm1 = gm1; k.igm1 = igm1;
-  k.ig1 = l_rcp(gamma + R(1));
-  k.mu = gm1 * k.ig1;
-  k.e1 = gm1 * (R(0.5) * l_rcp(gamma));
+  k.ig1 = ig1;
+  k.mu = gm1 * ig1;
+  k.e1 = gm1 * ig2;
+  k.sA0 = sA0;
   return k;
 }
 template <class R> __device__ __forceinline__ ExactSide<R> exact_side(R rho, R u, R P, const ExactConst<R>& k) {
@@ -457,61 +460,67 @@ template <class R> __device__ __forceinline__ ExactSide<R> exact_side(R rho, R u
   const R gP = k.gamma * P;
   s.irc = l_rsqrt(gP * rho);                      // 1 / (rho c)
   s.c = gP * s.irc;
-  s.sA = l_sqrt(k.ig1 + k.ig1) * l_rsqrt(rho);    // sqrt(A_K), A_K = 2 / ((g+1) rho)
+  s.sA = k.sA0 * l_rsqrt(rho);                    // sqrt(A_K), A_K = 2 / ((g+1) rho)
   s.B = k.mu * P;                                 // (g-1)/(g+1) P
   s.k = (s.c + s.c) * k.igm1;                     // 2 c / (g-1)
-  s.w = l_lg2(P);
+  s.iP = l_rcp(P);
   return s;
 }
-// f_K(p), f_K'(p) and, on the rarefaction branch, z = (p/P_K)^e1 (else 0); w = lg2(p), ips = 1/p
-template <class R> __device__ __forceinline__ void exact_fn(R ps, R w, R ips, const ExactSide<R>& s, R e1, R& f, R& df, R& z) {
+// f_K(p), f_K'(p), f_K''(p) and, on the rarefaction branch, z = (p/P_K)^e1 (else 0); ips = 1/p.  f_K is C^2 across
+// p = P_K (both branches give f'' = -(g+1) / (2 g P_K rho_K c_K) there).
+template <class R> __device__ __forceinline__ void exact_fn(R ps, R ips, const ExactSide<R>& s, R e1, R& f, R& df, R& ddf, R& z) {
   if (ps > s.P) {
-    const R rs = l_rsqrt(ps + s.B), q = s.sA * rs, d = ps - s.P;
+    const R rs = l_rsqrt(ps + s.B), q = s.sA * rs, d = ps - s.P, iu = rs * rs, di = d * iu;
     f = d * q;
-    df = q * m_fma(R(-0.5) * d, rs * rs, R(1));
+    df = q * m_fma(R(-0.5), di, R(1));
+    ddf = -(q * iu) * m_fma(R(-0.75), di, R(1));
     z = R(0);
   } else {
-    z = l_ex2(e1 * (w - s.w));
+    z = l_ex2(e1 * l_lg2(ps * s.iP));  // the logarithm of the RATIO, taken only where a rarefaction needs it
     f = s.k * (z - R(1));
     df = (z * s.P * ips) * s.irc;
+    ddf = (e1 - R(1)) * (df * ips);
   }
 }
-// Newton iteration on f_L + f_R + du = 0 from ps (S11: negative iterate -> eps_p, at most 40 evaluations).  Stops when the
-// relative change 2 |delta| / (p_new + p) falls below `stop`; returns the LAST EVALUATED point ps with f, f', z there and the
-// step delta to the accepted iterate ps + delta, whose distance to the root is of order delta^2 / p (Newton is quadratic).
-template <class R> struct ExactIter { R ps, dlt, ips, fL, dL, zL, fR, dR, zR; bool conv; };
+// Iteration on F(p) = f_L + f_R + du = 0 from ps (S11: negative iterate -> eps_p, at most 40 evaluations; S28: Halley's
+// third-order step delta = -t / (1 - t F'' / (2 F')), t = F / F', instead of Newton's -t -- F is increasing and concave, the root
+// unique).  An iterate is ACCEPTED without evaluating F there once the step is small enough for the cubic remainder to be
+// negligible: |delta| < stop * p, error of p + delta of order (delta/p)^3 p.  Returns the last evaluated point ps with f, f',
+// f'', z of both sides there and the step delta to the accepted iterate.
+template <class R> struct ExactIter { R ps, dlt, ips, fL, dL, eL, zL, fR, dR, eR, zR; bool conv; };
 template <class R> __device__ __forceinline__ ExactIter<R> exact_newton(const ExactSide<R>& L, const ExactSide<R>& Rs, R du, R e1, R epsp, R ps, R stop) {
   ExactIter<R> r;
   r.conv = false;
   r.dlt = R(0);
 #pragma unroll 1
   for (int it = 0; it < 40; ++it) {
-    R w = R(0);
-    r.ips = R(0);
-    if (!(ps > L.P) || !(ps > Rs.P)) { w = l_lg2(ps); r.ips = l_rcp(ps); }  // only the rarefaction branch needs them
-    exact_fn(ps, w, r.ips, L, e1, r.fL, r.dL, r.zL);
-    exact_fn(ps, w, r.ips, Rs, e1, r.fR, r.dR, r.zR);
-    R pn = ps - l_div((r.fL + r.fR) + du, r.dL + r.dR);
+    r.ips = l_rcp(ps);
+    exact_fn(ps, r.ips, L, e1, r.fL, r.dL, r.eL, r.zL);
+    exact_fn(ps, r.ips, Rs, e1, r.fR, r.dR, r.eR, r.zR);
+    const R idF = l_rcp(r.dL + r.dR), t = ((r.fL + r.fR) + du) * idF;
+    R den = m_fma(R(-0.5) * t, (r.eL + r.eR) * idF, R(1));
+    if (!(den > R(0.5))) den = R(1);                 // far from the root: a plain Newton step
+    R pn = ps - l_div(t, den);
     if (!(pn > R(0))) pn = epsp;
     r.dlt = pn - ps;
-    if (R(2) * m_abs(r.dlt) < stop * (pn + ps)) { r.conv = true; break; }
+    if (m_abs(r.dlt) < stop * ps) { r.conv = true; break; }
     ps = pn;
   }
   r.ps = ps;
   if (!r.conv) r.dlt = R(0);  // 40 evaluations without convergence: the last evaluated iterate stands
   return r;
 }
-// Stopping rule.  fp32: the oracle's tolerance 1e-6 (S11).  fp64: S11's 1e-12 bounds the error of p*; because the accepted
-// iterate is ps + delta with an error of order delta^2 / p, a step below 1e-7 p already puts it within 1e-14 p of the root --
-// the last evaluation S11's rule would spend only confirms that.  The fp64 iteration moreover starts from the root of an
-// fp32 Newton iteration on the rounded states (SFU logarithms, ~1e-6 p away), so two fp64 evaluations suffice.
+// Acceptance rule (S28).  The accepted iterate ps + delta misses the root by about (delta/p)^3 p (Halley is cubic; the constant is
+// of order one for this F).  fp32: |delta| < 4e-3 p puts it within 1e-7 p, inside the oracle's tolerance 1e-6 (S11).  fp64: S11's
+// 1e-12 bounds the error of p*; |delta| < 2e-5 p gives 1e-14 p.  The fp64 iteration starts from the root of the fp32 iteration on
+// the rounded states (~1e-6 p away), so that ONE fp64 evaluation suffices.
 template <class R> struct ExactStop;
-template <> struct ExactStop<float> { static __device__ __forceinline__ float v() { return 1e-6f; } };
-template <> struct ExactStop<double> { static __device__ __forceinline__ double v() { return 1e-7; } };
+template <> struct ExactStop<float> { static __device__ __forceinline__ float v() { return 4e-3f; } };
+template <> struct ExactStop<double> { static __device__ __forceinline__ double v() { return 2e-5; } };
 
 template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, const V5<R>& WR, const Par<R>& p, Cnt& c) {
   const R g = p.gamma;
-  const ExactConst<R> k = exact_const<R>(g, p.gm1, p.igm1);
+  const ExactConst<R> k = exact_const<R>(g, p.gm1, p.igm1, p.ig1, p.ig2, p.sA0);
   const R ig1 = k.ig1, mu = k.mu, e1 = k.e1;
   const ExactSide<R> L = exact_side(WL[0], WL[1], WL[4], k), Rs = exact_side(WR[0], WR[1], WR[4], k);
   const R du = Rs.u - L.u;
@@ -525,10 +534,10 @@ template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, 
   const R ppv = R(0.5) * (L.P + Rs.P) - R(0.125) * du * (L.rho + Rs.rho) * (L.c + Rs.c);
   R ps = m_max(epsp, ppv);
   if (sizeof(R) == 8) {  // fp64: start from the fp32 root (any start is allowed: the root is unique, f is monotone and concave)
-    const ExactConst<float> kf = exact_const<float>((float)g, (float)p.gm1, (float)p.igm1);
+    const ExactConst<float> kf = exact_const<float>((float)g, (float)p.gm1, (float)p.igm1, (float)p.ig1, (float)p.ig2, (float)p.sA0);
     const ExactSide<float> Lf = exact_side((float)WL[0], (float)WL[1], (float)WL[4], kf),
                            Rf = exact_side((float)WR[0], (float)WR[1], (float)WR[4], kf);
-    const ExactIter<float> rf = exact_newton<float>(Lf, Rf, (float)du, kf.e1, (float)epsp, (float)ps, 1e-6f);
+    const ExactIter<float> rf = exact_newton<float>(Lf, Rf, (float)du, kf.e1, (float)epsp, (float)ps, ExactStop<float>::v());
     const R pf = (R)(rf.ps + rf.dlt);
     if (pf > epsp && pf < R(3.0e38)) ps = pf;  // finite and positive in fp32's range; otherwise keep the linearised guess
   }
@@ -537,10 +546,12 @@ template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, 
   ps = it.ps;
   R fL = it.fL, fR = it.fR;
   const R dL = it.dL, dR = it.dR, zL = it.zL, zR = it.zR, dlt = it.dlt, ips = it.ips;
-  // first-order update of the last evaluation to the accepted iterate ps + dlt
-  fL = m_fma(dL, dlt, fL);
-  fR = m_fma(dR, dlt, fR);
-  const R zs = m_fma(e1 * ips, dlt, R(1));  // z(ps + dlt) / z(ps)
+  // second-order update of the last evaluation to the accepted iterate ps + dlt (error of order (dlt/p)^3, as the iterate's own)
+  const R hd = R(0.5) * dlt;
+  fL = m_fma(m_fma(it.eL, hd, dL), dlt, fL);
+  fR = m_fma(m_fma(it.eR, hd, dR), dlt, fR);
+  const R x = dlt * ips;
+  const R zs = m_fma(m_fma(R(0.5) * (e1 - R(1)), x, R(1)), e1 * x, R(1));  // z(ps + dlt) / z(ps) = (1 + x)^e1 to second order
   const R pst = ps + dlt;
   const R us = R(0.5) * (L.u + Rs.u) + R(0.5) * (fR - fL);
   // sample at x/t = 0 on the side of the contact given by sign(u*) (S19: u* = 0 -> left); right side mirrored
@@ -548,15 +559,16 @@ template <class R> __device__ __forceinline__ V5<R> lean_exact(const V5<R>& WL, 
   const R sg = left ? R(1) : R(-1);
   const R rK = left ? L.rho : Rs.rho, PK = left ? L.P : Rs.P, cK = left ? L.c : Rs.c, vK = left ? L.u : Rs.u;
   const R ircK = left ? L.irc : Rs.irc, zE = left ? zL : zR;
-  const R pr = pst * l_rcp(PK);
+  const R pr = pst * (left ? L.iP : Rs.iP);
   // z at the accepted iterate.  If the last evaluation took the shock branch (zE = 0) while the accepted iterate is a
-  // rarefaction, p* lies within one Newton step (< tol p) of P_K and z = 1 + e1 (p*/P_K - 1) to second order
-  const R zK = zE > R(0) ? zE * zs : m_fma(e1, pr - R(1), R(1));
+  // rarefaction, p* lies within one accepted step (< stop p) of P_K and z = (1 + y)^e1, y = p*/P_K - 1, to second order
+  const R y = pr - R(1);
+  const R zK = zE > R(0) ? zE * zs : m_fma(m_fma(R(0.5) * (e1 - R(1)), y, R(1)), e1 * y, R(1));
   V5<R> W;
   W[2] = left ? WL[2] : WR[2];
   W[3] = left ? WL[3] : WR[3];
   if (pst > PK) {  // shock
-    const R ig2 = R(0.5) * l_rcp(g);
+    const R ig2 = p.ig2;
     const R S = vK - sg * cK * l_sqrt(m_fma((g + R(1)) * ig2, pr, p.gm1 * ig2));
     const bool undisturbed = left ? (S >= R(0)) : (S <= R(0));
     if (undisturbed) { W[0] = rK; W[1] = vK; W[4] = PK; }

@@ -81,6 +81,7 @@ template <> struct Bits<double> {
 template <class R> struct Par {
   R gamma, gm1;   // gamma, gamma-1
   R igm1;         // 1/(gamma-1), formed once on the host
+  R ig1, ig2, sA0;  // 1/(gamma+1), 1/(2 gamma), sqrt(2/(gamma+1)): the exact solver's constants, formed once on the host
   R nu, hnu;      // dt/dh and half of it
   R theta;        // generalized-minmod coefficient (S7)
   R min_dens, min_pres;
