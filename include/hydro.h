@@ -215,8 +215,9 @@ HYDRO_API int hydro_flux_accum_f64(double* acc, const double* face_flux, long lo
  * state; one call = three sweeps with the same dt in the order x, y, z (order 0) or z, y, x (order 1; alternate them from step
  * to step).  face_flux receives the corrector flux of each direction's sweep at the faces f = 0, 8, 16 (the flux that sweep
  * used, so that the flux balance of hydro_solve_* holds).  opts: nghost (0 => 3), status ([1] counts non-positive rho / P),
- * max_speed + cfl (dt formed on the device), workspace + workspace_bytes REQUIRED: hydro_rtvd_workspace_bytes(Ng, precision)
- * (at least one slot of 5 x (22 x 22 x 16 + 22 x 16 x 16) elements; the kernel runs one CTA per slot).  No Riemann solver, no
+ * max_speed + cfl (dt formed on the device), workspace + workspace_bytes: hydro_rtvd_workspace_bytes(Ng, precision)
+ * (at least one slot of 5 x (22 x 22 x 16 + 22 x 16 x 16) elements; the kernel runs one CTA per slot) -- REQUIRED in fp64 and
+ * for nghost > 3; fp32 with nghost == 3 keeps the whole padded group in shared memory and ignores it.  No Riemann solver, no
  * limiter choice, no floors.  Errors as hydro_solve_* (HYDRO_E_GHOST: nghost < 3; HYDRO_E_WORKSPACE; HYDRO_E_ENUM: order). */
 HYDRO_API size_t hydro_rtvd_workspace_bytes(int Ng, int precision_bytes);
 HYDRO_API int hydro_rtvd_solve_f32(const float* in, float* out, float* face_flux, int Ng, float dt, float dh, float gamma, int order,
