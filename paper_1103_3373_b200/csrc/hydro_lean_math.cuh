@@ -30,7 +30,7 @@ __device__ __forceinline__ double m_fma(double a, double b, double c) { return f
 
 // Division-like operations of the lean path.  fp32: the SFU approximations of hydro_math.cuh.  fp64: an IEEE division
 // or square root is ~20 instructions with a branch to a slow path; the lean path instead refines the SFU's
-// 2^-23 seed (rcp.approx.ftz.f64 / rsqrt.approx.ftz.f64) with two Newton steps in FMAs: branch-free, <= 2 ulp,
+// 2^-23 seed (rcp.approx.ftz.f64 / rsqrt.approx.ftz.f64) with one third-order step in FMAs: branch-free, <= 2 ulp,
 // far inside the fp64 parity budget.  Zero / denormal arguments give inf / NaN, which every
 // caller either discards by a select (limiter) or routes to the Roe failure test; -DHYDRO_F64_IEEE=1 restores
 // IEEE operations for A/B measurements.
@@ -47,11 +47,14 @@ __device__ __forceinline__ double l_div(double a, double b) { return a / b; }
 __device__ __forceinline__ double l_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ double l_rsqrt(double x) { return rsqrt(x); }
 #else
+// one THIRD-order step from the 2^-23 seed (error e^3 ~ 2^-69, then the rounding of the last two operations): three / five
+// FP64-pipe instructions instead of the four / eight of two Newton steps -- the FP64 pipe (two issue cycles per warp
+// instruction) is what bounds the fp64 kernels
 __device__ __forceinline__ double l_rcp(double x) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  r = fma(r, fma(-x, r, 1.0), r);
-  return fma(r, fma(-x, r, 1.0), r);
+  const double e = fma(-x, r, 1.0);          // 1 - x r
+  return fma(r, fma(e, e, e), r);            // r (1 + e + e^2)
 }
 __device__ __forceinline__ double l_div(double a, double b) {
   const double r = l_rcp(b), q = a * r;
@@ -60,8 +63,8 @@ __device__ __forceinline__ double l_div(double a, double b) {
 __device__ __forceinline__ double l_rsqrt(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  y = fma(0.5 * y, fma(-x * y, y, 1.0), y);
-  return fma(0.5 * y, fma(-x * y, y, 1.0), y);
+  const double e = fma(-x * y, y, 1.0);      // 1 - x y^2
+  return fma(y, fma(0.375, e, 0.5) * e, y);  // y (1 + e/2 + 3 e^2 / 8)
 }
 __device__ __forceinline__ double l_sqrt(double x) {
   const double y = l_rsqrt(x), s = x * y;
