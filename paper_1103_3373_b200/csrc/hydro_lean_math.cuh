@@ -37,6 +37,9 @@ __device__ __forceinline__ double m_fma(double a, double b, double c) { return f
 #ifndef HYDRO_F64_IEEE
 #define HYDRO_F64_IEEE 0
 #endif
+#ifndef LEAN_DIV_REFINE
+#define LEAN_DIV_REFINE 0
+#endif
 __device__ __forceinline__ float l_rcp(float x) { return m_rcp(x); }
 __device__ __forceinline__ float l_div(float a, float b) { return m_div(a, b); }
 __device__ __forceinline__ float l_sqrt(float x) { return m_sqrt(x); }
@@ -56,10 +59,14 @@ __device__ __forceinline__ double l_rcp(double x) {
   const double e = fma(-x, r, 1.0);          // 1 - x r
   return fma(r, fma(e, e, e), r);            // r (1 + e + e^2)
 }
+#if LEAN_DIV_REFINE
 __device__ __forceinline__ double l_div(double a, double b) {
   const double r = l_rcp(b), q = a * r;
   return fma(fma(-b, q, a), r, q);
 }
+#else
+__device__ __forceinline__ double l_div(double a, double b) { return a * l_rcp(b); }  // <= 1.5 ulp; the residual step cost two more FP64-pipe instructions
+#endif
 __device__ __forceinline__ double l_rsqrt(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
