@@ -63,6 +63,15 @@ constexpr int VL_NT(int recon) { return 320 + 64 * (recon + 1) + 32; }
 // merged schedule (two CTA barriers per plane instead of four; its first-pass fluxes need two fields of their own): fp32 only.
 // Measured per 4096 groups: fp32 VL+PLM+Roe 1.87 -> 1.81 ms; fp64 5.08 -> 5.21 ms (and fp64 + PPM has no room for the fields)
 constexpr bool vl_merged(size_t elem, int recon) { return (void)recon, elem == 4; }
+// stages on warps of their own (hydro_lean_vl.cuh SPLIT): 23 warps leave 80 registers per thread, which the HLLE / HLLC solvers
+// fit in and Roe / exact do not.  Measured per 4096 groups, fp32 PLM: HLLC 1.67 -> 1.53 ms; Roe 1.79 -> 2.01 ms (100 bytes of
+// spills); PPM (25 warps, 72 registers) is slower with every solver.
+#ifndef VL_SPLIT
+#define VL_SPLIT 1
+#endif
+constexpr bool vl_split(size_t elem, int recon, int rs) {
+  return VL_SPLIT && elem == 4 && recon == RECON_PLM && (rs == RS_HLLC || rs == RS_HLLE);
+}
 // mbarriers | one primitive plane | W-half ring | LOX UPX LOY UPY FX FY | (merged: F1_x F1_y) | one raw plane
 constexpr size_t vl_smem_bytes(size_t elem, int recon, int g) {
   const size_t S = PS + 2 * g, SW = PS + 2 * (recon + 3), SH = PS + 2 * (recon + 2), NW = 2 * (1 + recon) + 1;

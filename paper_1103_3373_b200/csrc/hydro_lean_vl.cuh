@@ -21,8 +21,8 @@
 
 namespace hydro {
 
-template <class R, int RECON, int RS, int FAST, int GRID, int MERGE>
-__global__ void __launch_bounds__(VL_NT(RECON), 1)
+template <class R, int RECON, int RS, int FAST, int GRID, int MERGE, int SPLIT>
+__global__ void __launch_bounds__(VL_NT(RECON) + 320 * SPLIT, 1)
 vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g_arg, Par<R> p,
                const R* __restrict__ max_speed, R cfl, long long* status, GridIO<R> gio) {
   using Op = LeanOps<R, RECON, RS, FAST>;
@@ -33,7 +33,11 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
   constexpr int SF = PS + 2 * E + 1, FPL = (SF * SF + 3) / 4 * 4;  // first-pass flux grid (one more face than cells per row)
   constexpr int NC = LEAN_COLS, FT = PS + 2;
   constexpr int NP = 320 + 64 * (E - 1);                // plus cells; then one warp of boundary-face jobs
-  constexpr int NT = 320 + 64 * (RECON + 1) + 32;  // == VL_NT(RECON)
+  // SPLIT: the two stages run on warps of their own -- threads 0..319 the stage-2 columns, the next NP threads the stage-1 plus
+  // cells, then the boundary warp: 23 (25) warps instead of 13 (15) hide each other's latencies (a thread has ONE role, so its
+  // carried values share registers)
+  constexpr int S1 = SPLIT ? 320 : 0;              // first stage-1 thread
+  constexpr int NT = 320 + 64 * (RECON + 1) + 32 + S1;  // == VL_NT(RECON) + 320 SPLIT
   static_assert(2 * FPL <= 4 * NC, "first-pass flux fields must fit in LOX..UPY");
   // MERGE: the two stages share their barrier intervals (two CTA barriers per plane instead of four): stage 2 then runs one more
   // plane behind (b = a - 2 - RW) and the first-pass fluxes get their own fields.  The W-half ring needs no extra plane: S2
@@ -62,17 +66,19 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
   const int tid = threadIdx.x;
   // ---- stage-1 role: plus cell (ci, cj) in interior coordinates, or a boundary-face job of the extra warp
   int ci = 0, cj = 0;
-  const bool cell = tid < NP;
-  if (tid < PS * PS) { cj = tid >> 4; ci = tid & 15; }                                           // warps 0-7: interior columns
-  else if (tid < PS * PS + 32) { const int l = tid - PS * PS; cj = l >> 1; ci = (l & 1) ? PS : -1; }  // warp 8: x ring
-  else if (tid < 320) { const int l = tid - PS * FT; cj = (l < PS) ? -1 : PS; ci = l & (PS - 1); }    // warp 9: y ring
+  const int k1 = (SPLIT && tid >= S1) ? tid - S1 : tid;  // index within the stage's own numbering (the two coincide unless SPLIT)
+  const bool cell = tid >= S1 && k1 < NP;
+  if (k1 < PS * PS) { cj = k1 >> 4; ci = k1 & 15; }                                            // interior columns
+  else if (k1 < PS * PS + 32) { const int l = k1 - PS * PS; cj = l >> 1; ci = (l & 1) ? PS : -1; }  // x ring
+  else if (k1 < 320) { const int l = k1 - PS * FT; cj = (l < PS) ? -1 : PS; ci = l & (PS - 1); }    // y ring
   else if (cell) {
-    const int k = tid - 320, r = 2 + k / 64, arm = (k & 63) >> 4, pos = k & 15;
+    const int k = k1 - 320, r = 2 + k / 64, arm = (k & 63) >> 4, pos = k & 15;
     ci = arm == 0 ? -r : (arm == 1 ? PS - 1 + r : pos);
     cj = arm == 2 ? -r : (arm == 3 ? PS - 1 + r : pos);
   }
   const bool c_int = cell && ci >= 0 && ci < PS && cj >= 0 && cj < PS;
-  const int bl = tid - NP;  // lane of the boundary warp
+  const bool bndw = tid >= S1 + NP;  // the boundary warp
+  const int bl = tid - (S1 + NP);    // its lane
   // ---- stage-2 role (tid < 320): column of the 18 x 18 tile, as in the CTU / MHM kernels
   const int ii = ci + 1, jj = cj + 1;
   const bool s2 = tid < 320;
@@ -125,16 +131,19 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
     ++nseq;
   };
 
-  V5<R> Wprev, s1prev, f1zprev, uzc, Dz;  // W(a-1); (dF1_x + dF1_y)(a-1); F1_z(a-1); up_z(b-1); (dF_x + dF_y - F_z)(b-1)
+  V5<R> Wprev, s1prev, f1zprev, uzc_own, Dz_own;  // W(a-1); (dF1_x + dF1_y)(a-1); F1_z(a-1); up_z(b-1); (dF_x + dF_y - F_z)(b-1)
 #pragma unroll
-  for (int q = 0; q < 5; ++q) { Wprev[q] = R(1); s1prev[q] = R(0); f1zprev[q] = R(0); uzc[q] = R(0); Dz[q] = R(0); }
+  for (int q = 0; q < 5; ++q) { Wprev[q] = R(1); s1prev[q] = R(0); f1zprev[q] = R(0); uzc_own[q] = R(0); Dz_own[q] = R(0); }
+  // SPLIT: a thread carries either the stage-1 or the stage-2 values: the latter live in the former's registers
+  V5<R>& uzc = SPLIT ? Wprev : uzc_own;
+  V5<R>& Dz = SPLIT ? s1prev : Dz_own;
 
   for (int m = 0; m < my_groups; ++m) {
     const size_t grp = (size_t)blockIdx.x + (size_t)m * gridDim.x;
     const R* gin0 = in + grp * 5 * nS + ((size_t)g * S + (cj + g)) * S + (ci + g);
     R* gout0 = out + grp * 5 * PS * PS * PS + cj * PS + ci;
     if (GRID) {  // U^n and the result live in the grids (interior columns only)
-      const size_t cell0 = c_int ? grid_cell0(gio, grp, ci, cj) : 0;
+      const size_t cell0 = (c_int || interior) ? grid_cell0(gio, grp, ci, cj) : 0;
       gin0 = gio.gin + cell0;
       gout0 = gio.gout + cell0;
     }
@@ -175,7 +184,7 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
           stv(f1y, FPL, fb, Op::template riemann<1>(ldv(wa, WPL, wb - SW), W0, p, c));
         }
         if (zf) f1z = Op::template riemann<2>(Wprev, W0, p, c);
-      } else if (!cell && a_xy) {
+      } else if (bndw && a_xy) {
         // boundary warp: the upper faces that no plus cell owns.  Inner plane: x (16+E, l) / y (l, 16+E) for l < 16 and the
         // 2E arm-only rows / columns r: x (16, r) / y (r, 16).  Outer plane (interior columns only): x (16, l) / y (l, 16).
         int r = -100, edge = PS;
@@ -339,7 +348,8 @@ vl_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ fa
 }
 
 template <class R, int RECON, int RS, int FAST, int GRID = 0> cudaError_t launch_vl_lean(const SolveArgs<R>& a) {
-  auto kern = vl_lean_kernel<R, RECON, RS, FAST, GRID, vl_merged(sizeof(R), RECON) ? 1 : 0>;
+  constexpr int SPLIT = vl_split(sizeof(R), RECON, RS) ? 1 : 0;
+  auto kern = vl_lean_kernel<R, RECON, RS, FAST, GRID, vl_merged(sizeof(R), RECON) ? 1 : 0, SPLIT>;
   const size_t smem = vl_smem_bytes(sizeof(R), RECON, a.g);
   if (smem > SMEM_MAX_OPTIN) return cudaErrorInvalidConfiguration;
   static int sms = 0;
@@ -352,7 +362,7 @@ template <class R, int RECON, int RS, int FAST, int GRID = 0> cudaError_t launch
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   const int grid = a.Ng < sms ? a.Ng : sms;
-  kern<<<(unsigned)grid, VL_NT(RECON), smem, a.stream>>>(a.in, a.out, a.face_flux, a.Ng, a.g, a.par, a.max_speed, a.cfl, a.status, a.grid);
+  kern<<<(unsigned)grid, VL_NT(RECON) + 320 * SPLIT, smem, a.stream>>>(a.in, a.out, a.face_flux, a.Ng, a.g, a.par, a.max_speed, a.cfl, a.status, a.grid);
   return cudaGetLastError();
 }
 
