@@ -45,6 +45,12 @@ template <class R> __device__ __forceinline__ R rt_phi(R a, R b) {
   const R p = a * b;
   return p > R(0) ? m_div(p + p, a + b) : R(0);
 }
+// phi(a/2, b/2) = a b / (a + b): the halves of the limiter's arguments and the factor two cancel exactly in binary arithmetic,
+// three instructions fewer per limiter evaluation (ten evaluations per cell and sweep)
+template <class R> __device__ __forceinline__ R rt_phi_half(R a, R b) {
+  const R p = a * b;
+  return p > R(0) ? m_div(p, a + b) : R(0);
+}
 
 // One sweep along D of the pencils (a, b), a in [0, na), b in [0, nb).  src cell (q, a, b, x) at src[q sq + a sa + b sb + x sx],
 // x = 0 .. 21; dst likewise for the 16 updated cells x - 3.  ff: plane base of direction D (3 planes x 5 x 256) or nullptr;
@@ -105,8 +111,8 @@ __device__ __forceinline__ void rt_sweep(const R* __restrict__ src, size_t sq, i
                 const V5<R>& Hlo = Hw[(u + 1) & 1];
 #pragma unroll
                 for (int q = 0; q < 5; ++q) {
-                  const R frh = r1[c3][q] + rt_phi(R(0.5) * (r1[c3][q] - fr4[q]), R(0.5) * (r1[c2][q] - r1[c3][q]));
-                  const R flh = l1[c2][q] - rt_phi(R(0.5) * (l1[c2][q] - l1[c3][q]), R(0.5) * (l1[c1][q] - l1[c2][q]));
+                  const R frh = r1[c3][q] + rt_phi_half(r1[c3][q] - fr4[q], r1[c2][q] - r1[c3][q]);
+                  const R flh = l1[c2][q] - rt_phi_half(l1[c2][q] - l1[c3][q], l1[c1][q] - l1[c2][q]);
                   H[q] = frh - flh;
                 }
                 const int f = x - 2 - RT_G;  // face index of the group: 0 .. 16
@@ -221,7 +227,14 @@ rtvd_smem_kernel(const float* __restrict__ in, float* __restrict__ out, float* _
       __syncthreads();
       rt_sweep<1, R, RT_SNT>(box + RT_G * W2, W3, 1, W2, W, box + RT_G * W2 + RT_G * W, W3, 1, W2, W, W, PS, RT_G, 0, fy, nu, gamma, bad);
       __syncthreads();
-      rt_sweep<0, R, RT_SNT>(box + RT_G * W2 + RT_G * W, W3, W, W2, 1, gout, NI, PS, PS * PS, 1, PS, PS, 0, 0, fx, nu, gamma, bad);
+      // the x sweep comes last here: written straight to `out` its lanes (pencils j) would store 64 bytes apart, so it also runs
+      // in place and the interior leaves the box in a coalesced copy
+      rt_sweep<0, R, RT_SNT>(box + RT_G * W2 + RT_G * W, W3, W, W2, 1, box + RT_G * W2 + RT_G * W + RT_G, W3, W, W2, 1, PS, PS, 0, 0, fx, nu, gamma, bad);
+      __syncthreads();
+      for (int idx = threadIdx.x; idx < 5 * (int)NI; idx += RT_SNT) {
+        const int q = idx >> 12, c = idx & 4095, k = c >> 8, j = (c >> 4) & 15, i = c & 15;
+        gout[idx] = box[q * W3 + (k + RT_G) * W2 + (j + RT_G) * W + (i + RT_G)];
+      }
     }
     __syncthreads();  // the next group's copies overwrite the box
   }
