@@ -37,6 +37,20 @@ def test_gather_scatter_bit_exact(B, dtype, bc, g):
     assert np.array_equal(back.cpu().numpy(), wl.groups_to_grid(out.cpu().numpy(), U.shape[1:]))
 
 
+# the gather kernel walks the groups in 4 x 4 x 4 bricks and the rest in plain order: a grid with full bricks AND a ragged
+# remainder along every axis (6 x 9 x 5 groups), against the numpy definition
+@pytest.mark.parametrize("dtype", (np.float32, np.float64))
+@pytest.mark.parametrize("bc", ("periodic", "outflow"))
+def test_gather_bricks_and_remainder_bit_exact(B, dtype, bc):
+    import torch
+    rng = np.random.default_rng(7)
+    U = rng.standard_normal((5, 80, 144, 96)).astype(dtype)
+    for g in (2, 3):
+        ref = wl.grid_to_groups(U, g, bc)
+        G = B.hydro_gather(torch.from_numpy(U).cuda(), g, B.BC_PERIODIC if bc == "periodic" else B.BC_OUTFLOW)
+        assert np.array_equal(G.cpu().numpy(), ref)
+
+
 def test_gather_argument_errors(B):
     import torch
     bad = torch.zeros((5, 16, 16, 24), device="cuda")
