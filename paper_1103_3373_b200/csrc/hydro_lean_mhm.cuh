@@ -87,9 +87,9 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
 
   extern __shared__ __align__(16) unsigned char smem[];
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem);   // [2]
-  R* ring = reinterpret_cast<R*>(smem + 64);           // [NW] fields of WPL cells: primitive planes t-RW .. t+RW
-  R* xy = ring + NW * 5 * WPL;                         // [6] fields of NC cells: LOX UPX LOY UPY FX FY
-  R* raw = xy + 6 * 5 * NC;                            // [2][5][SS] landing zone of the bulk copies
+  // mbarriers [2] | ring: [NW] fields of WPL cells, the primitive planes t-RW .. t+RW | xy: [6] fields of NC cells, LOX UPX LOY
+  // UPY FX FY | raw: [2][5][SS], the landing zone of the bulk copies (last: only its size depends on g)
+  R* raw = reinterpret_cast<R*>(smem + 64) + NW * 5 * WPL + 6 * 5 * NC;
   // every shared-memory access below is LDS / STS [R + immediate] off 32-bit shared addresses formed once (hydro_ptx.cuh Fld<>);
   // the window base and tid are opaque so that ptxas holds them instead of re-deriving them (S2UR / S2R) at every use
   using FW = Fld<R, WPL>;  // a primitive plane of the ring
@@ -98,7 +98,6 @@ mhm_lean_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ f
   uint32_t sb = smem_u32(smem);
   asm volatile("" : "+r"(sb));
   const uint32_t sm_ring = sb + 64u, sm_xy = sm_ring + (uint32_t)(NW * 5 * WPL) * ES, sm_raw = sm_xy + (uint32_t)(6 * 5 * NC) * ES;
-  (void)ring; (void)xy;
 
   int tid = threadIdx.x;
   asm volatile("" : "+r"(tid));
