@@ -71,7 +71,8 @@ enum {
   HYDRO_E_GHOST = -5,     /* nghost < hydro_min_ghost(scheme, recon), or > 8 */
   HYDRO_E_WORKSPACE = -6, /* staged path selected and workspace missing / smaller than one slot */
   HYDRO_E_VALUE = -7,     /* gamma <= 1, dh <= 0, dt < 0, minmod_coeff outside [1,2], negative floor, cfl <= 0 */
-  HYDRO_E_NOFUSED = -8    /* impl == HYDRO_IMPL_FUSED and no such kernel exists (or fits) for this variant */
+  HYDRO_E_NOFUSED = -8,   /* impl == HYDRO_IMPL_FUSED and no such kernel exists (or fits) for this variant */
+  HYDRO_E_TOOBIG = -9     /* a size beyond the fixed maximum of an entry point that allocates nothing (hydro_rtvd_solve_noalloc_f64) */
 };
 
 typedef struct hydro_opts {      /* NULL => all defaults */
@@ -224,6 +225,22 @@ HYDRO_API int hydro_rtvd_solve_f32(const float* in, float* out, float* face_flux
                                    const hydro_opts* opts, hydro_stream_t stream);
 HYDRO_API int hydro_rtvd_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int order,
                                    const hydro_opts* opts, hydro_stream_t stream);
+
+/* The same split relaxing-TVD update (reading S26) through an entry point that ALLOCATES NOTHING, for
+ * callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it): fp64, ghost
+ * width 3 (in [Ng][5][22^3]), the kernel of hydro_rtvd_solve_f64 with its scratch slots in a file-scope device array of the
+ * library instead of a caller workspace: 32 slots = 17 121 280 bytes (16.3 MiB), which every GPU that loads the library holds
+ * until exit.  The caller still passes in, out, face_flux (or NULL) and status (device long long[3] or NULL; [1] counts
+ * non-positive rho / P, accumulated).  dt is a host scalar here (no device-formed dt).  Limit: Ng <= HYDRO_RTVD_NOALLOC_MAX_GROUPS
+ * per call, else HYDRO_E_TOOBIG; other errors as hydro_rtvd_solve_f64 (HYDRO_E_COUNT, _ENUM, _VALUE, _NULL, _ALIGN), > 0 = cudaError_t.
+ * No cudaMalloc / cudaFree / allocating library routine is called; the array's device address is looked up once per device
+ * (cudaGetSymbolAddress, on the first call with that device current).  ALL calls share the one array, which keeps the last
+ * call's contents: nothing in it has to start at zero (every sweep writes what the next sweep reads), but two calls that
+ * OVERLAP on the GPU (different streams, or graph branches) RACE on it -- serialise them.  Results equal hydro_rtvd_solve_f64
+ * bit for bit (groups are independent; only the number of CTAs differs). */
+#define HYDRO_RTVD_NOALLOC_MAX_GROUPS 4096
+HYDRO_API int hydro_rtvd_solve_noalloc_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma,
+                                           int order, long long* status, hydro_stream_t stream);
 
 /* Sizes and capabilities. */
 HYDRO_API int hydro_min_ghost(int scheme, int recon);                 /* 2/3 (MHM, CTU with PLM/PPM), 3/4 (VL)   */

@@ -24,7 +24,8 @@ EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64",
            "hydro_solve_grid_f32", "hydro_solve_grid_f64", "hydro_gather_f32", "hydro_gather_f64", "hydro_scatter_f32", "hydro_scatter_f64",
            "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror",
            "hydro_alu_peak_launch", "hydro_advance_f32", "hydro_advance_f64", "hydro_advance_workspace_bytes", "hydro_fluxfix_f32", "hydro_fluxfix_f64", "hydro_restrict_f32", "hydro_restrict_f64",
-           "hydro_flux_accum_f32", "hydro_flux_accum_f64", "hydro_rtvd_solve_f32", "hydro_rtvd_solve_f64", "hydro_rtvd_workspace_bytes")
+           "hydro_flux_accum_f32", "hydro_flux_accum_f64", "hydro_rtvd_solve_f32", "hydro_rtvd_solve_f64", "hydro_rtvd_workspace_bytes",
+           "hydro_rtvd_solve_noalloc_f64")
 
 
 class HydroOpts(C.Structure):
@@ -64,6 +65,7 @@ def lib():
             getattr(L, "hydro_flux_accum_" + name).argtypes = [vp, vp, C.c_longlong, ft, vp]
             getattr(L, "hydro_pipeline_solve_" + name).argtypes = [vp, vp, vp, vp, i, ft, ft, ft, i, i, i,
                                                                    C.POINTER(HydroOpts), vp, vp]
+        L.hydro_rtvd_solve_noalloc_f64.argtypes = [vp, vp, vp, i, C.c_double, C.c_double, C.c_double, i, vp, vp]
         L.hydro_pipeline_create.argtypes = [C.POINTER(vp), i, i, i, i]
         L.hydro_pipeline_destroy.argtypes = [vp]
         L.hydro_pipeline_destroy.restype = None
@@ -218,6 +220,28 @@ def hydro_rtvd_solve(in_, dt, dh, gamma, order=0, *, out=None, face_flux=True, s
         raise HydroError(rc, "hydro_rtvd_solve_" + sfx)
     if stream is not None:
         workspace.record_stream(stream)
+    return out, face_flux
+
+
+RTVD_NOALLOC_MAX_GROUPS = 4096  # HYDRO_RTVD_NOALLOC_MAX_GROUPS of include/hydro.h
+
+
+def hydro_rtvd_solve_noalloc(in_, dt, dh, gamma, order=0, *, out, face_flux=None, status=None, stream=None):
+    """hydro_rtvd_solve_noalloc_f64: the split relaxing-TVD update of fp64 groups with ghost width 3 through the entry point that
+    allocates nothing (scratch in a static device array of the library; at most RTVD_NOALLOC_MAX_GROUPS groups per call; calls
+    that overlap on the GPU race).  `out` (and `face_flux`, `status`) are caller tensors: this wrapper allocates nothing either."""
+    if not in_.is_cuda or in_.dtype != torch.float64 or not in_.is_contiguous() or in_.dim() != 5 or tuple(in_.shape[1:]) != (5, 22, 22, 22):
+        raise ValueError("hydro_rtvd_solve_noalloc: in_ must be a contiguous CUDA float64 tensor [Ng,5,22,22,22]")
+    for t in (out, face_flux):
+        if t is not None and (t.dtype != in_.dtype or t.device != in_.device or not t.is_contiguous()):
+            raise ValueError("hydro_rtvd_solve_noalloc: out / face_flux must match in_ (dtype, device) and be contiguous")
+    st = (stream or torch.cuda.current_stream(in_.device)).cuda_stream
+    with torch.cuda.device(in_.device):
+        rc = lib().hydro_rtvd_solve_noalloc_f64(in_.data_ptr(), out.data_ptr(), face_flux.data_ptr() if face_flux is not None else None,
+                                                in_.shape[0], dt, dh, gamma, order,
+                                                status.data_ptr() if status is not None else None, st)
+    if rc != 0:
+        raise HydroError(rc, "hydro_rtvd_solve_noalloc_f64")
     return out, face_flux
 
 

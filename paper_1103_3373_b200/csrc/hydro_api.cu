@@ -541,6 +541,7 @@ const char* hydro_strerror(int code) {
     case HYDRO_E_WORKSPACE: return "staged path needs opts->workspace of hydro_workspace_bytes()";
     case HYDRO_E_VALUE: return "scalar argument out of range";
     case HYDRO_E_NOFUSED: return "no fused kernel for this variant";
+    case HYDRO_E_TOOBIG: return "size beyond the fixed maximum of this no-allocation entry point (HYDRO_RTVD_NOALLOC_MAX_GROUPS)";
     default: return code > 0 ? cudaGetErrorString((cudaError_t)code) : "unknown hydro error";
   }
 }

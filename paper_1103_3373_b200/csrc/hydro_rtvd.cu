@@ -286,9 +286,54 @@ static int rtvd_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, in
   return (int)cudaGetLastError();
 }
 
+// ---- hydro_rtvd_solve_noalloc_f64: the scratch-slot kernel above with its scratch in a file-scope device array, for callers
+// that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Every GPU that loads the
+// library holds the array (16.3 MiB) until exit.  The array's NAME is a host-side stand-in in host code, not a device address:
+// the address comes from cudaGetSymbolAddress, once per device, with that device current.
+constexpr int NOALLOC_SLOTS = 32;  // CTAs of the launch, one scratch slot each
+constexpr size_t NOALLOC_SLOT_BYTES = 5 * ((size_t)RT_W * RT_W * PS + (size_t)RT_W * PS * PS) * sizeof(double);  // 535 040
+static __device__ __align__(256) unsigned char g_rtvd_noalloc_scratch[NOALLOC_SLOTS * NOALLOC_SLOT_BYTES];
+constexpr int NOALLOC_MAX_DEVICES = 64;
+
+static int rtvd_noalloc_impl(const double* in, double* out, double* ff, int Ng, double dt, double dh, double gamma, int order,
+                             long long* status, cudaStream_t st) {
+  if (Ng < 0) return HYDRO_E_COUNT;
+  if (Ng > HYDRO_RTVD_NOALLOC_MAX_GROUPS) return HYDRO_E_TOOBIG;
+  if (order < 0 || order > 1) return HYDRO_E_ENUM;
+  if (!(gamma > 1.0) || !(dh > 0.0) || !(dt >= 0.0)) return HYDRO_E_VALUE;
+  if (Ng == 0) return HYDRO_OK;
+  if (!in || !out) return HYDRO_E_NULL;
+  if (((uintptr_t)in & 15) || ((uintptr_t)out & 15) || ((uintptr_t)ff & 15) || ((uintptr_t)status & 7)) return HYDRO_E_ALIGN;
+  // set-up, once per device: the device address of the array on the CURRENT device (no allocation: the array is part of the
+  // loaded module).  A benign race between two host threads writes the same value twice.
+  static double* addr[NOALLOC_MAX_DEVICES] = {nullptr};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return (int)e;
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return HYDRO_E_VALUE;
+  double* scratch = addr[dev];
+  if (!scratch) {
+    void* ptr = nullptr;
+    e = cudaGetSymbolAddress(&ptr, g_rtvd_noalloc_scratch);
+    if (e != cudaSuccess) return (int)e;
+    if (!ptr) return (int)cudaErrorInvalidSymbol;
+    scratch = static_cast<double*>(ptr);
+    addr[dev] = scratch;
+  }
+  // nothing in the scratch must start at zero: every sweep writes the whole range the next sweep reads, so the contents the
+  // previous call left are never read
+  const int slots = Ng < NOALLOC_SLOTS ? Ng : NOALLOC_SLOTS;
+  rtvd_kernel<double><<<(unsigned)slots, RT_NT, 0, st>>>(in, out, ff, Ng, RT_G, dt / dh, gamma, order, nullptr, 0.0, scratch, status);
+  return (int)cudaGetLastError();
+}
+
 }  // namespace hydro
 
 extern "C" {
+int hydro_rtvd_solve_noalloc_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int order,
+                                 long long* status, hydro_stream_t stream) {
+  return hydro::rtvd_noalloc_impl(in, out, face_flux, Ng, dt, dh, gamma, order, status, (cudaStream_t)stream);
+}
 size_t hydro_rtvd_workspace_bytes(int Ng, int precision_bytes) {
   if (Ng <= 0 || (precision_bytes != 4 && precision_bytes != 8)) return 0;
   const size_t slots = Ng < hydro::RT_MAX_SLOTS ? (size_t)Ng : (size_t)hydro::RT_MAX_SLOTS;
