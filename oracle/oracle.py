@@ -223,5 +223,27 @@ def rtvd_solve(in_, dt, dh, gamma, order=0, want_flux=True, nthreads=1):
     return out, ff, status
 
 
+# ---- directionally split weighted average flux (oracle/waf_oracle.cpp), SURVEY.md 8(f)-4 ----
+def waf_solve(in_, dt, dh, gamma, order=0, want_flux=True, nthreads=1):
+    """One split WAF step (sweeps x,y,z for order 0; z,y,x for order 1) of Ng padded groups (g >= 3).
+    Returns (out, face_flux or None, status[8])."""
+    in_ = np.ascontiguousarray(in_)
+    Ng, S = in_.shape[0], in_.shape[2]
+    g = (S - PS) // 2
+    out = np.empty((Ng, 5, PS, PS, PS), in_.dtype)
+    ff = np.empty((Ng, 9, 5, PS, PS), in_.dtype) if want_flux else None
+    status = np.zeros(8, np.int64)
+    if in_.dtype == np.float64:
+        ct, fn = C.c_double, lib().oracle_waf_solve_f64
+    else:
+        ct, fn = C.c_float, lib().oracle_waf_solve_f32
+    fn.argtypes = [C.POINTER(ct), C.POINTER(ct), C.POINTER(ct), C.c_int, C.c_int, ct, ct, ct, C.c_int, C.POINTER(C.c_longlong), C.c_int]
+    rc = fn(_ptr(in_, ct), _ptr(out, ct), _ptr(ff, ct) if want_flux else None, Ng, g, dt, dh, gamma, order,
+            _ptr(status, C.c_longlong), nthreads)
+    if rc != 0:
+        raise ValueError(f"oracle_waf_solve rc={rc}")
+    return out, ff, status
+
+
 def max_threads():
     return int(lib().oracle_max_threads())
