@@ -226,6 +226,19 @@ HYDRO_API int hydro_rtvd_solve_f32(const float* in, float* out, float* face_flux
 HYDRO_API int hydro_rtvd_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int order,
                                    const hydro_opts* opts, hydro_stream_t stream);
 
+/* The directionally SPLIT weighted-average-flux update: the second split scheme the paper times next to the
+ * unsplit ones ("the weighted average flux scheme (WAF; see Toro 2009)").  Reading S29 of DESIGN.md: TVD WAF with the
+ * HLLC wave structure on piecewise-constant data -- at a face, F = (F_L + F_R)/2 - 1/2 sum_k sign(c_k) A_k (F(k+1) - F(k)) over the
+ * waves S_L, S*, S_R of the HLLC solution, c_k = dt S_k / dh, A_k = 1 - (1 - |c_k|) B(r_k) with the van Leer limiter B of the ratio
+ * of the upwind to the local jump across wave k (of the density; of the tangential momentum components themselves across the
+ * contact); one call = three sweeps x, y, z (order 0) or z, y, x (order 1).  Arguments, layouts, workspace
+ * (hydro_rtvd_workspace_bytes), face_flux planes, status and errors exactly as hydro_rtvd_solve_*; nghost >= 3 (the scheme
+ * itself uses two of the ghost layers).  Needs max_k |c_k| <= 1: dt <= dh / hydro_dt's maximum speed. */
+HYDRO_API int hydro_waf_solve_f32(const float* in, float* out, float* face_flux, int Ng, float dt, float dh, float gamma, int order,
+                                  const hydro_opts* opts, hydro_stream_t stream);
+HYDRO_API int hydro_waf_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int order,
+                                  const hydro_opts* opts, hydro_stream_t stream);
+
 /* The same split relaxing-TVD update (reading S26) through an entry point that ALLOCATES NOTHING, for
  * callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it): fp64, ghost
  * width 3 (in [Ng][5][22^3]), the kernel of hydro_rtvd_solve_f64 with its scratch slots in a file-scope device array of the

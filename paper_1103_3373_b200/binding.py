@@ -25,7 +25,7 @@ EXPORTS = ("hydro_solve_f32", "hydro_solve_f64", "hydro_dt_f32", "hydro_dt_f64",
            "hydro_has_fused", "hydro_fused_fits", "hydro_workspace_bytes", "hydro_staged_workspace_bytes", "hydro_strerror",
            "hydro_alu_peak_launch", "hydro_advance_f32", "hydro_advance_f64", "hydro_advance_workspace_bytes", "hydro_fluxfix_f32", "hydro_fluxfix_f64", "hydro_restrict_f32", "hydro_restrict_f64",
            "hydro_flux_accum_f32", "hydro_flux_accum_f64", "hydro_rtvd_solve_f32", "hydro_rtvd_solve_f64", "hydro_rtvd_workspace_bytes",
-           "hydro_rtvd_solve_noalloc_f64")
+           "hydro_rtvd_solve_noalloc_f64", "hydro_waf_solve_f32", "hydro_waf_solve_f64")
 
 
 class HydroOpts(C.Structure):
@@ -60,6 +60,7 @@ def lib():
             getattr(L, "hydro_solve_grid_" + name).argtypes = [vp, vp, i, i, i, i, ft, ft, ft, i, i, i, C.POINTER(HydroOpts), vp]
             getattr(L, "hydro_advance_" + name).argtypes = [vp, i, i, i, i, i, ft, ft, i, i, i, C.POINTER(HydroOpts), vp, sz, vp, vp]
             getattr(L, "hydro_rtvd_solve_" + name).argtypes = [vp, vp, vp, i, ft, ft, ft, i, C.POINTER(HydroOpts), vp]
+            getattr(L, "hydro_waf_solve_" + name).argtypes = [vp, vp, vp, i, ft, ft, ft, i, C.POINTER(HydroOpts), vp]
             getattr(L, "hydro_fluxfix_" + name).argtypes = [vp, vp, vp, vp, i, ft, ft, vp]
             getattr(L, "hydro_restrict_" + name).argtypes = [vp, vp, vp, i, vp]
             getattr(L, "hydro_flux_accum_" + name).argtypes = [vp, vp, C.c_longlong, ft, vp]
@@ -193,8 +194,13 @@ def _stream(t, stream):
     return (stream or torch.cuda.current_stream(t.device)).cuda_stream
 
 
+def hydro_waf_solve(in_, dt, dh, gamma, order=0, **kw):
+    """hydro_waf_solve_f32/f64: one directionally split weighted-average-flux step; arguments as hydro_rtvd_solve."""
+    return hydro_rtvd_solve(in_, dt, dh, gamma, order, _entry="hydro_waf_solve_", **kw)
+
+
 def hydro_rtvd_solve(in_, dt, dh, gamma, order=0, *, out=None, face_flux=True, status=None, workspace=None, stream=None,
-                     max_speed=None, cfl=0.0):
+                     max_speed=None, cfl=0.0, _entry="hydro_rtvd_solve_"):
     """hydro_rtvd_solve_f32/f64: one directionally split relaxing-TVD step (sweeps x,y,z for order 0; z,y,x for order 1) of
     in_[Ng,5,S,S,S] (ghost width >= 3).  Returns (out, face_flux or None).  workspace: uint8 CUDA tensor of
     hydro_rtvd_workspace_bytes(Ng, precision) (allocated if None)."""
@@ -213,11 +219,11 @@ def hydro_rtvd_solve(in_, dt, dh, gamma, order=0, *, out=None, face_flux=True, s
         workspace = torch.empty(max(16, lib().hydro_rtvd_workspace_bytes(Ng, in_.element_size())), dtype=torch.uint8, device=in_.device)
     o = make_opts(nghost=g, status=status, workspace=workspace, max_speed=max_speed, cfl=cfl)
     with torch.cuda.device(in_.device):
-        rc = getattr(lib(), "hydro_rtvd_solve_" + sfx)(in_.data_ptr(), out.data_ptr(),
+        rc = getattr(lib(), _entry + sfx)(in_.data_ptr(), out.data_ptr(),
                                                        face_flux.data_ptr() if face_flux is not None else None, Ng, ft(dt), ft(dh),
                                                        ft(gamma), order, C.byref(o), _stream(in_, stream))
     if rc != 0:
-        raise HydroError(rc, "hydro_rtvd_solve_" + sfx)
+        raise HydroError(rc, _entry + sfx)
     if stream is not None:
         workspace.record_stream(stream)
     return out, face_flux
@@ -241,7 +247,7 @@ def hydro_rtvd_solve_noalloc(in_, dt, dh, gamma, order=0, *, out, face_flux=None
                                                 in_.shape[0], dt, dh, gamma, order,
                                                 status.data_ptr() if status is not None else None, st)
     if rc != 0:
-        raise HydroError(rc, "hydro_rtvd_solve_noalloc_f64")
+        raise HydroError(rc, "hydro_rtvd_solve_noalloc_f64", "hydro_waf_solve_f32", "hydro_waf_solve_f64")
     return out, face_flux
 
 

@@ -135,7 +135,144 @@ __device__ __forceinline__ void rt_sweep(const R* __restrict__ src, size_t sq, i
   }
 }
 
-template <class R>
+// ---- the split WEIGHTED AVERAGE FLUX scheme ("WAF; see Toro 2009"): reading S29 of DESIGN.md, restated here
+// independently of oracle/waf_oracle.cpp.  TVD WAF with the HLLC wave structure on piecewise-constant data: at a face the
+// HLLC solution has regions F(1..4) = F_L, F*_L, F*_R, F_R separated by the waves S_L, S*, S_R (S9: Toro's pressure-based
+// speeds); F = (F(1) + F(4))/2 - 1/2 sum_k sign(c_k) A_k (F(k+1) - F(k)), c_k = nu S_k, A_k = 1 - (1 - |c_k|) B(a, b), B the
+// van Leer limiter 2a/(a+b) for ab > 0 (else 0) of the jump b of q across wave k at this face and the jump a at the upwind
+// face; q = rho, except that the tangential momentum components take their own jump across the contact for k = 2.
+// Everything below works in the NORMAL frame of the sweep: (rho, m_n, m_t1, m_t2, E).
+template <class R> struct WCell { R rho, u, v1, v2, P, c, E; };
+template <class R> struct WJump { R q[3], t1, t2; };                 // jumps across the three waves; tangential momenta across the contact
+template <class R> struct WFace { V5<R> hs, d1, d2, d3; R c[3]; };   // (F_L + F_R)/2, F(k+1) - F(k), Courant numbers
+template <class R> __device__ __forceinline__ WCell<R> waf_cell(const V5<R>& U, R gamma, int& bad) {
+  WCell<R> w;
+  const R ir = m_rcp(U[0]);
+  w.rho = U[0]; w.u = U[1] * ir; w.v1 = U[2] * ir; w.v2 = U[3] * ir; w.E = U[4];
+  w.P = (gamma - R(1)) * (U[4] - R(0.5) * U[0] * ((w.u * w.u + w.v1 * w.v1) + w.v2 * w.v2));
+  bad += (w.rho > R(0) && w.P > R(0)) ? 0 : 1;
+  w.c = m_sqrt(gamma * w.P * ir);
+  return w;
+}
+template <class R> __device__ __forceinline__ void waf_face(const WCell<R>& L, const WCell<R>& Rr, R nu, R gamma, WFace<R>& f, WJump<R>& j) {
+  const R ppv = R(0.5) * (L.P + Rr.P) - R(0.125) * (Rr.u - L.u) * (L.rho + Rr.rho) * (L.c + Rr.c);
+  const R ps = m_max(ppv, R(0));
+  const R gf = (gamma + R(1)) * m_rcp(gamma + gamma);
+  const R qL = ps <= L.P ? R(1) : m_sqrt(R(1) + gf * (m_div(ps, L.P) - R(1)));
+  const R qR = ps <= Rr.P ? R(1) : m_sqrt(R(1) + gf * (m_div(ps, Rr.P) - R(1)));
+  const R SL = L.u - L.c * qL, SR = Rr.u + Rr.c * qR;
+  const R mL = L.rho * (SL - L.u), mR = Rr.rho * (SR - Rr.u);
+  const R Ss = m_div((Rr.P - L.P) + L.u * mL - Rr.u * mR, mL - mR);
+  const R rsL = m_div(mL, SL - Ss), rsR = m_div(mR, SR - Ss);  // rho*_K
+  const R EsL = rsL * (m_div(L.E, L.rho) + (Ss - L.u) * (Ss + m_div(L.P, mL)));
+  const R EsR = rsR * (m_div(Rr.E, Rr.rho) + (Ss - Rr.u) * (Ss + m_div(Rr.P, mR)));
+  const R mnL = L.rho * L.u, mnR = Rr.rho * Rr.u;
+  // F*_L - F_L = S_L (U*_L - U_L);  F_R - F*_R = -S_R (U*_R - U_R);  the contact takes the rest of F_R - F_L
+  f.d1[0] = SL * (rsL - L.rho);              f.d3[0] = -SR * (rsR - Rr.rho);
+  f.d1[1] = SL * (rsL * Ss - mnL);           f.d3[1] = -SR * (rsR * Ss - mnR);
+  f.d1[2] = SL * (rsL * L.v1 - L.rho * L.v1); f.d3[2] = -SR * (rsR * Rr.v1 - Rr.rho * Rr.v1);
+  f.d1[3] = SL * (rsL * L.v2 - L.rho * L.v2); f.d3[3] = -SR * (rsR * Rr.v2 - Rr.rho * Rr.v2);
+  f.d1[4] = SL * (EsL - L.E);                f.d3[4] = -SR * (EsR - Rr.E);
+  V5<R> FL, FR;
+  FL[0] = mnL; FL[1] = mnL * L.u + L.P; FL[2] = mnL * L.v1; FL[3] = mnL * L.v2; FL[4] = (L.E + L.P) * L.u;
+  FR[0] = mnR; FR[1] = mnR * Rr.u + Rr.P; FR[2] = mnR * Rr.v1; FR[3] = mnR * Rr.v2; FR[4] = (Rr.E + Rr.P) * Rr.u;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    f.hs[q] = R(0.5) * (FL[q] + FR[q]);
+    f.d2[q] = ((FR[q] - FL[q]) - f.d1[q]) - f.d3[q];
+  }
+  f.c[0] = nu * SL; f.c[1] = nu * Ss; f.c[2] = nu * SR;
+  j.q[0] = rsL - L.rho; j.q[1] = rsR - rsL; j.q[2] = Rr.rho - rsR;
+  j.t1 = rsR * Rr.v1 - rsL * L.v1;
+  j.t2 = rsR * Rr.v2 - rsL * L.v2;
+}
+template <class R> __device__ __forceinline__ R waf_B(R a, R b) { return a * b > R(0) ? m_div(a + a, a + b) : R(0); }
+// half the signed weight sign(c) A / 2 of one wave for one limiter pair
+template <class R> __device__ __forceinline__ R waf_w(R c, R a, R b) {
+  const R sg = c > R(0) ? R(0.5) : (c < R(0) ? R(-0.5) : R(0));
+  return sg * (R(1) - (R(1) - m_abs(c)) * waf_B(a, b));
+}
+template <class R> __device__ __forceinline__ V5<R> waf_flux(const WFace<R>& f, const WJump<R>& jl, const WJump<R>& jc, const WJump<R>& ju) {
+  // upwind jumps of the three waves (selected by value: a run-time choice between two structs would put them in local memory)
+  const bool p0 = f.c[0] > R(0), p1 = f.c[1] > R(0), p2 = f.c[2] > R(0);
+  const R w0 = waf_w(f.c[0], p0 ? jl.q[0] : ju.q[0], jc.q[0]), w2 = waf_w(f.c[2], p2 ? jl.q[2] : ju.q[2], jc.q[2]);
+  const R w1 = waf_w(f.c[1], p1 ? jl.q[1] : ju.q[1], jc.q[1]);
+  const R w1a = waf_w(f.c[1], p1 ? jl.t1 : ju.t1, jc.t1), w1b = waf_w(f.c[1], p1 ? jl.t2 : ju.t2, jc.t2);
+  V5<R> H;
+  H[0] = ((f.hs[0] - w0 * f.d1[0]) - w1 * f.d2[0]) - w2 * f.d3[0];
+  H[1] = ((f.hs[1] - w0 * f.d1[1]) - w1 * f.d2[1]) - w2 * f.d3[1];
+  H[2] = ((f.hs[2] - w0 * f.d1[2]) - w1a * f.d2[2]) - w2 * f.d3[2];
+  H[3] = ((f.hs[3] - w0 * f.d1[3]) - w1b * f.d2[3]) - w2 * f.d3[3];
+  H[4] = ((f.hs[4] - w0 * f.d1[4]) - w1 * f.d2[4]) - w2 * f.d3[4];
+  return H;
+}
+
+// One WAF sweep along D: same pencil geometry and arguments as rt_sweep (cells 3 .. 18 of the 22-cell pencil are updated, the
+// scheme itself needs two of the three ghost cells).  Register windows: the cells x-1, x (primitives), the faces x-1, x
+// (flux data), the jumps of the faces x-2, x-1, x, the fluxes of the faces x-2, x-1; unrolled by their common period six.
+template <int D, class R, int NT = RT_NT>
+__device__ __forceinline__ void waf_sweep(const R* __restrict__ src, size_t sq, int sa, int sb, int sx, R* __restrict__ dst, size_t dq,
+                                          int da, int db, int dx, int na, int nb, int fa0, int fb0, R* __restrict__ ff, R nu, R gamma,
+                                          int& bad) {
+  constexpr int QN = 1 + D, QT1 = D == 0 ? 2 : 1, QT2 = D == 2 ? 2 : 3;  // global indices of m_n, m_t1, m_t2
+  for (int pidx = threadIdx.x; pidx < na * nb; pidx += NT) {
+    const int b = pidx / na, a = pidx - b * na;
+    const R* s = src + (size_t)a * sa + (size_t)b * sb;
+    R* d = dst + (size_t)a * da + (size_t)b * db;
+    const int ta = a - fa0, tb = b - fb0;
+    R* fp = (ff && ta >= 0 && ta < PS && tb >= 0 && tb < PS) ? ff + tb * PS + ta : nullptr;
+    WCell<R> cw[2];
+    WFace<R> fw[2];
+    WJump<R> jw[3];
+    V5<R> Hw[2], Unext;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { Hw[0][q] = Hw[1][q] = R(0); Unext[q] = s[q * sq]; }
+#pragma unroll 1
+    for (int x0 = 0; x0 < RT_W; x0 += 6) {
+#pragma unroll
+      for (int u = 0; u < 6; ++u) {
+        const int x = x0 + u;
+        if (x < RT_W) {
+          V5<R> Un;  // normal frame
+          Un[0] = Unext[0]; Un[1] = Unext[QN]; Un[2] = Unext[QT1]; Un[3] = Unext[QT2]; Un[4] = Unext[4];
+          if (x + 1 < RT_W) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) Unext[q] = s[q * sq + (size_t)(x + 1) * sx];
+          }
+          cw[u & 1] = waf_cell(Un, gamma, bad);
+          if (x >= 1) waf_face(cw[(u + 1) & 1], cw[u & 1], nu, gamma, fw[u & 1], jw[u % 3]);  // face x, between cells x-1 and x
+          if (x >= 4 && x <= RT_W - 2) {  // flux of face f = x-1 in 3 .. 19: jumps of the faces x-2, x-1, x
+            const V5<R> Hn = waf_flux(fw[(u + 1) & 1], jw[(u + 1) % 3], jw[(u + 2) % 3], jw[u % 3]);
+            V5<R>& H = Hw[u & 1];
+            H[0] = Hn[0]; H[QN] = Hn[1]; H[QT1] = Hn[2]; H[QT2] = Hn[3]; H[4] = Hn[4];
+            const int f = x - 1 - RT_G;  // face index of the group: 0 .. 16
+            if (fp && (f & 7) == 0) {
+#pragma unroll
+              for (int q = 0; q < 5; ++q) fp[((f >> 3) * 5 + q) * (PS * PS)] = H[q];
+            }
+            if (x >= 5) {  // cell x-2 = interior cell f-1
+              const V5<R>& Hlo = Hw[(u + 1) & 1];
+#pragma unroll
+              for (int q = 0; q < 5; ++q)
+                d[q * dq + (size_t)(x - 2 - RT_G) * dx] = s[q * sq + (size_t)(x - 2) * sx] - nu * (H[q] - Hlo[q]);
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
+constexpr int SPLIT_RTVD = 0, SPLIT_WAF = 1;
+template <int SCHEME, int D, class R, int NT = RT_NT>
+__device__ __forceinline__ void split_sweep(const R* __restrict__ src, size_t sq, int sa, int sb, int sx, R* __restrict__ dst, size_t dq,
+                                            int da, int db, int dx, int na, int nb, int fa0, int fb0, R* __restrict__ ff, R nu, R gamma,
+                                            int& bad) {
+  if (SCHEME == SPLIT_WAF) waf_sweep<D, R, NT>(src, sq, sa, sb, sx, dst, dq, da, db, dx, na, nb, fa0, fb0, ff, nu, gamma, bad);
+  else rt_sweep<D, R, NT>(src, sq, sa, sb, sx, dst, dq, da, db, dx, na, nb, fa0, fb0, ff, nu, gamma, bad);
+}
+
+template <class R, int SCHEME>
 __global__ void __launch_bounds__(RT_NT, sizeof(R) == 4 ? 2 : 1)
 rtvd_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_flux, int Ng, int g, R nu_arg, R gamma, int order,
             const R* __restrict__ max_speed, R cfl, R* __restrict__ scratch, long long* status) {
@@ -153,18 +290,18 @@ rtvd_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_
     R* gff = face_flux ? face_flux + (size_t)grp * 9 * 5 * PS * PS : nullptr;
     if (order == 0) {
       // x: pencils (j, k) of the padded box -> s1[q][k 22][j 22][i 16];  y: pencils (i, k) -> s2[q][k 22][j 16][i 16];  z: (i, j) -> out
-      rt_sweep<0, R>(gin, nS, S, S * S, 1, s1, N1, PS, RT_W * PS, 1, RT_W, RT_W, RT_G, RT_G, gff, nu, gamma, bad);
+      split_sweep<SCHEME, 0, R>(gin, nS, S, S * S, 1, s1, N1, PS, RT_W * PS, 1, RT_W, RT_W, RT_G, RT_G, gff, nu, gamma, bad);
       __syncthreads();
-      rt_sweep<1, R>(s1, N1, 1, RT_W * PS, PS, s2, N2, 1, PS * PS, PS, PS, RT_W, 0, RT_G, gff ? gff + 3 * 5 * PS * PS : nullptr, nu, gamma, bad);
+      split_sweep<SCHEME, 1, R>(s1, N1, 1, RT_W * PS, PS, s2, N2, 1, PS * PS, PS, PS, RT_W, 0, RT_G, gff ? gff + 3 * 5 * PS * PS : nullptr, nu, gamma, bad);
       __syncthreads();
-      rt_sweep<2, R>(s2, N2, 1, PS, PS * PS, gout, NI, 1, PS, PS * PS, PS, PS, 0, 0, gff ? gff + 6 * 5 * PS * PS : nullptr, nu, gamma, bad);
+      split_sweep<SCHEME, 2, R>(s2, N2, 1, PS, PS * PS, gout, NI, 1, PS, PS * PS, PS, PS, 0, 0, gff ? gff + 6 * 5 * PS * PS : nullptr, nu, gamma, bad);
     } else {
       // z: pencils (i, j) of the padded box -> s1[q][k 16][j 22][i 22];  y: pencils (i, k) -> s2[q][k 16][j 16][i 22];  x: (j, k) -> out
-      rt_sweep<2, R>(gin, nS, 1, S, S * S, s1, N1, 1, RT_W, RT_W * RT_W, RT_W, RT_W, RT_G, RT_G, gff ? gff + 6 * 5 * PS * PS : nullptr, nu, gamma, bad);
+      split_sweep<SCHEME, 2, R>(gin, nS, 1, S, S * S, s1, N1, 1, RT_W, RT_W * RT_W, RT_W, RT_W, RT_G, RT_G, gff ? gff + 6 * 5 * PS * PS : nullptr, nu, gamma, bad);
       __syncthreads();
-      rt_sweep<1, R>(s1, N1, 1, RT_W * RT_W, RT_W, s2, N2, 1, PS * RT_W, RT_W, RT_W, PS, RT_G, 0, gff ? gff + 3 * 5 * PS * PS : nullptr, nu, gamma, bad);
+      split_sweep<SCHEME, 1, R>(s1, N1, 1, RT_W * RT_W, RT_W, s2, N2, 1, PS * RT_W, RT_W, RT_W, PS, RT_G, 0, gff ? gff + 3 * 5 * PS * PS : nullptr, nu, gamma, bad);
       __syncthreads();
-      rt_sweep<0, R>(s2, N2, RT_W, PS * RT_W, 1, gout, NI, PS, PS * PS, 1, PS, PS, 0, 0, gff, nu, gamma, bad);
+      split_sweep<SCHEME, 0, R>(s2, N2, RT_W, PS * RT_W, 1, gout, NI, PS, PS * PS, 1, PS, PS, 0, 0, gff, nu, gamma, bad);
     }
     __syncthreads();  // the next group overwrites s1 / s2
   }
@@ -182,6 +319,7 @@ rtvd_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_
 // 6.9 stall cycles per instruction there).  The x sweep reads with a stride of 22 floats between lanes: two-way bank conflicts.
 constexpr int RT_SNT = 512;
 constexpr size_t RT_SMEM = 64 + 5 * (size_t)RT_W * RT_W * RT_W * sizeof(float);
+template <int SCHEME>
 __global__ void __launch_bounds__(RT_SNT, 1)
 rtvd_smem_kernel(const float* __restrict__ in, float* __restrict__ out, float* __restrict__ face_flux, int Ng, float nu_arg, float gamma,
                  int order, const float* __restrict__ max_speed, float cfl, long long* status) {
@@ -216,20 +354,20 @@ rtvd_smem_kernel(const float* __restrict__ in, float* __restrict__ out, float* _
     R* fx = gff, *fy = gff ? gff + 3 * 5 * PS * PS : nullptr, *fz = gff ? gff + 6 * 5 * PS * PS : nullptr;
     if (order == 0) {
       // x: pencils (j, k) of the box, in place;  y: pencils (i interior, k);  z: pencils (i, j) interior -> out
-      rt_sweep<0, R, RT_SNT>(box, W3, W, W2, 1, box + RT_G, W3, W, W2, 1, W, W, RT_G, RT_G, fx, nu, gamma, bad);
+      split_sweep<SCHEME, 0, R, RT_SNT>(box, W3, W, W2, 1, box + RT_G, W3, W, W2, 1, W, W, RT_G, RT_G, fx, nu, gamma, bad);
       __syncthreads();
-      rt_sweep<1, R, RT_SNT>(box + RT_G, W3, 1, W2, W, box + RT_G + RT_G * W, W3, 1, W2, W, PS, W, 0, RT_G, fy, nu, gamma, bad);
+      split_sweep<SCHEME, 1, R, RT_SNT>(box + RT_G, W3, 1, W2, W, box + RT_G + RT_G * W, W3, 1, W2, W, PS, W, 0, RT_G, fy, nu, gamma, bad);
       __syncthreads();
-      rt_sweep<2, R, RT_SNT>(box + RT_G + RT_G * W, W3, 1, W, W2, gout, NI, 1, PS, PS * PS, PS, PS, 0, 0, fz, nu, gamma, bad);
+      split_sweep<SCHEME, 2, R, RT_SNT>(box + RT_G + RT_G * W, W3, 1, W, W2, gout, NI, 1, PS, PS * PS, PS, PS, 0, 0, fz, nu, gamma, bad);
     } else {
       // z: pencils (i, j) of the box, in place;  y: pencils (i, k interior);  x: pencils (j, k) interior -> out
-      rt_sweep<2, R, RT_SNT>(box, W3, 1, W, W2, box + RT_G * W2, W3, 1, W, W2, W, W, RT_G, RT_G, fz, nu, gamma, bad);
+      split_sweep<SCHEME, 2, R, RT_SNT>(box, W3, 1, W, W2, box + RT_G * W2, W3, 1, W, W2, W, W, RT_G, RT_G, fz, nu, gamma, bad);
       __syncthreads();
-      rt_sweep<1, R, RT_SNT>(box + RT_G * W2, W3, 1, W2, W, box + RT_G * W2 + RT_G * W, W3, 1, W2, W, W, PS, RT_G, 0, fy, nu, gamma, bad);
+      split_sweep<SCHEME, 1, R, RT_SNT>(box + RT_G * W2, W3, 1, W2, W, box + RT_G * W2 + RT_G * W, W3, 1, W2, W, W, PS, RT_G, 0, fy, nu, gamma, bad);
       __syncthreads();
       // the x sweep comes last here: written straight to `out` its lanes (pencils j) would store 64 bytes apart, so it also runs
       // in place and the interior leaves the box in a coalesced copy
-      rt_sweep<0, R, RT_SNT>(box + RT_G * W2 + RT_G * W, W3, W, W2, 1, box + RT_G * W2 + RT_G * W + RT_G, W3, W, W2, 1, PS, PS, 0, 0, fx, nu, gamma, bad);
+      split_sweep<SCHEME, 0, R, RT_SNT>(box + RT_G * W2 + RT_G * W, W3, W, W2, 1, box + RT_G * W2 + RT_G * W + RT_G, W3, W, W2, 1, PS, PS, 0, 0, fx, nu, gamma, bad);
       __syncthreads();
       for (int idx = threadIdx.x; idx < 5 * (int)NI; idx += RT_SNT) {
         const int q = idx >> 12, c = idx & 4095, k = c >> 8, j = (c >> 4) & 15, i = c & 15;
@@ -249,7 +387,8 @@ constexpr int RT_MAX_SLOTS = 148 * 2;  // 296 slots x 267 KB (fp32) stay in the 
 inline size_t rtvd_slot_bytes(size_t elem) { return 5 * ((size_t)RT_W * RT_W * PS + (size_t)RT_W * PS * PS) * elem; }
 
 template <class R>
-static int rtvd_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, int order, const hydro_opts* o, cudaStream_t st) {
+static int rtvd_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, int order, const hydro_opts* o, cudaStream_t st,
+                     int scheme = SPLIT_RTVD) {
   if (Ng < 0) return HYDRO_E_COUNT;
   if (order < 0 || order > 1) return HYDRO_E_ENUM;
   const int g = (o && o->nghost) ? o->nghost : RT_G;
@@ -267,9 +406,10 @@ static int rtvd_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, in
         cudaGetDevice(&dev);
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
       }
-      cudaError_t e = cudaFuncSetAttribute(rtvd_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RT_SMEM);
+      auto kern = scheme == SPLIT_WAF ? rtvd_smem_kernel<SPLIT_WAF> : rtvd_smem_kernel<SPLIT_RTVD>;
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RT_SMEM);
       if (e != cudaSuccess) return (int)e;
-      rtvd_smem_kernel<<<(unsigned)(Ng < sms ? Ng : sms), RT_SNT, RT_SMEM, st>>>(in, out, ff, Ng, device_dt ? 0.f : dt / dh, gamma, order,
+      kern<<<(unsigned)(Ng < sms ? Ng : sms), RT_SNT, RT_SMEM, st>>>(in, out, ff, Ng, device_dt ? 0.f : dt / dh, gamma, order,
                                                                               device_dt ? static_cast<const float*>(o->max_speed) : nullptr,
                                                                               device_dt ? (float)o->cfl : 0.f, o ? o->status : nullptr);
       return (int)cudaGetLastError();
@@ -280,7 +420,8 @@ static int rtvd_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, in
   long long slots = (long long)(o->workspace_bytes / slot);
   if (slots > RT_MAX_SLOTS) slots = RT_MAX_SLOTS;
   if (slots > Ng) slots = Ng;
-  rtvd_kernel<R><<<(unsigned)slots, RT_NT, 0, st>>>(in, out, ff, Ng, g, device_dt ? R(0) : dt / dh, gamma, order,
+  auto kern = scheme == SPLIT_WAF ? rtvd_kernel<R, SPLIT_WAF> : rtvd_kernel<R, SPLIT_RTVD>;
+  kern<<<(unsigned)slots, RT_NT, 0, st>>>(in, out, ff, Ng, g, device_dt ? R(0) : dt / dh, gamma, order,
                                                    device_dt ? static_cast<const R*>(o->max_speed) : nullptr, device_dt ? (R)o->cfl : R(0),
                                                    static_cast<R*>(o->workspace), o->status);
   return (int)cudaGetLastError();
@@ -323,7 +464,7 @@ static int rtvd_noalloc_impl(const double* in, double* out, double* ff, int Ng, 
   // nothing in the scratch must start at zero: every sweep writes the whole range the next sweep reads, so the contents the
   // previous call left are never read
   const int slots = Ng < NOALLOC_SLOTS ? Ng : NOALLOC_SLOTS;
-  rtvd_kernel<double><<<(unsigned)slots, RT_NT, 0, st>>>(in, out, ff, Ng, RT_G, dt / dh, gamma, order, nullptr, 0.0, scratch, status);
+  rtvd_kernel<double, SPLIT_RTVD><<<(unsigned)slots, RT_NT, 0, st>>>(in, out, ff, Ng, RT_G, dt / dh, gamma, order, nullptr, 0.0, scratch, status);
   return (int)cudaGetLastError();
 }
 
@@ -346,5 +487,13 @@ int hydro_rtvd_solve_f32(const float* in, float* out, float* face_flux, int Ng, 
 int hydro_rtvd_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int order,
                          const hydro_opts* opts, hydro_stream_t stream) {
   return hydro::rtvd_impl<double>(in, out, face_flux, Ng, dt, dh, gamma, order, opts, (cudaStream_t)stream);
+}
+int hydro_waf_solve_f32(const float* in, float* out, float* face_flux, int Ng, float dt, float dh, float gamma, int order,
+                        const hydro_opts* opts, hydro_stream_t stream) {
+  return hydro::rtvd_impl<float>(in, out, face_flux, Ng, dt, dh, gamma, order, opts, (cudaStream_t)stream, hydro::SPLIT_WAF);
+}
+int hydro_waf_solve_f64(const double* in, double* out, double* face_flux, int Ng, double dt, double dh, double gamma, int order,
+                        const hydro_opts* opts, hydro_stream_t stream) {
+  return hydro::rtvd_impl<double>(in, out, face_flux, Ng, dt, dh, gamma, order, opts, (cudaStream_t)stream, hydro::SPLIT_WAF);
 }
 }
