@@ -265,20 +265,21 @@ def run_table(args):
         # machine balance of ~11 flop/B, so both fractions are reported: of the FMA roof (the binding one) and of the copy peak
         peaks = load_json(os.path.join(ROOT, "MEASURED_PEAKS.json"), {}) or {}
         hbm = float(peaks.get("hbm_gbs") or 6650.0)
-        for tdt in (torch.float32, torch.float64):
+        for split, tdt in ((sp, t) for sp in ("RTVD", "WAF") for t in (torch.float32, torch.float64)):
             es = 4 if tdt == torch.float32 else 8
-            if args.only and args.only.lower() != "rtvd,-,-," + ("fp32" if es == 4 else "fp64"):
+            if args.only and args.only.lower() != split.lower() + ",-,-," + ("fp32" if es == 4 else "fp64"):
                 continue
             u = wl.amr_batch(Ng, g=3, gamma=GAMMA, seed=0, dtype=str(tdt).replace("torch.", ""), device=dev)
             out = torch.empty((Ng, 5, 16, 16, 16), dtype=tdt, device=dev)
             ff = torch.empty((Ng, 9, 5, 16, 16), dtype=tdt, device=dev)
             ws = torch.empty(B.lib().hydro_rtvd_workspace_bytes(Ng, es), dtype=torch.uint8, device=dev)
-            ms = ev(lambda: B.hydro_rtvd_solve(u, 0.05, DH, GAMMA, 0, out=out, face_flux=ff, workspace=ws))
+            fn = B.hydro_rtvd_solve if split == "RTVD" else B.hydro_waf_solve
+            ms = ev(lambda: fn(u, 0.05, DH, GAMMA, 0, out=out, face_flux=ff, workspace=ws))
             byt = es * Ng * (5 * 22 ** 3 + 5 * CELLS + 45 * 256)
-            rows.append({"precision": "fp32" if es == 4 else "fp64", "scheme": "RTVD (split)", "recon": "-", "riemann": "-", "ms": ms,
+            rows.append({"precision": "fp32" if es == 4 else "fp64", "scheme": split + " (split)", "recon": "-", "riemann": "-", "ms": ms,
                          "cell_updates_per_s": Ng * CELLS / (ms * 1e-3), "fused": True,
                          "hbm_gbs": byt / ms / 1e6, "hbm_frac": byt / ms / 1e6 / hbm})
-            fl = (fpc.get("rtvd_g3") or {}).get("flops_per_cell")
+            fl = (fpc.get("rtvd_g3" if split == "RTVD" else "waf_g3") or {}).get("flops_per_cell")
             peak = mp.get("fp32_tflops_ffma" if es == 4 else "fp64_tflops")
             if fl and peak:
                 rows[-1].update({"flops_per_cell": fl, "frac": fl * Ng * CELLS / (ms * 1e-3) / 1e12 / peak, "bound": "alu"})

@@ -31,6 +31,29 @@ def build_rtvd():
     return LIB_RTVD
 
 
+def build_split(name):
+    lib_, src = os.path.join(HERE, "libflopcount_%s.so" % name), os.path.join(HERE, "flop_count_%s.cpp" % name)
+    deps = [src, os.path.join(HERE, name + "_oracle.cpp"), os.path.join(HERE, "flop_scalar.h")]
+    if not os.path.exists(lib_) or any(os.path.getmtime(d) > os.path.getmtime(lib_) for d in deps):
+        subprocess.run(["g++", "-std=c++17", "-O1", "-shared", "-fPIC", "-o", lib_, src], check=True, cwd=HERE)
+    return lib_
+
+
+def count_waf(G, dt, dh, gamma, order=0):
+    L = C.CDLL(build_split("waf"))
+    G = np.ascontiguousarray(G, np.float64)
+    Ng, S = G.shape[0], G.shape[2]
+    c = np.zeros(7, np.int64)
+    L.oracle_waf_count_ops.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
+                                       C.POINTER(C.c_longlong)]
+    L.oracle_waf_count_ops(G.ctypes.data_as(C.POINTER(C.c_double)), Ng, (S - 16) // 2, dt, dh, gamma, order,
+                           c.ctypes.data_as(C.POINTER(C.c_longlong)))
+    cells = Ng * 16 ** 3
+    per = {n: float(v) / cells for n, v in zip(("add", "mul", "div", "sqrt", "pow", "cmp", "abs"), c)}
+    per["flops_per_cell"] = per["add"] + per["mul"] + per["div"] + per["sqrt"] + per["pow"]
+    return per
+
+
 def count_rtvd(G, dt, dh, gamma, order=0):
     L = C.CDLL(build_rtvd())
     G = np.ascontiguousarray(G, np.float64)
@@ -100,6 +123,9 @@ def main():
     out["rtvd_g3"]["_note"] = ("three split sweeps over the oracle's ranges (484 + 352 + 256 pencils of 22 cells per group): "
                                "5.9 cell-sweeps per interior cell update")
     print("rtvd_g3", {k: round(v, 1) for k, v in out["rtvd_g3"].items() if k != "_note"})
+    out["waf_g3"] = count_waf(G, 0.3 * dh / O.hydro_dt(G, gamma, 0), dh, gamma, 0)
+    out["waf_g3"]["_note"] = "three split WAF sweeps over the oracle's ranges (the 22-cell pencils of the RTVD batches): 5.9 cell-sweeps per interior cell update"
+    print("waf_g3", {k: round(v, 1) for k, v in out["waf_g3"].items() if k != "_note"})
     with open(os.path.join(HERE, "flops_per_cell.json"), "w") as f:
         json.dump(out, f, indent=1)
 
