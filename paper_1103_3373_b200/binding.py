@@ -247,7 +247,7 @@ def hydro_rtvd_solve_noalloc(in_, dt, dh, gamma, order=0, *, out, face_flux=None
                                                 in_.shape[0], dt, dh, gamma, order,
                                                 status.data_ptr() if status is not None else None, st)
     if rc != 0:
-        raise HydroError(rc, "hydro_rtvd_solve_noalloc_f64", "hydro_waf_solve_f32", "hydro_waf_solve_f64")
+        raise HydroError(rc, "hydro_rtvd_solve_noalloc_f64")
     return out, face_flux
 
 

@@ -144,7 +144,7 @@ __device__ __forceinline__ void rt_sweep(const R* __restrict__ src, size_t sq, i
 // Everything below works in the NORMAL frame of the sweep: (rho, m_n, m_t1, m_t2, E).
 template <class R> struct WCell { R rho, u, v1, v2, P, c, E; };
 template <class R> struct WJump { R q[3], t1, t2; };                 // jumps across the three waves; tangential momenta across the contact
-template <class R> struct WFace { V5<R> hs, d1, d2, d3; R c[3]; };   // (F_L + F_R)/2, F(k+1) - F(k), Courant numbers
+template <class R> struct WWave { R SL, Ss, SR, rsL, rsR; };           // wave speeds and star densities of one face
 template <class R> __device__ __forceinline__ WCell<R> waf_cell(const V5<R>& U, R gamma, int& bad) {
   WCell<R> w;
   const R ir = m_rcp(U[0]);
@@ -154,37 +154,22 @@ template <class R> __device__ __forceinline__ WCell<R> waf_cell(const V5<R>& U, 
   w.c = m_sqrt(gamma * w.P * ir);
   return w;
 }
-template <class R> __device__ __forceinline__ void waf_face(const WCell<R>& L, const WCell<R>& Rr, R nu, R gamma, WFace<R>& f, WJump<R>& j) {
+// first half of a face: the wave structure and the jumps the limiter looks at (the neighbouring faces need these, not the fluxes)
+template <class R> __device__ __forceinline__ void waf_waves(const WCell<R>& L, const WCell<R>& Rr, R gamma, WWave<R>& w, WJump<R>& j) {
   const R ppv = R(0.5) * (L.P + Rr.P) - R(0.125) * (Rr.u - L.u) * (L.rho + Rr.rho) * (L.c + Rr.c);
   const R ps = m_max(ppv, R(0));
   const R gf = (gamma + R(1)) * m_rcp(gamma + gamma);
   const R qL = ps <= L.P ? R(1) : m_sqrt(R(1) + gf * (m_div(ps, L.P) - R(1)));
   const R qR = ps <= Rr.P ? R(1) : m_sqrt(R(1) + gf * (m_div(ps, Rr.P) - R(1)));
-  const R SL = L.u - L.c * qL, SR = Rr.u + Rr.c * qR;
-  const R mL = L.rho * (SL - L.u), mR = Rr.rho * (SR - Rr.u);
-  const R Ss = m_div((Rr.P - L.P) + L.u * mL - Rr.u * mR, mL - mR);
-  const R rsL = m_div(mL, SL - Ss), rsR = m_div(mR, SR - Ss);  // rho*_K
-  const R EsL = rsL * (m_div(L.E, L.rho) + (Ss - L.u) * (Ss + m_div(L.P, mL)));
-  const R EsR = rsR * (m_div(Rr.E, Rr.rho) + (Ss - Rr.u) * (Ss + m_div(Rr.P, mR)));
-  const R mnL = L.rho * L.u, mnR = Rr.rho * Rr.u;
-  // F*_L - F_L = S_L (U*_L - U_L);  F_R - F*_R = -S_R (U*_R - U_R);  the contact takes the rest of F_R - F_L
-  f.d1[0] = SL * (rsL - L.rho);              f.d3[0] = -SR * (rsR - Rr.rho);
-  f.d1[1] = SL * (rsL * Ss - mnL);           f.d3[1] = -SR * (rsR * Ss - mnR);
-  f.d1[2] = SL * (rsL * L.v1 - L.rho * L.v1); f.d3[2] = -SR * (rsR * Rr.v1 - Rr.rho * Rr.v1);
-  f.d1[3] = SL * (rsL * L.v2 - L.rho * L.v2); f.d3[3] = -SR * (rsR * Rr.v2 - Rr.rho * Rr.v2);
-  f.d1[4] = SL * (EsL - L.E);                f.d3[4] = -SR * (EsR - Rr.E);
-  V5<R> FL, FR;
-  FL[0] = mnL; FL[1] = mnL * L.u + L.P; FL[2] = mnL * L.v1; FL[3] = mnL * L.v2; FL[4] = (L.E + L.P) * L.u;
-  FR[0] = mnR; FR[1] = mnR * Rr.u + Rr.P; FR[2] = mnR * Rr.v1; FR[3] = mnR * Rr.v2; FR[4] = (Rr.E + Rr.P) * Rr.u;
-#pragma unroll
-  for (int q = 0; q < 5; ++q) {
-    f.hs[q] = R(0.5) * (FL[q] + FR[q]);
-    f.d2[q] = ((FR[q] - FL[q]) - f.d1[q]) - f.d3[q];
-  }
-  f.c[0] = nu * SL; f.c[1] = nu * Ss; f.c[2] = nu * SR;
-  j.q[0] = rsL - L.rho; j.q[1] = rsR - rsL; j.q[2] = Rr.rho - rsR;
-  j.t1 = rsR * Rr.v1 - rsL * L.v1;
-  j.t2 = rsR * Rr.v2 - rsL * L.v2;
+  w.SL = L.u - L.c * qL;
+  w.SR = Rr.u + Rr.c * qR;
+  const R mL = L.rho * (w.SL - L.u), mR = Rr.rho * (w.SR - Rr.u);
+  w.Ss = m_div((Rr.P - L.P) + L.u * mL - Rr.u * mR, mL - mR);
+  w.rsL = m_div(mL, w.SL - w.Ss);
+  w.rsR = m_div(mR, w.SR - w.Ss);
+  j.q[0] = w.rsL - L.rho; j.q[1] = w.rsR - w.rsL; j.q[2] = Rr.rho - w.rsR;
+  j.t1 = w.rsR * Rr.v1 - w.rsL * L.v1;
+  j.t2 = w.rsR * Rr.v2 - w.rsL * L.v2;
 }
 template <class R> __device__ __forceinline__ R waf_B(R a, R b) { return a * b > R(0) ? m_div(a + a, a + b) : R(0); }
 // half the signed weight sign(c) A / 2 of one wave for one limiter pair
@@ -192,24 +177,42 @@ template <class R> __device__ __forceinline__ R waf_w(R c, R a, R b) {
   const R sg = c > R(0) ? R(0.5) : (c < R(0) ? R(-0.5) : R(0));
   return sg * (R(1) - (R(1) - m_abs(c)) * waf_B(a, b));
 }
-template <class R> __device__ __forceinline__ V5<R> waf_flux(const WFace<R>& f, const WJump<R>& jl, const WJump<R>& jc, const WJump<R>& ju) {
+// second half: the WAF flux of the face (normal frame) from its cells, its waves, its own jumps jc and those of the lower (jl)
+// and upper (ju) faces.  The region fluxes are formed here and consumed at once, so that only the wave data of a face is carried
+// from step to step of the march
+template <class R> __device__ __forceinline__ V5<R> waf_flux(const WCell<R>& L, const WCell<R>& Rr, const WWave<R>& w, R nu,
+                                                             const WJump<R>& jl, const WJump<R>& jc, const WJump<R>& ju) {
+  const R mL = L.rho * (w.SL - L.u), mR = Rr.rho * (w.SR - Rr.u);
+  const R EsL = w.rsL * (m_div(L.E, L.rho) + (w.Ss - L.u) * (w.Ss + m_div(L.P, mL)));
+  const R EsR = w.rsR * (m_div(Rr.E, Rr.rho) + (w.Ss - Rr.u) * (w.Ss + m_div(Rr.P, mR)));
+  const R mnL = L.rho * L.u, mnR = Rr.rho * Rr.u;
+  V5<R> d1, d3, FL, FR;  // F*_L - F_L = S_L (U*_L - U_L);  F_R - F*_R = -S_R (U*_R - U_R);  the contact takes the rest of F_R - F_L
+  d1[0] = w.SL * (w.rsL - L.rho);                  d3[0] = -w.SR * (w.rsR - Rr.rho);
+  d1[1] = w.SL * (w.rsL * w.Ss - mnL);             d3[1] = -w.SR * (w.rsR * w.Ss - mnR);
+  d1[2] = w.SL * (w.rsL * L.v1 - L.rho * L.v1);    d3[2] = -w.SR * (w.rsR * Rr.v1 - Rr.rho * Rr.v1);
+  d1[3] = w.SL * (w.rsL * L.v2 - L.rho * L.v2);    d3[3] = -w.SR * (w.rsR * Rr.v2 - Rr.rho * Rr.v2);
+  d1[4] = w.SL * (EsL - L.E);                      d3[4] = -w.SR * (EsR - Rr.E);
+  FL[0] = mnL; FL[1] = mnL * L.u + L.P; FL[2] = mnL * L.v1; FL[3] = mnL * L.v2; FL[4] = (L.E + L.P) * L.u;
+  FR[0] = mnR; FR[1] = mnR * Rr.u + Rr.P; FR[2] = mnR * Rr.v1; FR[3] = mnR * Rr.v2; FR[4] = (Rr.E + Rr.P) * Rr.u;
+  const R c0 = nu * w.SL, c1 = nu * w.Ss, c2 = nu * w.SR;
   // upwind jumps of the three waves (selected by value: a run-time choice between two structs would put them in local memory)
-  const bool p0 = f.c[0] > R(0), p1 = f.c[1] > R(0), p2 = f.c[2] > R(0);
-  const R w0 = waf_w(f.c[0], p0 ? jl.q[0] : ju.q[0], jc.q[0]), w2 = waf_w(f.c[2], p2 ? jl.q[2] : ju.q[2], jc.q[2]);
-  const R w1 = waf_w(f.c[1], p1 ? jl.q[1] : ju.q[1], jc.q[1]);
-  const R w1a = waf_w(f.c[1], p1 ? jl.t1 : ju.t1, jc.t1), w1b = waf_w(f.c[1], p1 ? jl.t2 : ju.t2, jc.t2);
+  const bool p0 = c0 > R(0), p1 = c1 > R(0), p2 = c2 > R(0);
+  const R w0 = waf_w(c0, p0 ? jl.q[0] : ju.q[0], jc.q[0]), w2 = waf_w(c2, p2 ? jl.q[2] : ju.q[2], jc.q[2]);
+  const R w1 = waf_w(c1, p1 ? jl.q[1] : ju.q[1], jc.q[1]);
+  const R w1a = waf_w(c1, p1 ? jl.t1 : ju.t1, jc.t1), w1b = waf_w(c1, p1 ? jl.t2 : ju.t2, jc.t2);
+  const R wk[5] = {w1, w1, w1a, w1b, w1};
   V5<R> H;
-  H[0] = ((f.hs[0] - w0 * f.d1[0]) - w1 * f.d2[0]) - w2 * f.d3[0];
-  H[1] = ((f.hs[1] - w0 * f.d1[1]) - w1 * f.d2[1]) - w2 * f.d3[1];
-  H[2] = ((f.hs[2] - w0 * f.d1[2]) - w1a * f.d2[2]) - w2 * f.d3[2];
-  H[3] = ((f.hs[3] - w0 * f.d1[3]) - w1b * f.d2[3]) - w2 * f.d3[3];
-  H[4] = ((f.hs[4] - w0 * f.d1[4]) - w1 * f.d2[4]) - w2 * f.d3[4];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    const R d2 = ((FR[q] - FL[q]) - d1[q]) - d3[q];
+    H[q] = ((R(0.5) * (FL[q] + FR[q]) - w0 * d1[q]) - wk[q] * d2) - w2 * d3[q];
+  }
   return H;
 }
 
 // One WAF sweep along D: same pencil geometry and arguments as rt_sweep (cells 3 .. 18 of the 22-cell pencil are updated, the
-// scheme itself needs two of the three ghost cells).  Register windows: the cells x-1, x (primitives), the faces x-1, x
-// (flux data), the jumps of the faces x-2, x-1, x, the fluxes of the faces x-2, x-1; unrolled by their common period six.
+// scheme itself needs two of the three ghost cells).  Register windows: the cells x-2, x-1, x (primitives), the wave data of the
+// faces x-1, x, the jumps of the faces x-2, x-1, x, the fluxes of the faces x-2, x-1; unrolled by their common period six.
 template <int D, class R, int NT = RT_NT>
 __device__ __forceinline__ void waf_sweep(const R* __restrict__ src, size_t sq, int sa, int sb, int sx, R* __restrict__ dst, size_t dq,
                                           int da, int db, int dx, int na, int nb, int fa0, int fb0, R* __restrict__ ff, R nu, R gamma,
@@ -221,8 +224,8 @@ __device__ __forceinline__ void waf_sweep(const R* __restrict__ src, size_t sq, 
     R* d = dst + (size_t)a * da + (size_t)b * db;
     const int ta = a - fa0, tb = b - fb0;
     R* fp = (ff && ta >= 0 && ta < PS && tb >= 0 && tb < PS) ? ff + tb * PS + ta : nullptr;
-    WCell<R> cw[2];
-    WFace<R> fw[2];
+    WCell<R> cw[3];
+    WWave<R> ww[2];
     WJump<R> jw[3];
     V5<R> Hw[2], Unext;
 #pragma unroll
@@ -239,10 +242,10 @@ __device__ __forceinline__ void waf_sweep(const R* __restrict__ src, size_t sq, 
 #pragma unroll
             for (int q = 0; q < 5; ++q) Unext[q] = s[q * sq + (size_t)(x + 1) * sx];
           }
-          cw[u & 1] = waf_cell(Un, gamma, bad);
-          if (x >= 1) waf_face(cw[(u + 1) & 1], cw[u & 1], nu, gamma, fw[u & 1], jw[u % 3]);  // face x, between cells x-1 and x
-          if (x >= 4 && x <= RT_W - 2) {  // flux of face f = x-1 in 3 .. 19: jumps of the faces x-2, x-1, x
-            const V5<R> Hn = waf_flux(fw[(u + 1) & 1], jw[(u + 1) % 3], jw[(u + 2) % 3], jw[u % 3]);
+          cw[u % 3] = waf_cell(Un, gamma, bad);
+          if (x >= 1) waf_waves(cw[(u + 2) % 3], cw[u % 3], gamma, ww[u & 1], jw[u % 3]);  // face x, between cells x-1 and x
+          if (x >= 4 && x <= RT_W - 2) {  // flux of face f = x-1 in 3 .. 19 (cells x-2, x-1): jumps of the faces x-2, x-1, x
+            const V5<R> Hn = waf_flux(cw[(u + 1) % 3], cw[(u + 2) % 3], ww[(u + 1) & 1], nu, jw[(u + 1) % 3], jw[(u + 2) % 3], jw[u % 3]);
             V5<R>& H = Hw[u & 1];
             H[0] = Hn[0]; H[QN] = Hn[1]; H[QT1] = Hn[2]; H[QT2] = Hn[3]; H[4] = Hn[4];
             const int f = x - 1 - RT_G;  // face index of the group: 0 .. 16
@@ -318,9 +321,12 @@ rtvd_kernel(const R* __restrict__ in, R* __restrict__ out, R* __restrict__ face_
 // writes `out`: no scratch, no intermediate traffic, no long-scoreboard stalls on L2 (the scratch kernel above spends 3.2 of its
 // 6.9 stall cycles per instruction there).  The x sweep reads with a stride of 22 floats between lanes: two-way bank conflicts.
 constexpr int RT_SNT = 512;
+#ifndef WAF_SNT
+#define WAF_SNT 256
+#endif
 constexpr size_t RT_SMEM = 64 + 5 * (size_t)RT_W * RT_W * RT_W * sizeof(float);
-template <int SCHEME>
-__global__ void __launch_bounds__(RT_SNT, 1)
+template <int SCHEME, int SNT>
+__global__ void __launch_bounds__(SNT, 1)
 rtvd_smem_kernel(const float* __restrict__ in, float* __restrict__ out, float* __restrict__ face_flux, int Ng, float nu_arg, float gamma,
                  int order, const float* __restrict__ max_speed, float cfl, long long* status) {
   using R = float;
@@ -354,22 +360,22 @@ rtvd_smem_kernel(const float* __restrict__ in, float* __restrict__ out, float* _
     R* fx = gff, *fy = gff ? gff + 3 * 5 * PS * PS : nullptr, *fz = gff ? gff + 6 * 5 * PS * PS : nullptr;
     if (order == 0) {
       // x: pencils (j, k) of the box, in place;  y: pencils (i interior, k);  z: pencils (i, j) interior -> out
-      split_sweep<SCHEME, 0, R, RT_SNT>(box, W3, W, W2, 1, box + RT_G, W3, W, W2, 1, W, W, RT_G, RT_G, fx, nu, gamma, bad);
+      split_sweep<SCHEME, 0, R, SNT>(box, W3, W, W2, 1, box + RT_G, W3, W, W2, 1, W, W, RT_G, RT_G, fx, nu, gamma, bad);
       __syncthreads();
-      split_sweep<SCHEME, 1, R, RT_SNT>(box + RT_G, W3, 1, W2, W, box + RT_G + RT_G * W, W3, 1, W2, W, PS, W, 0, RT_G, fy, nu, gamma, bad);
+      split_sweep<SCHEME, 1, R, SNT>(box + RT_G, W3, 1, W2, W, box + RT_G + RT_G * W, W3, 1, W2, W, PS, W, 0, RT_G, fy, nu, gamma, bad);
       __syncthreads();
-      split_sweep<SCHEME, 2, R, RT_SNT>(box + RT_G + RT_G * W, W3, 1, W, W2, gout, NI, 1, PS, PS * PS, PS, PS, 0, 0, fz, nu, gamma, bad);
+      split_sweep<SCHEME, 2, R, SNT>(box + RT_G + RT_G * W, W3, 1, W, W2, gout, NI, 1, PS, PS * PS, PS, PS, 0, 0, fz, nu, gamma, bad);
     } else {
       // z: pencils (i, j) of the box, in place;  y: pencils (i, k interior);  x: pencils (j, k) interior -> out
-      split_sweep<SCHEME, 2, R, RT_SNT>(box, W3, 1, W, W2, box + RT_G * W2, W3, 1, W, W2, W, W, RT_G, RT_G, fz, nu, gamma, bad);
+      split_sweep<SCHEME, 2, R, SNT>(box, W3, 1, W, W2, box + RT_G * W2, W3, 1, W, W2, W, W, RT_G, RT_G, fz, nu, gamma, bad);
       __syncthreads();
-      split_sweep<SCHEME, 1, R, RT_SNT>(box + RT_G * W2, W3, 1, W2, W, box + RT_G * W2 + RT_G * W, W3, 1, W2, W, W, PS, RT_G, 0, fy, nu, gamma, bad);
+      split_sweep<SCHEME, 1, R, SNT>(box + RT_G * W2, W3, 1, W2, W, box + RT_G * W2 + RT_G * W, W3, 1, W2, W, W, PS, RT_G, 0, fy, nu, gamma, bad);
       __syncthreads();
       // the x sweep comes last here: written straight to `out` its lanes (pencils j) would store 64 bytes apart, so it also runs
       // in place and the interior leaves the box in a coalesced copy
-      split_sweep<SCHEME, 0, R, RT_SNT>(box + RT_G * W2 + RT_G * W, W3, W, W2, 1, box + RT_G * W2 + RT_G * W + RT_G, W3, W, W2, 1, PS, PS, 0, 0, fx, nu, gamma, bad);
+      split_sweep<SCHEME, 0, R, SNT>(box + RT_G * W2 + RT_G * W, W3, W, W2, 1, box + RT_G * W2 + RT_G * W + RT_G, W3, W, W2, 1, PS, PS, 0, 0, fx, nu, gamma, bad);
       __syncthreads();
-      for (int idx = threadIdx.x; idx < 5 * (int)NI; idx += RT_SNT) {
+      for (int idx = threadIdx.x; idx < 5 * (int)NI; idx += SNT) {
         const int q = idx >> 12, c = idx & 4095, k = c >> 8, j = (c >> 4) & 15, i = c & 15;
         gout[idx] = box[q * W3 + (k + RT_G) * W2 + (j + RT_G) * W + (i + RT_G)];
       }
@@ -406,12 +412,15 @@ static int rtvd_impl(const R* in, R* out, R* ff, int Ng, R dt, R dh, R gamma, in
         cudaGetDevice(&dev);
         if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
       }
-      auto kern = scheme == SPLIT_WAF ? rtvd_smem_kernel<SPLIT_WAF> : rtvd_smem_kernel<SPLIT_RTVD>;
+      // RTVD: 512 threads (one pass over the 484 pencils of the first sweep, 124 registers).  WAF holds more per pencil: WAF_SNT
+      // threads leave it the registers it needs
+      auto kern = scheme == SPLIT_WAF ? rtvd_smem_kernel<SPLIT_WAF, WAF_SNT> : rtvd_smem_kernel<SPLIT_RTVD, RT_SNT>;
+      const int nt = scheme == SPLIT_WAF ? WAF_SNT : RT_SNT;
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RT_SMEM);
       if (e != cudaSuccess) return (int)e;
-      kern<<<(unsigned)(Ng < sms ? Ng : sms), RT_SNT, RT_SMEM, st>>>(in, out, ff, Ng, device_dt ? 0.f : dt / dh, gamma, order,
-                                                                              device_dt ? static_cast<const float*>(o->max_speed) : nullptr,
-                                                                              device_dt ? (float)o->cfl : 0.f, o ? o->status : nullptr);
+      kern<<<(unsigned)(Ng < sms ? Ng : sms), nt, RT_SMEM, st>>>(in, out, ff, Ng, device_dt ? 0.f : dt / dh, gamma, order,
+                                                                 device_dt ? static_cast<const float*>(o->max_speed) : nullptr,
+                                                                 device_dt ? (float)o->cfl : 0.f, o ? o->status : nullptr);
       return (int)cudaGetLastError();
     }
   }
